@@ -1,0 +1,149 @@
+"""CPU fp64 oracle for the Tropical multiplexed iteration -- TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It never imports
+``paper_2606_16264_b200`` and shares no code with it.  The arithmetic is in
+``tropical_oracle.c`` (plain C, fp64); this file only marshals numpy arrays through ctypes.
+
+Citations: PAPER.md:143, :159 (the multiplexed iteration), BASELINE.json north_star (the
+attention definition and tolerances), SURVEY.md section 8(c) (readings S1-S28).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tropical_oracle.c")
+_LIB = os.path.join(_HERE, "libtropical_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile tropical_oracle.c -> libtropical_oracle.so (gcc, OpenMP, no fast-math)."""
+    if force or (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.oracle_num_threads.restype = ctypes.c_int
+        _lib.oracle_attention_rows.restype = ctypes.c_int
+        _lib.oracle_mixed_attention.restype = ctypes.c_int
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _u16(a) -> np.ndarray:
+    a = np.asarray(a)
+    assert a.dtype == np.uint16 and a.flags.c_contiguous, "bf16 tensors are passed as contiguous uint16"
+    return a
+
+
+def kv_append(k_pool, v_pool, q_lens, ctx_lens, q_offsets, page_table, k_new, v_new) -> None:
+    """In-place append of this step's K/V rows into the pools (tropical_oracle.c: oracle_kv_append)."""
+    k_pool, v_pool, k_new, v_new = _u16(k_pool), _u16(v_pool), _u16(k_new), _u16(v_new)
+    assert k_pool.flags.writeable and v_pool.flags.writeable
+    _, Hkv, P, d = k_pool.shape
+    q_lens, ctx_lens, q_offsets, page_table = _i32(q_lens), _i32(ctx_lens), _i32(q_offsets), _i32(page_table)
+    _load().oracle_kv_append(
+        ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(P), ctypes.c_int(q_lens.shape[0]),
+        _p(q_lens), _p(ctx_lens), _p(q_offsets), _p(page_table), ctypes.c_int(page_table.shape[1]),
+        _p(k_pool), _p(v_pool), _p(k_new), _p(v_new))
+
+
+def kv_gather(k_pool, v_pool, page_table, req: int, n_keys: int) -> Tuple[np.ndarray, np.ndarray]:
+    """Dense bf16 copy-out [n_keys, Hkv, d] of request req's first n_keys keys/values."""
+    k_pool, v_pool = _u16(k_pool), _u16(v_pool)
+    _, Hkv, P, d = k_pool.shape
+    page_table = _i32(page_table)
+    kd = np.empty((n_keys, Hkv, d), np.uint16)
+    vd = np.empty((n_keys, Hkv, d), np.uint16)
+    _load().oracle_kv_gather(
+        ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(P), _p(page_table),
+        ctypes.c_int(page_table.shape[1]), ctypes.c_int(req), ctypes.c_int(n_keys),
+        _p(k_pool), _p(v_pool), _p(kd), _p(vd))
+    return kd, vd
+
+
+def attention_rows(k_pool, v_pool, q, q_lens, ctx_lens, q_offsets, page_table,
+                   rows: Sequence[Tuple[int, int]], sm_scale: float = 0.0, want_wsum: bool = False):
+    """fp64 attention for chosen (request, new-token index) rows; all q heads of each row.
+
+    Returns (out [n, Hq, d] f64, lse [n, Hq] f64[, wsum [n, Hq] f64])."""
+    k_pool, v_pool, q = _u16(k_pool), _u16(v_pool), _u16(q)
+    _, Hkv, P, d = k_pool.shape
+    Hq = q.shape[1]
+    q_lens, ctx_lens, q_offsets, page_table = _i32(q_lens), _i32(ctx_lens), _i32(q_offsets), _i32(page_table)
+    rows = list(rows)
+    n = len(rows)
+    row_req = _i32([r for r, _ in rows])
+    row_t = _i32([t for _, t in rows])
+    for r, t in rows:
+        assert 0 <= r < q_lens.shape[0] and 0 <= t < q_lens[r], (r, t)
+    out = np.zeros((n, Hq, d), np.float64)
+    lse = np.zeros((n, Hq), np.float64)
+    wsum = np.zeros((n, Hq), np.float64) if want_wsum else None
+    rc = _load().oracle_attention_rows(
+        ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(P),
+        _p(q_lens), _p(ctx_lens), _p(q_offsets), _p(page_table), ctypes.c_int(page_table.shape[1]),
+        _p(k_pool), _p(v_pool), _p(q), ctypes.c_double(sm_scale), ctypes.c_int(n),
+        _p(row_req), _p(row_t), _p(out), _p(lse), _p(wsum))
+    if rc != 0:
+        raise MemoryError("oracle scratch allocation failed")
+    return (out, lse, wsum) if want_wsum else (out, lse)
+
+
+def mixed_attention(k_pool, v_pool, q, q_lens, ctx_lens, q_offsets, page_table,
+                    sm_scale: float = 0.0, want_wsum: bool = False):
+    """fp64 attention for every row of the step (pools must already hold this step's rows).
+
+    Returns (out [T, Hq, d] f64, lse [T, Hq] f64[, wsum])."""
+    k_pool, v_pool, q = _u16(k_pool), _u16(v_pool), _u16(q)
+    _, Hkv, P, d = k_pool.shape
+    T, Hq = q.shape[0], q.shape[1]
+    q_lens, ctx_lens, q_offsets, page_table = _i32(q_lens), _i32(ctx_lens), _i32(q_offsets), _i32(page_table)
+    assert int(q_offsets[-1]) == T
+    out = np.zeros((T, Hq, d), np.float64)
+    lse = np.zeros((T, Hq), np.float64)
+    wsum = np.zeros((T, Hq), np.float64) if want_wsum else None
+    rc = _load().oracle_mixed_attention(
+        ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(P), ctypes.c_int(q_lens.shape[0]),
+        _p(q_lens), _p(ctx_lens), _p(q_offsets), _p(page_table), ctypes.c_int(page_table.shape[1]),
+        _p(k_pool), _p(v_pool), _p(q), ctypes.c_double(sm_scale), _p(out), _p(lse), _p(wsum))
+    if rc != 0:
+        raise MemoryError("oracle scratch allocation failed")
+    return (out, lse, wsum) if want_wsum else (out, lse)
+
+
+def step(inputs, sm_scale: float = 0.0):
+    """Whole step on a synth.StepInputs: append into COPIES of the pools, then attend.
+
+    Returns (out f64 [T,Hq,d], lse f64 [T,Hq], k_pool_after, v_pool_after)."""
+    kp, vp = inputs.copy_pools()
+    kv_append(kp, vp, inputs.q_lens, inputs.ctx_lens, inputs.q_offsets, inputs.page_table,
+              inputs.k_new, inputs.v_new)
+    out, lse = mixed_attention(kp, vp, inputs.q, inputs.q_lens, inputs.ctx_lens, inputs.q_offsets,
+                               inputs.page_table, sm_scale)
+    return out, lse, kp, vp

@@ -1,0 +1,207 @@
+/*
+ * tropical_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU fp64 definition of what one multiplexed worker
+ * iteration computes (PAPER.md:143, :159 -- a prefill chunk co-run with the decode batch of
+ * one worker; the paper inherits the attention itself from its vLLM/PagedAttention substrate,
+ * PAPER.md:182, :224, :246).  BASELINE.json north_star fixes the definition:
+ * "softmax(QK^T/sqrt(d) + causal mask)V over gathered pages", fp64, after the KV append.
+ * SURVEY.md section 8(c) restates it with the readings S1-S28; DESIGN.md lists them.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may build, load or call this file.  It shares no code with paper_2606_16264_b200/.
+ *
+ * The GPU path reaches exactly this result by re-association (tiling, online softmax,
+ * split-K, paging), so the oracle is the definition written out -- no blocking, no fusion,
+ * no online softmax.  Every score of a row is materialised, then max, then sum, then the
+ * weighted sum over values.
+ *
+ * Pins (tests/test_oracle_pins.py): brute-force dense attention, torch fp64 SDPA, closed
+ * forms, row-sum-to-one, page-size and page-permutation invariance, chunk/decode
+ * consistency, needle selection.  Step-cost model: not in this file (parity unpinned, see
+ * DESIGN.md).
+ *
+ * Layouts (host pointers, bf16 carried as uint16 bit patterns):
+ *   q            [T][Hq][d]           k_new, v_new [T][Hkv][d]
+ *   k_pool/v_pool [num_pages][Hkv][P][d]
+ *   page_table   [num_reqs][stride]   q_lens, ctx_lens [num_reqs]   q_offsets [num_reqs+1]
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+static inline double bf16_to_double(uint16_t b)
+{
+    uint32_t u = ((uint32_t)b) << 16; /* bf16 is the top half of an IEEE binary32 */
+    float f;
+    memcpy(&f, &u, sizeof f);
+    return (double)f;
+}
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* Phase 1 -- KV append (reading S4 "append-all then attend").
+ * for t < q_i: pos = c_i + t; page = page_table[i][pos / P]; slot = pos % P;
+ * pool[page][h][slot][:] = new[q_off_i + t][h][:]   -- raw 16-bit copies, no FP. */
+void oracle_kv_append(int Hkv, int d, int P, int num_reqs, const int32_t *q_lens,
+                      const int32_t *ctx_lens, const int32_t *q_offsets,
+                      const int32_t *page_table, int stride, uint16_t *k_pool, uint16_t *v_pool,
+                      const uint16_t *k_new, const uint16_t *v_new)
+{
+    for (int i = 0; i < num_reqs; ++i) {
+        for (int t = 0; t < q_lens[i]; ++t) {
+            int64_t pos = (int64_t)ctx_lens[i] + t;
+            int64_t page = page_table[(int64_t)i * stride + pos / P];
+            int64_t slot = pos % P;
+            for (int h = 0; h < Hkv; ++h) {
+                int64_t dst = ((page * Hkv + h) * P + slot) * d;
+                int64_t src = (((int64_t)q_offsets[i] + t) * Hkv + h) * d;
+                for (int c = 0; c < d; ++c) {
+                    k_pool[dst + c] = k_new[src + c];
+                    v_pool[dst + c] = v_new[src + c];
+                }
+            }
+        }
+    }
+}
+
+/* Page gather (row A2): logical key j of request i -> (page_table[i][j / P], j % P).
+ * Dense copy-out of the first n_keys keys of request req: k_dense/v_dense [n_keys][Hkv][d]. */
+void oracle_kv_gather(int Hkv, int d, int P, const int32_t *page_table, int stride, int req,
+                      int n_keys, const uint16_t *k_pool, const uint16_t *v_pool,
+                      uint16_t *k_dense, uint16_t *v_dense)
+{
+    for (int j = 0; j < n_keys; ++j) {
+        int64_t page = page_table[(int64_t)req * stride + j / P];
+        int64_t slot = j % P;
+        for (int h = 0; h < Hkv; ++h) {
+            int64_t src = ((page * Hkv + h) * P + slot) * d;
+            int64_t dst = ((int64_t)j * Hkv + h) * d;
+            for (int c = 0; c < d; ++c) {
+                k_dense[dst + c] = k_pool[src + c];
+                v_dense[dst + c] = v_pool[src + c];
+            }
+        }
+    }
+}
+
+/* One (request i, new-token t, q-head hq) row of phase 2 (rows A3/A4/A5 all compute this):
+ *   hk = hq / (Hq/Hkv)                        (S6: contiguous GQA groups)
+ *   n  = c_i + t + 1                          (S3: causal, bottom-right aligned; S4: sees itself)
+ *   s_j = scale * sum_c q[c] * K_j[c]         j in [0, n)
+ *   m = max_j s_j;  Z = sum_j exp(s_j - m);   w_j = exp(s_j - m) / Z
+ *   out[c] = sum_j w_j * V_j[c];              lse = m + log Z;   wsum = sum_j w_j
+ * scratch s: n doubles. */
+static void attention_row(int Hq, int Hkv, int d, int P, const int32_t *ctx_lens,
+                          const int32_t *q_offsets, const int32_t *page_table, int stride,
+                          const uint16_t *k_pool, const uint16_t *v_pool, const uint16_t *q,
+                          double scale, int i, int t, int hq, double *s, double *out, double *lse,
+                          double *wsum)
+{
+    const int g = Hq / Hkv;
+    const int hk = hq / g;
+    const int64_t n = (int64_t)ctx_lens[i] + t + 1;
+    const uint16_t *qrow = q + (((int64_t)q_offsets[i] + t) * Hq + hq) * d;
+    const int32_t *pt = page_table + (int64_t)i * stride;
+
+    for (int64_t j = 0; j < n; ++j) {
+        const uint16_t *krow = k_pool + (((int64_t)pt[j / P] * Hkv + hk) * P + j % P) * d;
+        double acc = 0.0;
+        for (int c = 0; c < d; ++c) acc += bf16_to_double(qrow[c]) * bf16_to_double(krow[c]);
+        s[j] = scale * acc;
+    }
+    double m = s[0];
+    for (int64_t j = 1; j < n; ++j) m = s[j] > m ? s[j] : m;
+    double Z = 0.0;
+    for (int64_t j = 0; j < n; ++j) Z += exp(s[j] - m);
+    for (int c = 0; c < d; ++c) out[c] = 0.0;
+    double ws = 0.0;
+    for (int64_t j = 0; j < n; ++j) {
+        const uint16_t *vrow = v_pool + (((int64_t)pt[j / P] * Hkv + hk) * P + j % P) * d;
+        double w = exp(s[j] - m) / Z;
+        ws += w;
+        for (int c = 0; c < d; ++c) out[c] += w * bf16_to_double(vrow[c]);
+    }
+    if (lse) *lse = m + log(Z);
+    if (wsum) *wsum = ws;
+}
+
+/* Phase 2 on a chosen subset of rows: row r is (row_req[r], row_t[r]) with 0 <= t < q_lens[req].
+ * out [n_rows][Hq][d], lse (nullable) [n_rows][Hq], wsum (nullable) [n_rows][Hq].
+ * scale <= 0 selects 1/sqrt(d) (S2).  Returns 0, or -1 if scratch allocation failed. */
+int oracle_attention_rows(int Hq, int Hkv, int d, int P, const int32_t *q_lens,
+                          const int32_t *ctx_lens, const int32_t *q_offsets,
+                          const int32_t *page_table, int stride, const uint16_t *k_pool,
+                          const uint16_t *v_pool, const uint16_t *q, double scale, int n_rows,
+                          const int32_t *row_req, const int32_t *row_t, double *out, double *lse,
+                          double *wsum)
+{
+    (void)q_lens;
+    if (!(scale > 0.0)) scale = 1.0 / sqrt((double)d);
+    int64_t max_n = 1;
+    for (int r = 0; r < n_rows; ++r) {
+        int64_t n = (int64_t)ctx_lens[row_req[r]] + row_t[r] + 1;
+        if (n > max_n) max_n = n;
+    }
+    int failed = 0;
+#pragma omp parallel
+    {
+        double *s = (double *)malloc(sizeof(double) * (size_t)max_n);
+        if (!s) {
+#pragma omp atomic write
+            failed = 1;
+        }
+#pragma omp for collapse(2) schedule(dynamic, 4)
+        for (int r = 0; r < n_rows; ++r) {
+            for (int hq = 0; hq < Hq; ++hq) {
+                if (!s) continue;
+                int64_t o = (int64_t)r * Hq + hq;
+                attention_row(Hq, Hkv, d, P, ctx_lens, q_offsets, page_table, stride, k_pool,
+                              v_pool, q, scale, row_req[r], row_t[r], hq, s, out + o * d,
+                              lse ? lse + o : 0, wsum ? wsum + o : 0);
+            }
+        }
+        free(s);
+    }
+    return failed ? -1 : 0;
+}
+
+/* Phase 2 on every row of the step: out [T][Hq][d], lse/wsum (nullable) [T][Hq]. */
+int oracle_mixed_attention(int Hq, int Hkv, int d, int P, int num_reqs, const int32_t *q_lens,
+                           const int32_t *ctx_lens, const int32_t *q_offsets,
+                           const int32_t *page_table, int stride, const uint16_t *k_pool,
+                           const uint16_t *v_pool, const uint16_t *q, double scale, double *out,
+                           double *lse, double *wsum)
+{
+    int64_t T = q_offsets[num_reqs];
+    if (T == 0) return 0;
+    int32_t *row_req = (int32_t *)malloc(sizeof(int32_t) * (size_t)T);
+    int32_t *row_t = (int32_t *)malloc(sizeof(int32_t) * (size_t)T);
+    if (!row_req || !row_t) {
+        free(row_req);
+        free(row_t);
+        return -1;
+    }
+    for (int i = 0; i < num_reqs; ++i)
+        for (int t = 0; t < q_lens[i]; ++t) {
+            row_req[q_offsets[i] + t] = i;
+            row_t[q_offsets[i] + t] = t;
+        }
+    int rc = oracle_attention_rows(Hq, Hkv, d, P, q_lens, ctx_lens, q_offsets, page_table, stride,
+                                   k_pool, v_pool, q, scale, (int)T, row_req, row_t, out, lse, wsum);
+    free(row_req);
+    free(row_t);
+    return rc;
+}
