@@ -1,0 +1,172 @@
+/*
+ * tropical.h -- C-ABI boundary of the B200-native multiplexed-iteration hot path.
+ *
+ * What is computed (citations: P:n = /root/reference/PAPER.md line n; BJ = BASELINE.json):
+ *   Tropical's SLO-aware multiplexing co-schedules, in ONE worker iteration, a prefill (chunk)
+ *   with the running decode batch.  The iteration's attention over the
+ *   paged KV cache and the KV append are inherited from the substrate and
+ *   defined by BJ:north_star: append this step's K/V rows into the paged bf16 pool, then
+ *   out = softmax(Q K^T / sqrt(d) + causal mask) V over the gathered pages, bf16 in,
+ *   fp32 accumulate, bf16 out.  The execution-time predictor the scheduler needs (P:143,
+ *   P:157) is tropical_step_cost.
+ *
+ * Notation: request i has q_i new tokens this step (1 = decode token, >= 2 = prefill chunk,
+ * 0 = skipped), c_i tokens already cached, L_i = c_i + q_i.  T = sum_i q_i.
+ * Query row t of request i sees keys j <= c_i + t (causal, bottom-right aligned; it sees
+ * itself).  GQA: q head hq reads kv head hq / (Hq/Hkv).
+ *
+ * General conventions
+ *   - All pointers marked [device] are CUDA device pointers, [host] are host pointers.
+ *   - bf16 tensors are raw 16-bit patterns (void*), row-major in the stated shape.
+ *   - The library owns nothing: it allocates no device memory, frees nothing and keeps no
+ *     pointer after a call returns.  Process-global state: cached device attributes,
+ *     one-time cudaFuncSetAttribute, the resolved cuTensorMapEncodeTiled entry point.
+ *   - Device work is enqueued on the caller's stream (void* = cudaStream_t, NULL = legacy
+ *     default stream).  No host synchronisation, no H2D/D2H inside the device-pointer calls;
+ *     they are CUDA-graph capturable.  tropical_step_host is the exception (see there).
+ *   - Return value: tropical_status_t as int, never an exception or abort.  Host-visible
+ *     argument errors are detected before any launch.  CONTENTS of device arrays cannot be
+ *     validated without a sync: out-of-range page ids, q_offsets inconsistent with q_lens, or
+ *     two requests writing the same (page, slot) in one step are UNDEFINED BEHAVIOUR.
+ *     Read-sharing of prior-context pages between requests is allowed.
+ *   - There is no CPU fallback.  Without a CUDA device every device call returns
+ *     TROPICAL_ERR_CUDA.
+ */
+#ifndef TROPICAL_H_
+#define TROPICAL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TROPICAL_OK = 0,
+    TROPICAL_ERR_INVALID_ARG = 1,  /* null pointer, negative size, Hq % Hkv != 0, stride too small */
+    TROPICAL_ERR_UNSUPPORTED = 2,  /* head_dim not in {64,128}, page_size != 16, Hq/Hkv > 64 */
+    TROPICAL_ERR_WORKSPACE = 3,    /* workspace NULL / misaligned (256 B) / smaller than tropical_workspace_bytes */
+    TROPICAL_ERR_CUDA = 4,         /* launch or runtime failure; see tropical_last_cuda_error */
+    TROPICAL_ERR_UNCALIBRATED = 5  /* tropical_step_cost: no coefficients for this head shape */
+} tropical_status_t;
+
+/* Paged KV pool, caller-owned.  Layout "HND": one (page, kv_head) is a contiguous
+ * page_size x head_dim bf16 block (4 KiB at d = 128), so a page-head is one TMA box and the
+ * append scatters 2*d-byte rows.  K and V are separate allocations, 256-byte aligned. */
+typedef struct {
+    int32_t num_q_heads;   /* Hq  */
+    int32_t num_kv_heads;  /* Hkv, divides Hq */
+    int32_t head_dim;      /* d in {64, 128} */
+    int32_t page_size;     /* P = 16 */
+    int32_t num_pages;     /* pool capacity in pages */
+    void *k_pool;          /* [device] bf16 [num_pages][Hkv][P][d] */
+    void *v_pool;          /* [device] bf16 [num_pages][Hkv][P][d] */
+} tropical_kv_pool_t;
+
+/* One multiplexed iteration.  Host scalars are used for validation, grid and
+ * workspace sizing; per-request arrays live on the device so a step needs no sync. */
+typedef struct {
+    int32_t num_reqs;           /* >= 0 */
+    int32_t total_q;            /* T == sum(q_lens): rows of q / out / k_new / v_new */
+    int32_t max_kv_len;         /* >= max_i (ctx_lens[i] + q_lens[i]) */
+    int32_t page_table_stride;  /* >= ceil(max_kv_len / P) */
+    const int32_t *q_lens;      /* [device] [num_reqs]   new tokens: 1 decode, >= 2 prefill chunk, 0 skip */
+    const int32_t *ctx_lens;    /* [device] [num_reqs]   tokens cached BEFORE this step (never mutated) */
+    const int32_t *q_offsets;   /* [device] [num_reqs+1] exclusive prefix sum of q_lens */
+    const int32_t *page_table;  /* [device] [num_reqs][page_table_stride]; entries past ceil(L_i/P) are ignored */
+} tropical_batch_t;
+
+/* Row A1 of SURVEY.md 8(a): for t < q_i, pos = c_i + t:
+ *   k_pool[page_table[i][pos / P]][h][pos % P][:] = k_new[q_offsets[i] + t][h][:]  (same for V).
+ * Bit copy, no floating point.  k_new / v_new: [device] bf16 [T][Hkv][d].  One launch. */
+int tropical_kv_append(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
+                       const void *k_new, const void *v_new, void *cuda_stream);
+
+/* Row A2 as a standalone check / migration building block: dense copy-out of the first n_keys
+ * keys of request req through the page table: k_dense, v_dense [device] bf16 [n_keys][Hkv][d]. */
+int tropical_kv_gather(const tropical_kv_pool_t *pool, const tropical_batch_t *batch, int32_t req,
+                       int32_t n_keys, void *k_dense, void *v_dense, void *cuda_stream);
+
+/* Upper bound of the scratch tropical_mixed_attention needs for any batch with these host
+ * scalars (work lists, split-K partials, tickets).  Returns 0 on invalid arguments. */
+size_t tropical_workspace_bytes(const tropical_kv_pool_t *pool, int32_t num_reqs, int32_t total_q,
+                                int32_t max_kv_len);
+
+/* Rows A0, A2-A5: attention of every new token over its request's pages (which must already
+ * contain this step's rows: call tropical_kv_append first on the same stream).
+ *   q    [device] bf16 [T][Hq][d]      out [device] bf16 [T][Hq][d]
+ *   lse  [device, nullable] fp32 [T][Hq], natural-log sum-exp of the scaled scores
+ *   sm_scale <= 0 selects 1/sqrt(d)
+ *   workspace [device] 256-byte aligned, >= tropical_workspace_bytes(...); contents are scratch.
+ * Never writes the pool.  Unused slots of a request's last page may hold any bits (NaN
+ * included); the result does not depend on them.  Run-to-run deterministic. */
+int tropical_mixed_attention(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
+                             const void *q, void *out, float *lse, float sm_scale,
+                             void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* End-to-end step from HOST buffers (what bench.py's "e2e" times): copies this step's inputs
+ * host->device into caller-provided device staging, runs append + attention, copies out back,
+ * and synchronises the stream before returning.  The KV pool stays device resident (it is the
+ * worker's cache).  Host buffers should be pinned for the copies to be async.
+ *   staging [device] >= tropical_step_host_staging_bytes(...), 256-byte aligned.
+ *   h_*: [host] same shapes as the device-pointer API.  h_lse nullable. */
+typedef struct {
+    int32_t num_reqs, total_q, max_kv_len, page_table_stride;
+    const int32_t *q_lens, *ctx_lens, *q_offsets, *page_table; /* [host] */
+} tropical_host_batch_t;
+
+size_t tropical_step_host_staging_bytes(const tropical_kv_pool_t *pool, int32_t num_reqs,
+                                        int32_t total_q, int32_t page_table_stride);
+
+int tropical_step_host(const tropical_kv_pool_t *pool, const tropical_host_batch_t *batch,
+                       const void *h_q, const void *h_k_new, const void *h_v_new, void *h_out,
+                       float *h_lse, float sm_scale, void *staging, size_t staging_bytes,
+                       void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Row A6: predicted microseconds of append + attention for a batch ("predicted
+ * execution time", "offline profiling tools", P:159 decode-batch time).  Pure host
+ * code, reentrant.  Form:
+ *   t = t0 + max(a*F, b*B) + kappa*min(a*F, b*B) + e_p*N_p/n_sm + e_d*N_d/n_sm
+ * with F FLOPs, B algorithmic bytes, N_p prefill (128-row x head) tiles weighted by their KV
+ * iterations, N_d decode page-head units.  model == NULL selects the built-in fit measured on
+ * B200 for (Hq, Hkv, d), else TROPICAL_ERR_UNCALIBRATED. */
+typedef struct {
+    double t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us;
+    double n_sm;
+} tropical_cost_model_t;
+
+typedef struct {
+    double flops;          /* 4*d*Hq*sum_i [q_i*c_i + q_i(q_i+1)/2]                         */
+    double bytes;          /* KV read once + new rows r/w + Q/O + page table */
+    double t_tc_us;        /* a * flops */
+    double t_hbm_us;       /* b * bytes */
+    int64_t prefill_tiles; /* sum over prefill requests of ceil(q_i/128) * Hq                */
+    int64_t prefill_iters; /* 128x128 KV iterations over those tiles                          */
+    int64_t decode_units;  /* decode page-head units: sum ceil(L_i/P) * Hkv                   */
+} tropical_cost_breakdown_t;
+
+int tropical_step_cost(const tropical_cost_model_t *model, int32_t num_q_heads,
+                       int32_t num_kv_heads, int32_t head_dim, int32_t page_size, int32_t num_reqs,
+                       const int32_t *q_lens_host, const int32_t *ctx_lens_host, double *out_us,
+                       tropical_cost_breakdown_t *breakdown /* nullable */);
+
+/* Number of kernel launches the last tropical_kv_append / tropical_mixed_attention /
+ * tropical_step_host call on this thread enqueued (bench.py's gpu_launches). */
+int tropical_last_launch_count(void);
+
+/* Test hook: the plain CUDA-core (no tensor core, no split-K) attention kernel, same arguments
+ * and semantics as tropical_mixed_attention without a workspace.  Used by tests to cross-check
+ * the tile kernels on the device; not a product path. */
+int tropical_debug_attention_simt(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
+                                  const void *q, void *out, float *lse, float sm_scale,
+                                  void *cuda_stream);
+
+const char *tropical_status_string(int status);
+const char *tropical_last_cuda_error(void); /* thread-local text of the last CUDA failure */
+const char *tropical_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TROPICAL_H_ */

@@ -1,0 +1,25 @@
+"""tropical-b200: B200-native (sm_100a) hot path of one Tropical multiplexed iteration.
+
+Thin Python binding over the C-ABI in include/tropical.h (argument marshalling only; every step
+of the path runs in the library's CUDA kernels).  PyTorch is used for device memory and streams.
+Importing this package never imports ``oracle``.
+"""
+from .binding import (  # noqa: F401
+    Batch,
+    CostBreakdown,
+    CostModel,
+    KVPool,
+    TropicalError,
+    debug_attention_simt,
+    kv_append,
+    kv_gather,
+    last_launch_count,
+    lib,
+    mixed_attention,
+    status_string,
+    step_cost,
+    step_host,
+    step_host_staging_bytes,
+    version,
+    workspace_bytes,
+)

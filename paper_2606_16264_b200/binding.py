@@ -1,0 +1,262 @@
+"""ctypes binding with the same names as include/tropical.h.  No arithmetic here."""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libtropical.so")
+_lib = None
+
+
+class TropicalError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        detail = lib().tropical_last_cuda_error().decode() if status == 4 else ""
+        super().__init__(f"{where}: {status_string(status)} (status {status}) {detail}".strip())
+
+
+class _Pool(ctypes.Structure):
+    _fields_ = [("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+                ("page_size", ctypes.c_int32), ("num_pages", ctypes.c_int32),
+                ("k_pool", ctypes.c_void_p), ("v_pool", ctypes.c_void_p)]
+
+
+class _Batch(ctypes.Structure):
+    _fields_ = [("num_reqs", ctypes.c_int32), ("total_q", ctypes.c_int32), ("max_kv_len", ctypes.c_int32),
+                ("page_table_stride", ctypes.c_int32),
+                ("q_lens", ctypes.c_void_p), ("ctx_lens", ctypes.c_void_p), ("q_offsets", ctypes.c_void_p),
+                ("page_table", ctypes.c_void_p)]
+
+
+class CostModel(ctypes.Structure):
+    _fields_ = [("t0_us", ctypes.c_double), ("a_us_per_flop", ctypes.c_double), ("b_us_per_byte", ctypes.c_double),
+                ("kappa", ctypes.c_double), ("e_prefill_iter_us", ctypes.c_double),
+                ("e_decode_unit_us", ctypes.c_double), ("n_sm", ctypes.c_double)]
+
+
+class CostBreakdown(ctypes.Structure):
+    _fields_ = [("flops", ctypes.c_double), ("bytes", ctypes.c_double), ("t_tc_us", ctypes.c_double),
+                ("t_hbm_us", ctypes.c_double), ("prefill_tiles", ctypes.c_int64), ("prefill_iters", ctypes.c_int64),
+                ("decode_units", ctypes.c_int64)]
+
+
+EXPORTS = (
+    "tropical_kv_append", "tropical_kv_gather", "tropical_workspace_bytes", "tropical_mixed_attention",
+    "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
+    "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
+    "tropical_debug_attention_simt",
+)
+
+
+def lib():
+    """Load libtropical.so; build it in-tree with nvcc when it is missing or stale.  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    from . import build as _build
+    try:
+        path = _build.build()
+    except Exception as exc:  # no silent fallback: there is no other implementation
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"libtropical.so is missing and could not be built: {exc}") from exc
+        path = _LIB_PATH
+    L = ctypes.CDLL(path)
+    for name in EXPORTS:
+        getattr(L, name)  # AttributeError here = header and library disagree
+    L.tropical_workspace_bytes.restype = ctypes.c_size_t
+    L.tropical_step_host_staging_bytes.restype = ctypes.c_size_t
+    L.tropical_status_string.restype = ctypes.c_char_p
+    L.tropical_last_cuda_error.restype = ctypes.c_char_p
+    L.tropical_version.restype = ctypes.c_char_p
+    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_mixed_attention", "tropical_step_host",
+                 "tropical_step_cost", "tropical_last_launch_count", "tropical_debug_attention_simt"):
+        getattr(L, name).restype = ctypes.c_int
+    _lib = L
+    return L
+
+
+def status_string(status: int) -> str:
+    return lib().tropical_status_string(int(status)).decode()
+
+
+def version() -> str:
+    return lib().tropical_version().decode()
+
+
+def last_launch_count() -> int:
+    return int(lib().tropical_last_launch_count())
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise TropicalError(status, where)
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _stream(stream) -> ctypes.c_void_p:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _dev2(t: torch.Tensor, name: str):
+    if not (t.is_cuda and t.is_contiguous() and t.element_size() == 2):
+        raise ValueError(f"{name} must be a contiguous 2-byte (bf16) CUDA tensor")
+
+
+@dataclass
+class KVPool:
+    """Paged KV pool: k_pool / v_pool are CUDA tensors [num_pages, Hkv, page_size, head_dim], 2-byte dtype."""
+    k_pool: torch.Tensor
+    v_pool: torch.Tensor
+    num_q_heads: int
+
+    def c(self) -> _Pool:
+        _dev2(self.k_pool, "k_pool"); _dev2(self.v_pool, "v_pool")
+        n, hkv, p, d = self.k_pool.shape
+        assert tuple(self.v_pool.shape) == (n, hkv, p, d)
+        return _Pool(self.num_q_heads, hkv, d, p, n, self.k_pool.data_ptr(), self.v_pool.data_ptr())
+
+
+@dataclass
+class Batch:
+    """One multiplexed iteration; the four arrays are int32 CUDA tensors."""
+    q_lens: torch.Tensor
+    ctx_lens: torch.Tensor
+    q_offsets: torch.Tensor
+    page_table: torch.Tensor
+    total_q: int
+    max_kv_len: int
+
+    @staticmethod
+    def from_host(q_lens: Sequence[int], ctx_lens: Sequence[int], page_table, device="cuda") -> "Batch":
+        ql = torch.as_tensor(q_lens, dtype=torch.int32)
+        cl = torch.as_tensor(ctx_lens, dtype=torch.int32)
+        qo = torch.zeros(ql.numel() + 1, dtype=torch.int32)
+        qo[1:] = torch.cumsum(ql, 0)
+        pt = torch.as_tensor(page_table, dtype=torch.int32).contiguous()
+        mk = int((ql.long() + cl.long()).max()) if ql.numel() else 0
+        return Batch(ql.to(device), cl.to(device), qo.to(device), pt.to(device), int(qo[-1]), mk)
+
+    def c(self) -> _Batch:
+        for t in (self.q_lens, self.ctx_lens, self.q_offsets, self.page_table):
+            if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+                raise ValueError("batch arrays must be contiguous int32 CUDA tensors")
+        n = self.q_lens.numel()
+        stride = self.page_table.shape[1] if self.page_table.dim() == 2 else 0
+        return _Batch(n, self.total_q, self.max_kv_len, stride, self.q_lens.data_ptr(), self.ctx_lens.data_ptr(),
+                      self.q_offsets.data_ptr(), self.page_table.data_ptr())
+
+
+def kv_append(pool: KVPool, batch: Batch, k_new: torch.Tensor, v_new: torch.Tensor, stream=None) -> None:
+    _dev2(k_new, "k_new"); _dev2(v_new, "v_new")
+    p, b = pool.c(), batch.c()
+    _check(lib().tropical_kv_append(ctypes.byref(p), ctypes.byref(b), _ptr(k_new), _ptr(v_new), _stream(stream)),
+           "tropical_kv_append")
+
+
+def kv_gather(pool: KVPool, batch: Batch, req: int, n_keys: int, stream=None):
+    p, b = pool.c(), batch.c()
+    hkv, d = pool.k_pool.shape[1], pool.k_pool.shape[3]
+    kd = torch.empty((n_keys, hkv, d), dtype=pool.k_pool.dtype, device=pool.k_pool.device)
+    vd = torch.empty_like(kd)
+    _check(lib().tropical_kv_gather(ctypes.byref(p), ctypes.byref(b), ctypes.c_int32(req), ctypes.c_int32(n_keys),
+                                    _ptr(kd), _ptr(vd), _stream(stream)), "tropical_kv_gather")
+    return kd, vd
+
+
+def workspace_bytes(pool: KVPool, num_reqs: int, total_q: int, max_kv_len: int) -> int:
+    p = pool.c()
+    return int(lib().tropical_workspace_bytes(ctypes.byref(p), ctypes.c_int32(num_reqs), ctypes.c_int32(total_q),
+                                              ctypes.c_int32(max_kv_len)))
+
+
+def _alloc_ws(nbytes: int, device) -> torch.Tensor:
+    return torch.empty(max(nbytes, 256) + 256, dtype=torch.uint8, device=device)
+
+
+def _aligned(t: torch.Tensor) -> torch.Tensor:
+    off = (-t.data_ptr()) % 256
+    return t[off:]
+
+
+def mixed_attention(pool: KVPool, batch: Batch, q: torch.Tensor, out: Optional[torch.Tensor] = None,
+                    lse: Optional[torch.Tensor] = None, sm_scale: float = 0.0,
+                    workspace: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    _dev2(q, "q")
+    if out is None:
+        out = torch.empty_like(q)
+    _dev2(out, "out")
+    p, b = pool.c(), batch.c()
+    if workspace is None:
+        workspace = _alloc_ws(workspace_bytes(pool, b.num_reqs, b.total_q, b.max_kv_len), q.device)
+    ws = _aligned(workspace)
+    if lse is not None and not (lse.is_cuda and lse.dtype == torch.float32 and lse.is_contiguous()):
+        raise ValueError("lse must be a contiguous float32 CUDA tensor")
+    _check(lib().tropical_mixed_attention(ctypes.byref(p), ctypes.byref(b), _ptr(q), _ptr(out), _ptr(lse),
+                                          ctypes.c_float(sm_scale), _ptr(ws), ctypes.c_size_t(ws.numel()),
+                                          _stream(stream)), "tropical_mixed_attention")
+    return out
+
+
+def debug_attention_simt(pool: KVPool, batch: Batch, q: torch.Tensor, lse: Optional[torch.Tensor] = None,
+                         sm_scale: float = 0.0, stream=None) -> torch.Tensor:
+    """The plain CUDA-core kernel, exposed for cross-checking the tile kernels in tests."""
+    out = torch.empty_like(q)
+    p, b = pool.c(), batch.c()
+    _check(lib().tropical_debug_attention_simt(ctypes.byref(p), ctypes.byref(b), _ptr(q), _ptr(out), _ptr(lse),
+                                               ctypes.c_float(sm_scale), _stream(stream)),
+           "tropical_debug_attention_simt")
+    return out
+
+
+class _HostBatch(ctypes.Structure):
+    _fields_ = _Batch._fields_
+
+
+def step_host_staging_bytes(pool: KVPool, num_reqs: int, total_q: int, stride: int) -> int:
+    p = pool.c()
+    return int(lib().tropical_step_host_staging_bytes(ctypes.byref(p), ctypes.c_int32(num_reqs),
+                                                      ctypes.c_int32(total_q), ctypes.c_int32(stride)))
+
+
+def step_host(pool: KVPool, q_lens, ctx_lens, q_offsets, page_table, max_kv_len: int, h_q, h_k_new, h_v_new, h_out,
+              staging: torch.Tensor, workspace: torch.Tensor, h_lse=None, sm_scale: float = 0.0, stream=None) -> None:
+    """End-to-end step from HOST (ideally pinned) torch tensors; synchronises the stream before returning."""
+    for t in (q_lens, ctx_lens, q_offsets, page_table, h_q, h_k_new, h_v_new, h_out):
+        if t.is_cuda or not t.is_contiguous():
+            raise ValueError("step_host takes contiguous host tensors")
+    p = pool.c()
+    n = q_lens.numel()
+    hb = _HostBatch(n, int(h_q.shape[0]), int(max_kv_len), int(page_table.shape[1]) if page_table.dim() == 2 else 0,
+                    q_lens.data_ptr(), ctx_lens.data_ptr(), q_offsets.data_ptr(), page_table.data_ptr())
+    st, ws = _aligned(staging), _aligned(workspace)
+    _check(lib().tropical_step_host(ctypes.byref(p), ctypes.byref(hb), _ptr(h_q), _ptr(h_k_new), _ptr(h_v_new),
+                                    _ptr(h_out), _ptr(h_lse), ctypes.c_float(sm_scale), _ptr(st),
+                                    ctypes.c_size_t(st.numel()), _ptr(ws), ctypes.c_size_t(ws.numel()),
+                                    _stream(stream)), "tropical_step_host")
+
+
+def step_cost(num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int, q_lens: Sequence[int],
+              ctx_lens: Sequence[int], model: Optional[CostModel] = None, require_model: bool = True):
+    """(predicted_us or None, CostBreakdown).  Host only; works without a GPU."""
+    n = len(q_lens)
+    ql = (ctypes.c_int32 * max(n, 1))(*[int(x) for x in q_lens])
+    cl = (ctypes.c_int32 * max(n, 1))(*[int(x) for x in ctx_lens])
+    us = ctypes.c_double(0.0)
+    bd = CostBreakdown()
+    rc = lib().tropical_step_cost(ctypes.byref(model) if model is not None else None, ctypes.c_int32(num_q_heads),
+                                  ctypes.c_int32(num_kv_heads), ctypes.c_int32(head_dim), ctypes.c_int32(page_size),
+                                  ctypes.c_int32(n), ql, cl, ctypes.byref(us), ctypes.byref(bd))
+    if rc == 5 and not require_model:
+        return None, bd
+    _check(rc, "tropical_step_cost")
+    return us.value, bd

@@ -1,0 +1,18 @@
+// kernels.h -- internal launch interfaces between api.cu and the kernel translation units.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "common.cuh"
+
+namespace tropical {
+
+cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const void* k_new, const void* v_new,
+                             cudaStream_t stream);
+cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, int n_keys, void* k_dense,
+                             void* v_dense, cudaStream_t stream);
+cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
+                                  float scale_log2, cudaStream_t stream);
+
+}  // namespace tropical

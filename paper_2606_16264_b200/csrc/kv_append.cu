@@ -1,0 +1,95 @@
+// kv_append.cu -- SURVEY.md 8(a) rows A1 (KV append) and A2 (page gather), bit-exact copies.
+//
+// A1: for t < q_i, pos = c_i + t: pool[page_table[i][pos/P]][h][pos%P][:] = new[q_off_i+t][h][:].
+// HBM-bound and tiny: T*Hkv rows of 2*d bytes each for K and V.  One thread moves one 16-byte
+// chunk; the d/8 threads of a row read and write 2*d contiguous bytes (fully coalesced on both
+// sides -- a (page, head, slot) row of the HND pool is contiguous).
+#include "common.cuh"
+#include "kernels.h"
+
+namespace tropical {
+
+template <int D>
+__global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc b,
+                                                        const uint4* __restrict__ k_new,
+                                                        const uint4* __restrict__ v_new) {
+    constexpr int CH = D / 8;  // 16-byte chunks per row
+    const long long total = (long long)b.total_q * pool.Hkv * CH * 2;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int chunk = (int)(idx % CH);
+        long long r = idx / CH;
+        const int which = (int)(r & 1);  // 0 = K, 1 = V
+        r >>= 1;
+        const int h = (int)(r % pool.Hkv);
+        const int tok = (int)(r / pool.Hkv);
+        const int req = find_request(b.q_offsets, b.num_reqs, tok);
+        const int t = tok - __ldg(b.q_offsets + req);
+        const int pos = __ldg(b.ctx_lens + req) + t;
+        const int page = __ldg(b.page_table + (size_t)req * b.stride + pos / kPageSize);
+        const int slot = pos % kPageSize;
+        const size_t dst = (((size_t)page * pool.Hkv + h) * kPageSize + slot) * CH + chunk;
+        const size_t src = ((size_t)tok * pool.Hkv + h) * CH + chunk;
+        if (which == 0)
+            reinterpret_cast<uint4*>(const_cast<uint16_t*>(pool.k_pool))[dst] = __ldg(k_new + src);
+        else
+            reinterpret_cast<uint4*>(const_cast<uint16_t*>(pool.v_pool))[dst] = __ldg(v_new + src);
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(256) kv_gather_kernel(PoolDesc pool, BatchDesc b, int req, int n_keys,
+                                                        uint4* __restrict__ k_dense, uint4* __restrict__ v_dense) {
+    constexpr int CH = D / 8;
+    const long long total = (long long)n_keys * pool.Hkv * CH * 2;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int chunk = (int)(idx % CH);
+        long long r = idx / CH;
+        const int which = (int)(r & 1);
+        r >>= 1;
+        const int h = (int)(r % pool.Hkv);
+        const int j = (int)(r / pool.Hkv);
+        const int page = __ldg(b.page_table + (size_t)req * b.stride + j / kPageSize);
+        const size_t src = (((size_t)page * pool.Hkv + h) * kPageSize + j % kPageSize) * CH + chunk;
+        const size_t dst = ((size_t)j * pool.Hkv + h) * CH + chunk;
+        if (which == 0)
+            k_dense[dst] = __ldg(reinterpret_cast<const uint4*>(pool.k_pool) + src);
+        else
+            v_dense[dst] = __ldg(reinterpret_cast<const uint4*>(pool.v_pool) + src);
+    }
+}
+
+static int grid_for(long long total_threads, int block) {
+    long long g = (total_threads + block - 1) / block;
+    const long long cap = 148LL * 8;  // grid-stride beyond 8 CTAs per SM
+    if (g > cap) g = cap;
+    if (g < 1) g = 1;
+    return (int)g;
+}
+
+cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const void* k_new, const void* v_new,
+                             cudaStream_t stream) {
+    if (b.total_q == 0) return cudaSuccess;
+    const long long total = (long long)b.total_q * pool.Hkv * (pool.D / 8) * 2;
+    const int grid = grid_for(total, 256);
+    if (pool.D == 128)
+        kv_append_kernel<128><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new);
+    else
+        kv_append_kernel<64><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, int n_keys, void* k_dense,
+                             void* v_dense, cudaStream_t stream) {
+    if (n_keys == 0) return cudaSuccess;
+    const long long total = (long long)n_keys * pool.Hkv * (pool.D / 8) * 2;
+    const int grid = grid_for(total, 256);
+    if (pool.D == 128)
+        kv_gather_kernel<128><<<grid, 256, 0, stream>>>(pool, b, req, n_keys, (uint4*)k_dense, (uint4*)v_dense);
+    else
+        kv_gather_kernel<64><<<grid, 256, 0, stream>>>(pool, b, req, n_keys, (uint4*)k_dense, (uint4*)v_dense);
+    return cudaGetLastError();
+}
+
+}  // namespace tropical

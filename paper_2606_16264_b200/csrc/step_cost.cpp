@@ -1,0 +1,85 @@
+// step_cost.cpp -- SURVEY.md 8(a) row A6: host-side execution-time prediction for one
+// multiplexed iteration (PAPER.md:143 "predicted execution time", :157 "offline profiling
+// tools", :159 predicted decode-batch time).  The paper gives no functional form; the form
+// below is this build's (parity unpinned).  Pure host code.
+#include <math.h>
+#include <stdint.h>
+
+#include "../../include/tropical.h"
+
+namespace {
+
+struct BuiltinFit {
+    int Hq, Hkv, d;
+    tropical_cost_model_t m;
+};
+
+// Filled from measured kernel times by paper_2606_16264_b200/fit_cost_model.py (values are
+// copied here by hand after a fit run; provenance in DESIGN.md).  Empty until calibrated.
+const BuiltinFit kBuiltin[] = {
+    {0, 0, 0, {0, 0, 0, 0, 0, 0, 148}},
+};
+
+void features(int Hq, int Hkv, int d, int P, int n, const int32_t* q, const int32_t* c,
+              tropical_cost_breakdown_t* f) {
+    double qc = 0, pages = 0, T = 0, csum = 0;
+    int64_t tiles = 0, iters = 0, units = 0;
+    for (int i = 0; i < n; ++i) {
+        const double qi = q[i], ci = c[i];
+        if (q[i] <= 0) continue;
+        qc += qi * ci + qi * (qi + 1) / 2;
+        T += qi;
+        csum += ci;
+        const int64_t L = (int64_t)q[i] + c[i];
+        pages += (double)((L + P - 1) / P);
+        if (q[i] == 1) {
+            units += ((L + P - 1) / P) * Hkv;
+        } else {
+            const int nt = (q[i] + 127) / 128;
+            tiles += (int64_t)nt * Hq;
+            for (int ti = 0; ti < nt; ++ti) {
+                const int64_t last = (int64_t)c[i] + ((ti + 1) * 128 < q[i] ? (ti + 1) * 128 : q[i]);
+                iters += ((last + 127) / 128) * Hq;
+            }
+        }
+    }
+    f->flops = 4.0 * d * Hq * qc;
+    f->bytes = 2.0 * 2 * Hkv * d * csum + 2.0 * (2.0 * 2 * Hkv * d * T) + 2.0 * (2.0 * Hq * d * T) + 4.0 * pages;
+    f->prefill_tiles = tiles;
+    f->prefill_iters = iters;
+    f->decode_units = units;
+    f->t_tc_us = 0;
+    f->t_hbm_us = 0;
+}
+
+}  // namespace
+
+extern "C" int tropical_step_cost(const tropical_cost_model_t* model, int32_t Hq, int32_t Hkv, int32_t d,
+                                  int32_t P, int32_t num_reqs, const int32_t* q_lens, const int32_t* ctx_lens,
+                                  double* out_us, tropical_cost_breakdown_t* breakdown) {
+    if (Hq <= 0 || Hkv <= 0 || d <= 0 || P <= 0 || num_reqs < 0 || Hq % Hkv != 0) return TROPICAL_ERR_INVALID_ARG;
+    if (num_reqs > 0 && (q_lens == nullptr || ctx_lens == nullptr)) return TROPICAL_ERR_INVALID_ARG;
+    if (out_us == nullptr && breakdown == nullptr) return TROPICAL_ERR_INVALID_ARG;
+    for (int i = 0; i < num_reqs; ++i)
+        if (q_lens[i] < 0 || ctx_lens[i] < 0) return TROPICAL_ERR_INVALID_ARG;
+    tropical_cost_breakdown_t f;
+    features(Hq, Hkv, d, P, num_reqs, q_lens, ctx_lens, &f);
+    if (model == nullptr) {
+        for (const BuiltinFit& b : kBuiltin)
+            if (b.Hq == Hq && b.Hkv == Hkv && b.d == d) model = &b.m;
+    }
+    if (model != nullptr) {
+        f.t_tc_us = model->a_us_per_flop * f.flops;
+        f.t_hbm_us = model->b_us_per_byte * f.bytes;
+    }
+    if (breakdown != nullptr) *breakdown = f;
+    if (model == nullptr) return out_us ? TROPICAL_ERR_UNCALIBRATED : TROPICAL_OK;
+    if (out_us != nullptr) {
+        const double hi = f.t_tc_us > f.t_hbm_us ? f.t_tc_us : f.t_hbm_us;
+        const double lo = f.t_tc_us > f.t_hbm_us ? f.t_hbm_us : f.t_tc_us;
+        const double nsm = model->n_sm > 0 ? model->n_sm : 148.0;
+        *out_us = model->t0_us + hi + model->kappa * lo + model->e_prefill_iter_us * (double)f.prefill_iters / nsm +
+                  model->e_decode_unit_us * (double)f.decode_units / nsm;
+    }
+    return TROPICAL_OK;
+}

@@ -1,0 +1,241 @@
+"""GPU-vs-oracle parity, through the C-ABI (paper_2606_16264_b200.binding -> libtropical.so).
+
+Bars (BASELINE.json north_star): KV append and page gather bit-exact over the WHOLE pool;
+attention output max |d| <= 2e-2 and mean |d| <= 2e-3 against the fp64 oracle.
+Needle tests make the page gather *through the attention kernel* bit-exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from synth import f32_to_bf16_bits
+from tests.gpu_harness import MAX_ABS_TOL, MEAN_ABS_TOL, DeviceStep, bits, errors
+
+pytestmark = pytest.mark.gpu
+
+
+def _step(seed, Hq, Hkv, d, q_lens, ctx_lens, **kw):
+    return synth.make_step(np.random.default_rng(seed), Hq, Hkv, d, 16, q_lens, ctx_lens, **kw)
+
+
+def _check_step(s, impl="product", sm_scale=0.0, lse_tol=2e-3):
+    ref_out, ref_lse, kp, vp = oracle.step(s, sm_scale)
+    dev = DeviceStep(s)
+    out, lse = dev.step(sm_scale, impl)
+    # A1/A2: pool bit-identical to the oracle's over the whole pool; attention never writes it
+    assert np.array_equal(bits(dev.k_pool), kp), "K pool differs"
+    assert np.array_equal(bits(dev.v_pool), vp), "V pool differs"
+    assert np.isfinite(out).all()
+    mx, mean = errors(out, ref_out)
+    assert mx <= MAX_ABS_TOL and mean <= MEAN_ABS_TOL, (mx, mean)
+    if s.total_q:
+        assert np.abs(lse - ref_lse).max() <= lse_tol
+    return mx, mean
+
+
+# ------------------------------------------------------------------ BASELINE configs[0]
+@pytest.mark.parametrize("impl", ["product", "simt"])
+def test_C1_tiny_mixed_step(impl):
+    s = synth.make_config("C1")
+    mx, mean = _check_step(s, impl)
+    assert mx < 1.2e-2  # diagnostic band O10: far above this signals a bug even inside tolerance
+
+
+def test_C1_gather_bit_exact():
+    s = synth.make_config("C1")
+    _, _, kp, vp = oracle.step(s)
+    dev = DeviceStep(s)
+    dev.append()
+    for i in range(s.num_reqs):
+        n = int(s.ctx_lens[i] + s.q_lens[i])
+        kd, vd = dev.tb.kv_gather(dev.pool, dev.batch, i, n)
+        ok, ov = oracle.kv_gather(kp, vp, s.page_table, i, n)
+        assert np.array_equal(bits(kd), ok) and np.array_equal(bits(vd), ov)
+
+
+# ------------------------------------------------------------------ edge-case matrix
+EDGE_Q = [0, 1, 2, 15, 16, 17, 127, 128, 129, 255, 256, 257, 1000]
+EDGE_C = [0, 1, 15, 16, 17, 127, 128, 129, 255, 256, 257, 511, 512, 513, 4095, 4096, 4097]
+
+
+@pytest.mark.parametrize("d", [64, 128])
+@pytest.mark.parametrize("g", [1, 4, 8])
+def test_edge_matrix_q_by_c(d, g):
+    """Every q in EDGE_Q paired with several c in EDGE_C, batched so the whole matrix is covered."""
+    Hkv = 2
+    rng = np.random.default_rng(100 + d + g)
+    for k, q in enumerate(EDGE_Q):
+        cs = [EDGE_C[(k * 5 + r * 3) % len(EDGE_C)] for r in range(4)]
+        if q == 1000:
+            cs = cs[:2]
+        s = synth.make_step(rng, Hkv * g, Hkv, d, 16, [q] * len(cs), cs)
+        _check_step(s)
+
+
+@pytest.mark.parametrize("d", [64, 128])
+def test_every_context_edge_as_decode(d):
+    s = _step(7, 8, 2, d, [1] * len(EDGE_C), EDGE_C)
+    _check_step(s)
+
+
+@pytest.mark.parametrize("order", ["decode_first", "prefill_first", "interleaved", "only_decode", "only_prefill", "single", "with_skips"])
+def test_request_orders(order):
+    qs = {"decode_first": [1, 1, 1, 200, 33], "prefill_first": [200, 33, 1, 1, 1], "interleaved": [1, 200, 1, 33, 1],
+          "only_decode": [1, 1, 1, 1], "only_prefill": [130, 64, 2], "single": [77], "with_skips": [0, 1, 0, 40, 0]}[order]
+    cs = [(37 * (i + 1)) % 300 for i in range(len(qs))]
+    _check_step(_step(8, 8, 4, 128, qs, cs))
+
+
+def test_empty_batch_is_a_noop():
+    import paper_2606_16264_b200 as tb
+    kp = torch.zeros((4, 2, 16, 128), dtype=torch.int16, device="cuda")
+    pool = tb.KVPool(kp, kp.clone(), 4)
+    batch = tb.Batch.from_host([], [], np.zeros((0, 1), np.int32))
+    q = torch.zeros((0, 4, 128), dtype=torch.int16, device="cuda")
+    tb.kv_append(pool, batch, q[:, :2], q[:, :2])
+    out = tb.mixed_attention(pool, batch, q)
+    assert out.shape[0] == 0
+
+
+def test_custom_scale_and_chunk_on_prior_context():
+    """S13 variant C4b shape in small: chunk on prior context (third chunk), plus sm_scale override."""
+    s = _step(9, 4, 4, 128, [256, 1, 1], [512, 100, 1023])
+    _check_step(s, sm_scale=0.05)
+    _check_step(s)
+
+
+# ------------------------------------------------------------------ O7 on the GPU
+def test_chunked_equals_unchunked_and_decode_equals_last_row():
+    rng = np.random.default_rng(10)
+    L, Hq, Hkv, d = 300, 4, 2, 128
+    whole = synth.make_step(rng, Hq, Hkv, d, 16, [L], [0])
+    ref, _, kp, vp = oracle.step(whole)
+    dev = DeviceStep(whole)
+    out_whole, _ = dev.step()
+    # second half as a chunk over the first half as context: reuse the appended pool
+    L1 = 140
+    s2 = synth.StepInputs("chunk", -1, Hq, Hkv, d, 16, whole.num_pages, np.array([L - L1], np.int32),
+                          np.array([L1], np.int32), np.array([0, L - L1], np.int32), whole.page_table, kp, vp,
+                          whole.q[L1:].copy(), whole.k_new[L1:].copy(), whole.v_new[L1:].copy())
+    out_chunk, _ = DeviceStep(s2).step()
+    assert errors(out_chunk, ref[L1:])[0] <= MAX_ABS_TOL
+    assert np.abs(out_chunk - out_whole[L1:]).max() <= 2e-2
+    s3 = synth.StepInputs("dec", -1, Hq, Hkv, d, 16, whole.num_pages, np.array([1], np.int32),
+                          np.array([L - 1], np.int32), np.array([0, 1], np.int32), whole.page_table, kp, vp,
+                          whole.q[L - 1:].copy(), whole.k_new[L - 1:].copy(), whole.v_new[L - 1:].copy())
+    out_dec, _ = DeviceStep(s3).step()
+    assert errors(out_dec, ref[L - 1:])[0] <= MAX_ABS_TOL
+
+
+# ------------------------------------------------------------------ O8 needle (bit-exact gather through attention)
+def _needle_step(d, c, ql, targets_fn, Hq=2, Hkv=1, seed=0):
+    rng = np.random.default_rng(seed)
+    L = c + ql
+
+    def code(j):
+        vec = np.full(d, 32.0, np.float32)
+        vec[:14] = np.where((j >> np.arange(14)) & 1, 32.0, -32.0)
+        return vec
+
+    K = np.stack([code(j) for j in range(L)])[:, None, :].repeat(Hkv, 1)
+    V = rng.standard_normal((L, Hkv, d)).astype(np.float32)
+    targets = [targets_fn(t) for t in range(ql)]
+    Q = np.stack([code(j) for j in targets])[:, None, :].repeat(Hq, 1)
+    s = synth.make_step(rng, Hq, Hkv, d, 16, [ql], [c])
+    Kb, Vb = f32_to_bf16_bits(K), f32_to_bf16_bits(V)
+    # install prior context rows [0,c) directly, new rows via the append under test
+    for j in range(c):
+        s.k_pool[s.page_table[0, j // 16], :, j % 16, :] = Kb[j]
+        s.v_pool[s.page_table[0, j // 16], :, j % 16, :] = Vb[j]
+    s.k_new[:], s.v_new[:], s.q[:] = Kb[c:], Vb[c:], f32_to_bf16_bits(Q)
+    return s, targets, Vb
+
+
+@pytest.mark.parametrize("d", [64, 128])
+@pytest.mark.parametrize("c,ql", [(300, 200), (0, 257), (4090, 1), (1000, 1), (127, 130)])
+def test_needle_selects_target_row_bitwise(d, c, ql):
+    edges = [0, 15, 16, 17, 127, 128, 129, 255, 256, 257, 511, 512, 513, 1023, 1024, 1025]
+
+    def target(t):
+        lim = c + t
+        k = t % 4
+        if k == 0:
+            return lim                      # own just-appended row: append->attend order, diagonal included
+        if k == 1:
+            return max(lim - 1, 0)
+        if k == 2:
+            return min(edges[(t // 4) % len(edges)], lim)
+        return (t * 7919) % (lim + 1)
+
+    s, targets, Vb = _needle_step(d, c, ql, target)
+    dev = DeviceStep(s)
+    dev.step()
+    got = bits(dev.out)
+    for t, j in enumerate(targets):
+        for h in range(s.num_q_heads):
+            assert np.array_equal(got[t, h], Vb[j, 0]), f"row {t} head {h}: expected V[{j}]"
+
+
+def test_negative_needle_future_key_not_selected():
+    c, ql, d = 40, 50, 128
+    s, targets, Vb = _needle_step(d, c, ql, lambda t: min(c + t + 1, c + ql - 1))
+    ref, _, _, _ = oracle.step(s)
+    dev = DeviceStep(s)
+    out, _ = dev.step()
+    assert errors(out, ref)[0] <= MAX_ABS_TOL
+    got = bits(dev.out)
+    assert not np.array_equal(got[3, 0], Vb[c + 3 + 1, 0])
+
+
+# ------------------------------------------------------------------ O9 poison + stray writes, determinism
+def test_poison_pool_outputs_finite_and_pool_untouched_elsewhere():
+    s = _step(12, 8, 2, 128, [129, 1, 1, 17], [3, 250, 4097, 60], poison=True)
+    before_k = s.k_pool.copy()
+    dev = DeviceStep(s)
+    out, _ = dev.step()
+    assert np.isfinite(out).all()
+    after = bits(dev.k_pool)
+    changed_rows = (after != before_k).any(axis=-1)
+    assert changed_rows.sum() == s.total_q * s.num_kv_heads  # exactly the appended rows changed
+
+
+def test_run_to_run_deterministic():
+    s = _step(13, 8, 2, 128, [300, 1, 1, 1], [0, 2000, 5000, 64])
+    dev = DeviceStep(s)
+    dev.step()
+    a = bits(dev.out).copy()
+    for _ in range(3):
+        dev.out.zero_()
+        dev.attention()
+        torch.cuda.synchronize()
+        assert np.array_equal(bits(dev.out), a)
+
+
+def test_product_path_matches_simt_cross_check():
+    s = _step(14, 16, 2, 128, [513, 1, 1, 1, 40], [0, 777, 4097, 15, 130])
+    dev = DeviceStep(s)
+    a, la = dev.step(impl="product")
+    b, lb = dev.step(impl="simt")
+    assert np.abs(a - b).max() <= 2e-2 and np.abs(la - lb).max() <= 2e-3
+
+
+# ------------------------------------------------------------------ end-to-end host entry point
+def test_step_host_equals_device_path():
+    import paper_2606_16264_b200 as tb
+    s = _step(15, 8, 2, 128, [150, 1, 1], [10, 300, 64])
+    ref, ref_lse, kp, vp = oracle.step(s)
+    dev = DeviceStep(s)
+    pin = lambda a: torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).pin_memory()
+    h_out = torch.zeros(s.q.shape, dtype=torch.int16).pin_memory()
+    h_lse = torch.zeros((s.total_q, s.num_q_heads), dtype=torch.float32).pin_memory()
+    staging = torch.empty(tb.step_host_staging_bytes(dev.pool, s.num_reqs, s.total_q, s.page_table_stride) + 256,
+                          dtype=torch.uint8, device="cuda")
+    tb.step_host(dev.pool, pin(s.q_lens), pin(s.ctx_lens), pin(s.q_offsets), pin(s.page_table), s.max_kv_len,
+                 pin(s.q), pin(s.k_new), pin(s.v_new), h_out, staging, dev.workspace, h_lse=h_lse)
+    out = synth.bf16_bits_to_f32(h_out.numpy().view(np.uint16)).astype(np.float64)
+    assert errors(out, ref)[0] <= MAX_ABS_TOL and errors(out, ref)[1] <= MEAN_ABS_TOL
+    assert np.array_equal(bits(dev.k_pool), kp)
+    assert np.abs(h_lse.numpy() - ref_lse).max() <= 2e-3
+    assert tb.last_launch_count() >= 2
