@@ -99,7 +99,7 @@ class ClockSampler(threading.Thread):
 
 
 # ----------------------------------------------------------------------------- oracle leg (CPU)
-def oracle_sample_us(s: synth.StepInputs, budget_rows_flops: float = 6e9, seed: int = 0):
+def oracle_sample_us(s: synth.StepInputs, budget_rows_flops: float = 4e11, seed: int = 0):
     """Time the fp64 oracle on a seeded random sample of rows of this workload and extrapolate to one
     full step by FLOP ratio.  Returns (us_per_step_extrapolated, description, cores, sample_seconds)."""
     import oracle

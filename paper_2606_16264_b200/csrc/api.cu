@@ -77,13 +77,12 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 int mixed_attention_impl(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* q, void* out,
                          float* lse, float sm_scale, void* workspace, size_t workspace_bytes, cudaStream_t stream,
                          int* launches) {
-    (void)workspace;
     (void)workspace_bytes;
     const float scale = sm_scale > 0.f ? sm_scale : 1.0f / sqrtf((float)pool->head_dim);
     const float scale_log2 = scale * 1.4426950408889634f;
-    cudaError_t e = launch_attention_simt(to_pool(pool), to_batch(batch), q, out, lse, scale_log2, stream);
-    if (e != cudaSuccess) return cuda_fail(e, "attention_simt");
-    *launches += 1;
+    cudaError_t e = launch_mixed_attention(to_pool(pool), to_batch(batch), q, out, lse, scale_log2, workspace, stream,
+                                           launches);
+    if (e != cudaSuccess) return cuda_fail(e, "mixed_attention");
     return TROPICAL_OK;
 }
 
@@ -127,8 +126,10 @@ int tropical_kv_gather(const tropical_kv_pool_t* pool, const tropical_batch_t* b
 size_t tropical_workspace_bytes(const tropical_kv_pool_t* pool, int32_t num_reqs, int32_t total_q,
                                 int32_t max_kv_len) {
     if (pool == nullptr || num_reqs < 0 || total_q < 0 || max_kv_len < 0) return 0;
-    if (pool->num_q_heads <= 0 || pool->num_kv_heads <= 0) return 0;
-    return 256;
+    if (pool->num_q_heads <= 0 || pool->num_kv_heads <= 0 || pool->num_q_heads % pool->num_kv_heads) return 0;
+    if (pool->head_dim != 64 && pool->head_dim != 128) return 0;
+    (void)max_kv_len;  // split-K partials are bounded by the unit budget, not by the context length
+    return mixed_workspace_bytes(pool->num_q_heads, pool->num_kv_heads, pool->head_dim, num_reqs, total_q);
 }
 
 int tropical_mixed_attention(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* q, void* out,

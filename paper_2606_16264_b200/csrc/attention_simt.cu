@@ -17,7 +17,7 @@ template <int D>
 __global__ void __launch_bounds__(kSimtWarps * 32) attention_simt_kernel(PoolDesc pool, BatchDesc b,
                                                                          const uint16_t* __restrict__ q,
                                                                          uint16_t* __restrict__ out,
-                                                                         float* __restrict__ lse, float scale_log2) {
+                                                                         float* __restrict__ lse, float scale_log2, int skip_decode) {
     constexpr int EPL = D / 32;  // output elements per lane (4 at d=128, 2 at d=64)
     __shared__ float q_s[kSimtWarps][D];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -28,6 +28,7 @@ __global__ void __launch_bounds__(kSimtWarps * 32) attention_simt_kernel(PoolDes
          row += (long long)gridDim.x * kSimtWarps) {
         const int tok = (int)(row / pool.Hq), hq = (int)(row % pool.Hq), hk = hq / g;
         const int req = find_request(b.q_offsets, b.num_reqs, tok);
+        if (skip_decode && __ldg(b.q_lens + req) == 1) continue;  // decode rows belong to the decode tiles
         const int t = tok - __ldg(b.q_offsets + req);
         const int n = __ldg(b.ctx_lens + req) + t + 1;  // visible keys
         const int* pt = b.page_table + (size_t)req * b.stride;
@@ -111,17 +112,17 @@ __global__ void __launch_bounds__(kSimtWarps * 32) attention_simt_kernel(PoolDes
 }
 
 cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
-                                  float scale_log2, cudaStream_t stream) {
+                                  float scale_log2, cudaStream_t stream, bool skip_decode) {
     const long long n_rows = (long long)b.total_q * pool.Hq;
     if (n_rows == 0) return cudaSuccess;
     long long grid = (n_rows + kSimtWarps - 1) / kSimtWarps;
     if (grid > 148LL * 64) grid = 148LL * 64;
     if (pool.D == 128)
         attention_simt_kernel<128><<<(int)grid, kSimtWarps * 32, 0, stream>>>(pool, b, (const uint16_t*)q,
-                                                                              (uint16_t*)out, lse, scale_log2);
+                                                                              (uint16_t*)out, lse, scale_log2, skip_decode ? 1 : 0);
     else
         attention_simt_kernel<64><<<(int)grid, kSimtWarps * 32, 0, stream>>>(pool, b, (const uint16_t*)q,
-                                                                             (uint16_t*)out, lse, scale_log2);
+                                                                             (uint16_t*)out, lse, scale_log2, skip_decode ? 1 : 0);
     return cudaGetLastError();
 }
 

@@ -13,6 +13,9 @@ cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const voi
 cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, int n_keys, void* k_dense,
                              void* v_dense, cudaStream_t stream);
 cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
-                                  float scale_log2, cudaStream_t stream);
+                                  float scale_log2, cudaStream_t stream, bool skip_decode = false);
+cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
+                                   float scale_log2, void* workspace, cudaStream_t stream, int* launches);
+size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q);
 
 }  // namespace tropical

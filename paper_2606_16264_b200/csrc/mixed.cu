@@ -1,0 +1,135 @@
+// mixed.cu -- kernels of tropical_mixed_attention: plan (A0), decode tiles (A4), combine (A5),
+// prefill tiles (A3) and their launchers.
+#include <cuda.h>
+
+#include "common.cuh"
+#include "decode.cuh"
+#include "kernels.h"
+#include "plan.cuh"
+#include "tma_host.h"
+
+namespace tropical {
+
+constexpr int kDecodeWarps = 4;
+constexpr int kDecodeStages = 3;
+
+template <int D>
+__global__ void __launch_bounds__(kDecodeWarps * 32, 2)
+decode_kernel(DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
+    using C = DecodeCfg<D>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kDecodeWarps * kDecodeStages * C::STAGE_BYTES);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        tma_prefetch_desc(&tm_k);
+        tma_prefetch_desc(&tm_v);
+        for (int i = 0; i < kDecodeWarps * kDecodeStages; ++i) mbar_init(bars + i, 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    uint32_t it = 0;
+    decode_warp_worker<D, kDecodeStages>(A, &tm_k, &tm_v, smem + warp * kDecodeStages * C::STAGE_BYTES,
+                                         bars + warp * kDecodeStages, it);
+    (void)lane;
+}
+
+template <int D>
+__global__ void __launch_bounds__(128) combine_kernel(CombineArgs A) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long n = (long long)A.b.num_reqs * A.pool.Hq;
+    for (long long r = (long long)blockIdx.x * 4 + warp; r < n; r += (long long)gridDim.x * 4)
+        combine_row<D>(A, (int)(r / A.pool.Hq), (int)(r % A.pool.Hq), lane);
+}
+
+static int g_num_sms = 0;
+static int num_sms() {
+    if (g_num_sms == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (g_num_sms <= 0) g_num_sms = 148;
+    }
+    return g_num_sms;
+}
+
+size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q) {
+    return make_layout(Hq, Hkv, D, num_reqs, total_q).total;
+}
+
+template <int D>
+static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
+                                  float scale_log2, void* workspace, cudaStream_t stream, int* launches) {
+    const WorkspaceLayout w = make_layout(pool.Hq, pool.Hkv, D, b.num_reqs, b.total_q);
+    char* ws = (char*)workspace;
+    PlanPtrs P;
+    P.hdr = (int*)(ws + w.hdr);
+    P.req_info = (int4*)(ws + w.req_info);
+    P.items = (int2*)(ws + w.items);
+    P.units = (int4*)(ws + w.units);
+    plan_kernel<<<1, kPlanThreads, 0, stream>>>(b, pool.Hq, pool.Hkv, P);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    ++*launches;
+
+    // prefill rows (q_i >= 2): CUDA-core kernel until the tcgen05 tile path lands
+    e = launch_attention_simt(pool, b, q, out, lse, scale_log2, stream, /*skip_decode=*/true);
+    if (e != cudaSuccess) return e;
+    ++*launches;
+
+    CUtensorMap tm_k, tm_v;
+    const long long rows = (long long)pool.num_pages * pool.Hkv * kPageSize;
+    if (!encode_pool_map(&tm_k, pool.k_pool, rows, D) || !encode_pool_map(&tm_v, pool.v_pool, rows, D))
+        return cudaErrorInvalidValue;
+    DecodeArgs A;
+    A.pool = pool;
+    A.b = b;
+    A.q = (const uint16_t*)q;
+    A.out = (uint16_t*)out;
+    A.lse = lse;
+    A.scale_log2 = scale_log2;
+    A.hdr = P.hdr;
+    A.ticket = P.hdr + HDR_TICKET_DECODE;
+    A.req_info = P.req_info;
+    A.units = P.units;
+    A.part_ml = (float2*)(ws + w.part_ml);
+    A.part_o = (float*)(ws + w.part_o);
+    const size_t smem = (size_t)kDecodeWarps * kDecodeStages * DecodeCfg<D>::STAGE_BYTES + 1024 + 256;
+    static bool attr_done = false;
+    if (!attr_done) {
+        e = cudaFuncSetAttribute(decode_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    decode_kernel<D><<<2 * num_sms(), kDecodeWarps * 32, smem, stream>>>(A, tm_k, tm_v);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    ++*launches;
+
+    CombineArgs Cb;
+    Cb.pool = pool;
+    Cb.b = b;
+    Cb.out = (uint16_t*)out;
+    Cb.lse = lse;
+    Cb.req_info = P.req_info;
+    Cb.part_ml = A.part_ml;
+    Cb.part_o = A.part_o;
+    long long rows_c = (long long)b.num_reqs * pool.Hq;
+    int grid = (int)((rows_c + 3) / 4);
+    if (grid > 8 * num_sms()) grid = 8 * num_sms();
+    if (grid > 0) {
+        combine_kernel<D><<<grid, 128, 0, stream>>>(Cb);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        ++*launches;
+    }
+    return cudaSuccess;
+}
+
+cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
+                                   float scale_log2, void* workspace, cudaStream_t stream, int* launches) {
+    if (pool.D == 128) return launch_mixed_t<128>(pool, b, q, out, lse, scale_log2, workspace, stream, launches);
+    return launch_mixed_t<64>(pool, b, q, out, lse, scale_log2, workspace, stream, launches);
+}
+
+}  // namespace tropical

@@ -1,0 +1,154 @@
+// plan.cuh -- SURVEY.md 8(a) row A0: the tile directory.  One small kernel turns the per-request
+// (q_i, c_i) arrays into two explicit work lists in the workspace -- prefill items
+// (request, 128-row q tile, q head) and decode units (request, kv head, head block, page range) --
+// so that the persistent attention kernel only pops tickets.  No host sync, no host plan.
+#pragma once
+#include "common.cuh"
+
+namespace tropical {
+
+constexpr int kQTile = 128;          // query rows per prefill item
+constexpr int kKvTile = 128;         // keys per prefill KV iteration (8 pages)
+constexpr int kHeadBlock = 8;        // q heads of one kv group handled by one decode unit (MMA M rows used)
+constexpr int kTargetUnits = 9472;   // ~8 decode units per resident decode warp (148 SMs x 8 warps x 8)
+constexpr int kMinSplitPages = 8;    // never split finer than 128 tokens
+
+enum { HDR_N_ITEMS = 0, HDR_N_UNITS = 1, HDR_SPLIT_PAGES = 2, HDR_TICKET_PREFILL = 3, HDR_TICKET_DECODE = 4,
+       HDR_N_COMBINE = 5, HDR_INTS = 64 };
+
+// req_info[i] = {kind, unit_base, nsplit, item_base}; kind 0 skip, 1 decode, 2 prefill
+struct WorkspaceLayout {
+    size_t hdr, req_info, items, units, part_ml, part_o, total;
+    int max_items, max_units;
+};
+
+__host__ __device__ inline size_t ws_align(size_t x) { return (x + 255) / 256 * 256; }
+
+__host__ __device__ inline WorkspaceLayout make_layout(int Hq, int Hkv, int D, int num_reqs, int total_q) {
+    WorkspaceLayout w;
+    const int g = Hq / Hkv;
+    const int HB = (g + kHeadBlock - 1) / kHeadBlock;
+    w.max_items = (total_q / kQTile + num_reqs) * Hq;
+    w.max_units = kTargetUnits + num_reqs * Hkv * HB;
+    size_t off = 0;
+    w.hdr = off;       off += ws_align(HDR_INTS * sizeof(int));
+    w.req_info = off;  off += ws_align((size_t)(num_reqs > 0 ? num_reqs : 1) * sizeof(int4));
+    w.items = off;     off += ws_align((size_t)(w.max_items > 0 ? w.max_items : 1) * sizeof(int2));
+    w.units = off;     off += ws_align((size_t)w.max_units * sizeof(int4));
+    w.part_ml = off;   off += ws_align((size_t)w.max_units * kHeadBlock * sizeof(float2));
+    w.part_o = off;    off += ws_align((size_t)w.max_units * kHeadBlock * D * sizeof(float));
+    w.total = off;
+    return w;
+}
+
+struct PlanPtrs {
+    int* hdr;
+    int4* req_info;
+    int2* items;   // {req, (qtile << 16) | head}
+    int4* units;   // {req, kvh | (hb << 16), page_start, page_count}
+};
+
+// largest i in [0, n) with base(i) <= e, base non-decreasing
+template <int FIELD>
+__device__ __forceinline__ int find_owner(const int4* __restrict__ info, int n, int e) {
+    int lo = 0, hi = n;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        const int4 v = info[mid];
+        const int base = FIELD == 1 ? v.y : v.w;
+        if (base <= e) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+constexpr int kPlanThreads = 1024;
+
+__global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P) {
+    __shared__ int s_units[kPlanThreads], s_items[kPlanThreads];
+    __shared__ int s_pages;
+    const int tid = threadIdx.x;
+    const int g = Hq / Hkv;
+    const int HB = (g + kHeadBlock - 1) / kHeadBlock;
+    const int n = b.num_reqs;
+    const int chunk = (n + kPlanThreads - 1) / kPlanThreads;
+    const int i0 = tid * chunk, i1 = min(n, i0 + chunk);
+
+    if (tid == 0) s_pages = 0;
+    __syncthreads();
+    int my_pages = 0;
+    for (int i = i0; i < i1; ++i)
+        if (b.q_lens[i] == 1) my_pages += (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+    if (my_pages) atomicAdd(&s_pages, my_pages);
+    __syncthreads();
+    const long long page_heads = (long long)s_pages * Hkv * HB;
+    int split = (int)((page_heads + kTargetUnits - 1) / kTargetUnits);
+    if (split < kMinSplitPages) split = kMinSplitPages;
+
+    int my_units = 0, my_items = 0;
+    for (int i = i0; i < i1; ++i) {
+        const int q = b.q_lens[i];
+        if (q == 1) {
+            const int pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+            my_units += ((pages + split - 1) / split) * Hkv * HB;
+        } else if (q > 1) {
+            my_items += ((q + kQTile - 1) / kQTile) * Hq;
+        }
+    }
+    s_units[tid] = my_units;
+    s_items[tid] = my_items;
+    __syncthreads();
+    for (int off = 1; off < kPlanThreads; off <<= 1) {  // inclusive Hillis-Steele scan
+        int u = 0, it = 0;
+        if (tid >= off) { u = s_units[tid - off]; it = s_items[tid - off]; }
+        __syncthreads();
+        s_units[tid] += u;
+        s_items[tid] += it;
+        __syncthreads();
+    }
+    int ubase = s_units[tid] - my_units, ibase = s_items[tid] - my_items;
+    const int n_units = s_units[kPlanThreads - 1], n_items = s_items[kPlanThreads - 1];
+    for (int i = i0; i < i1; ++i) {
+        const int q = b.q_lens[i];
+        int4 info = make_int4(0, ubase, 0, ibase);
+        if (q == 1) {
+            const int pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+            info.x = 1;
+            info.z = (pages + split - 1) / split;
+            ubase += info.z * Hkv * HB;
+        } else if (q > 1) {
+            info.x = 2;
+            ibase += ((q + kQTile - 1) / kQTile) * Hq;
+        }
+        P.req_info[i] = info;
+    }
+    if (tid == 0) {
+        P.hdr[HDR_N_ITEMS] = n_items;
+        P.hdr[HDR_N_UNITS] = n_units;
+        P.hdr[HDR_SPLIT_PAGES] = split;
+        P.hdr[HDR_TICKET_PREFILL] = 0;
+        P.hdr[HDR_TICKET_DECODE] = 0;
+    }
+    __syncthreads();  // req_info visible to the whole block (same-block global writes + barrier)
+
+    for (int e = tid; e < n_units; e += kPlanThreads) {
+        const int i = find_owner<1>(P.req_info, n, e);
+        const int4 info = P.req_info[i];
+        const int u = e - info.y;
+        const int hb = u % HB;
+        const int s = (u / HB) % info.z;
+        const int kvh = u / (HB * info.z);
+        const int pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+        const int p0 = s * split;
+        P.units[e] = make_int4(i, kvh | (hb << 16), p0, min(split, pages - p0));
+    }
+    for (int e = tid; e < n_items; e += kPlanThreads) {
+        const int i = find_owner<3>(P.req_info, n, e);
+        const int4 info = P.req_info[i];
+        const int local = e - info.w;
+        const int ntile = (b.q_lens[i] + kQTile - 1) / kQTile;
+        const int qt = ntile - 1 - local / Hq;  // heaviest (most KV tiles) first
+        P.items[e] = make_int2(i, (qt << 16) | (local % Hq));
+    }
+}
+
+}  // namespace tropical

@@ -1,0 +1,7 @@
+#pragma once
+#include <cuda.h>
+
+namespace tropical {
+bool encode_pool_map(CUtensorMap* map, const void* base, long long rows, int D);
+bool encode_q_map(CUtensorMap* map, const void* base, int T, int Hq, int D);
+}  // namespace tropical

@@ -9,6 +9,7 @@ import pytest
 import torch
 
 import oracle
+import paper_2606_16264_b200 as tb
 import synth
 from synth import f32_to_bf16_bits
 from tests.gpu_harness import MAX_ABS_TOL, MEAN_ABS_TOL, DeviceStep, bits, errors
@@ -50,7 +51,7 @@ def test_C1_gather_bit_exact():
     dev.append()
     for i in range(s.num_reqs):
         n = int(s.ctx_lens[i] + s.q_lens[i])
-        kd, vd = dev.tb.kv_gather(dev.pool, dev.batch, i, n)
+        kd, vd = tb.kv_gather(dev.pool, dev.batch, i, n)
         ok, ov = oracle.kv_gather(kp, vp, s.page_table, i, n)
         assert np.array_equal(bits(kd), ok) and np.array_equal(bits(vd), ov)
 
