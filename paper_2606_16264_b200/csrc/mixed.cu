@@ -6,6 +6,7 @@
 #include "decode.cuh"
 #include "kernels.h"
 #include "plan.cuh"
+#include "prefill.cuh"
 #include "tma_host.h"
 
 namespace tropical {
@@ -32,6 +33,40 @@ decode_kernel(DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __gr
     decode_warp_worker<D, kDecodeStages>(A, &tm_k, &tm_v, smem + warp * kDecodeStages * C::STAGE_BYTES,
                                          bars + warp * kDecodeStages, it);
     (void)lane;
+}
+
+
+constexpr int kPrefillThreads = 192;  // warps 0-3 softmax, warp 4 TMA producer, warp 5 MMA issuer
+
+template <int D>
+__global__ void __launch_bounds__(kPrefillThreads, 1)
+prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+               const __grid_constant__ CUtensorMap tm_v) {
+    using C = PrefillCfg<D>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    PrefillBars* B = reinterpret_cast<PrefillBars*>(tiles + C::SMEM_TILES);
+    const int warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        tma_prefetch_desc(&tm_q);
+        tma_prefetch_desc(&tm_k);
+        tma_prefetch_desc(&tm_v);
+        prefill_init_bars(B);
+        fence_mbar_init();
+    }
+    if (warp == 0) {
+        tmem_alloc(&B->tmem_base, C::TM_COLS);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    if (warp < 4) prefill_softmax<D>(A, B, warp);
+    else if (warp == 4) prefill_producer<D>(A, B, tiles, &tm_q, &tm_k, &tm_v);
+    else prefill_mma<D>(A, B, tiles);
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(B->tmem_base, C::TM_COLS);
 }
 
 template <int D>
@@ -72,15 +107,40 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     if (e != cudaSuccess) return e;
     ++*launches;
 
-    // prefill rows (q_i >= 2): CUDA-core kernel until the tcgen05 tile path lands
-    e = launch_attention_simt(pool, b, q, out, lse, scale_log2, stream, /*skip_decode=*/true);
-    if (e != cudaSuccess) return e;
-    ++*launches;
-
-    CUtensorMap tm_k, tm_v;
+    CUtensorMap tm_q, tm_k, tm_v;
     const long long rows = (long long)pool.num_pages * pool.Hkv * kPageSize;
-    if (!encode_pool_map(&tm_k, pool.k_pool, rows, D) || !encode_pool_map(&tm_v, pool.v_pool, rows, D))
+    if (!encode_pool_map(&tm_k, pool.k_pool, rows, D) || !encode_pool_map(&tm_v, pool.v_pool, rows, D) ||
+        !encode_q_map(&tm_q, q, b.total_q, pool.Hq, D))
         return cudaErrorInvalidValue;
+
+    // A3: prefill tiles (q_i >= 2) on tcgen05
+    {
+        PrefillArgs PA;
+        PA.pool = pool;
+        PA.b = b;
+        PA.out = (uint16_t*)out;
+        PA.lse = lse;
+        PA.scale_log2 = scale_log2;
+        PA.hdr = P.hdr;
+        PA.ticket = P.hdr + HDR_TICKET_PREFILL;
+        PA.items = P.items;
+        const size_t smem_p = (size_t)PrefillCfg<D>::SMEM_TILES + sizeof(PrefillBars) + 1024;
+        static bool attr_p = false;
+        if (!attr_p) {
+            e = cudaFuncSetAttribute(prefill_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p);
+            if (e != cudaSuccess) return e;
+            attr_p = true;
+        }
+        int grid_p = (b.total_q / 2) * pool.Hq;  // upper bound of items worth a CTA; every q_i >= 2 row pair
+        if (grid_p > num_sms()) grid_p = num_sms();
+        if (grid_p > 0) {
+            prefill_kernel<D><<<grid_p, kPrefillThreads, smem_p, stream>>>(PA, tm_q, tm_k, tm_v);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            ++*launches;
+        }
+    }
+
     DecodeArgs A;
     A.pool = pool;
     A.b = b;

@@ -1,0 +1,369 @@
+// prefill.cuh -- SURVEY.md 8(a) row A3: prefill tiles on the 5th-gen tensor cores.
+//
+// Item = (request i, 128-row query tile qt, q head h).  For every 128-key KV tile kt that the
+// item's rows can see (keys j <= c_i + t, bottom-right aligned causal mask):
+//     S  = Q K^T          tcgen05.mma kind::f16, A = Q (smem, K-major SW128), B = K (smem, K-major
+//                         SW128), fp32 accumulator in TMEM (two S slots, alternating per KV tile)
+//     P  = exp2(S*scale*log2e - m)   one thread per query row (tcgen05.ld 32x32b), fp32 online
+//                         softmax with lazy rescale of O, P written back to TMEM as packed bf16
+//                         over the S slot it came from
+//     O += P V            tcgen05.mma, A = P (TMEM), B = V (smem, MN-major SW128), fp32 in TMEM
+// and finally out = O / l (bf16), lse = ln2 * (m + log2 l).
+//
+// Three warp roles, all persistent over the item queue (tickets popped by the producer and
+// handed to the other roles through a 2-deep shared-memory mailbox):
+//   producer warp : TMA. Q tile (3-D map, 2 boxes) and, per KV tile, the 8 page-heads of K and of V
+//                   (2-D map, one 64-col x 16-row SW128 box per page-head half, issued by 16 lanes in
+//                   parallel) into 2-stage K and V rings.  The HND pool makes every box one
+//                   contiguous 2 KiB run of HBM/L2.
+//   MMA warp      : one elected lane issues S(kt+1) ahead of PV(kt) so the tensor pipe works on
+//                   the next scores while the softmax warps work on the current ones.
+//   softmax warps : 4 warps, thread r owns query row r (TMEM lane r): no shuffles.
+// Unused slots of a request's last page may hold NaN bit patterns: scores are masked by select,
+// and the V rows past the last visible key of the last tile are zeroed in shared memory before
+// PV is issued (0 * NaN would poison the whole accumulator column).
+#pragma once
+#include <cuda.h>
+
+#include "common.cuh"
+#include "plan.cuh"
+
+namespace tropical {
+
+template <int D>
+struct PrefillCfg {
+    static constexpr int CB = D / 64;                    // 64-column (128-byte) swizzle halves per row
+    static constexpr int HALF_BYTES = kKvTile * 128;     // one half of a 128-row tile: 16 KiB
+    static constexpr int TILE_BYTES = CB * HALF_BYTES;   // Q tile / K tile / V tile
+    static constexpr int PAGE_BOX = kPageSize * 128;     // one TMA box: 16 rows x 128 B
+    static constexpr int KV_STAGES = 2;
+    static constexpr int SMEM_TILES = TILE_BYTES * (1 + 2 * KV_STAGES);
+    // TMEM columns: S slot 0 at 0, S slot 1 at 128, O at 256
+    static constexpr uint32_t TM_S = 0, TM_O = 256, TM_COLS = 512;
+};
+
+// mbarriers of the prefill role set
+struct PrefillBars {
+    uint64_t item_full[2], item_empty[2];
+    uint64_t q_full, q_empty;
+    uint64_t k_full[2], k_empty[2], v_full[2], v_empty[2];
+    uint64_t s_full[2], p_full[2];
+    uint64_t pv_done, o_empty;
+    int mailbox[2];
+    uint32_t tmem_base;
+};
+
+struct PrefillArgs {
+    PoolDesc pool;
+    BatchDesc b;
+    uint16_t* out;
+    float* lse;
+    float scale_log2;
+    const int* hdr;
+    int* ticket;
+    const int2* items;
+};
+
+struct PrefillItem {
+    int req, qt, h, hk;
+    int c, ql, tok0;   // context length, chunk length, first packed row of the request
+    int l_tile;        // keys visible to the last row of the tile: c + min(ql, (qt+1)*128)
+    int n_kt;          // KV tiles
+};
+
+__device__ __forceinline__ PrefillItem load_item(const PrefillArgs& A, int id) {
+    PrefillItem it;
+    const int2 v = A.items[id];
+    it.req = v.x;
+    it.qt = v.y >> 16;
+    it.h = v.y & 0xffff;
+    it.hk = it.h / (A.pool.Hq / A.pool.Hkv);
+    it.c = __ldg(A.b.ctx_lens + it.req);
+    it.ql = __ldg(A.b.q_lens + it.req);
+    it.tok0 = __ldg(A.b.q_offsets + it.req);
+    it.l_tile = it.c + min(it.ql, (it.qt + 1) * kQTile);
+    it.n_kt = (it.l_tile + kKvTile - 1) / kKvTile;
+    return it;
+}
+
+__device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
+    for (int i = 0; i < 2; ++i) {
+        mbar_init(&B->item_full[i], 1);
+        mbar_init(&B->item_empty[i], 5);  // MMA lane 0 + lane 0 of each softmax warp
+        mbar_init(&B->k_full[i], 1);
+        mbar_init(&B->k_empty[i], 1);
+        mbar_init(&B->v_full[i], 1);
+        mbar_init(&B->v_empty[i], 1);
+        mbar_init(&B->s_full[i], 1);
+        mbar_init(&B->p_full[i], 128);
+    }
+    mbar_init(&B->q_full, 1);
+    mbar_init(&B->q_empty, 1);
+    mbar_init(&B->pv_done, 1);
+    mbar_init(&B->o_empty, 128);
+}
+
+// ------------------------------------------------------------------------------------------------
+// producer warp
+template <int D>
+__device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBars* B, uint8_t* tiles,
+                                                 const CUtensorMap* tm_q, const CUtensorMap* tm_k,
+                                                 const CUtensorMap* tm_v) {
+    using C = PrefillCfg<D>;
+    const int lane = threadIdx.x & 31;
+    const int n_items = A.hdr[HDR_N_ITEMS];
+    uint8_t* q_s = tiles;
+    uint8_t* k_s = tiles + C::TILE_BYTES;
+    uint8_t* v_s = tiles + C::TILE_BYTES * (1 + C::KV_STAGES);
+    uint32_t item_it = 0, kv_it = 0;
+    for (;;) {
+        const int ms = item_it & 1;
+        mbar_wait(&B->item_empty[ms], ((item_it >> 1) & 1) ^ 1);
+        int id = 0;
+        if (lane == 0) {
+            id = atomicAdd(A.ticket, 1);
+            B->mailbox[ms] = id;
+            mbar_arrive(&B->item_full[ms]);
+        }
+        id = __shfl_sync(0xffffffffu, id, 0);
+        if (id >= n_items) break;
+        const PrefillItem it = load_item(A, id);
+        const int* pt = A.b.page_table + (size_t)it.req * A.b.stride;
+
+        mbar_wait(&B->q_empty, (item_it & 1) ^ 1);
+        if (lane == 0) {
+            mbar_arrive_expect_tx(&B->q_full, C::TILE_BYTES);
+#pragma unroll
+            for (int cb = 0; cb < C::CB; ++cb)
+                tma_load_3d(q_s + cb * C::HALF_BYTES, tm_q, cb * 64, it.h, it.tok0 + it.qt * kQTile, &B->q_full);
+        }
+        const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
+        for (int kt = 0; kt < it.n_kt; ++kt, ++kv_it) {
+            const int st = kv_it & 1;
+            const uint32_t par = ((kv_it >> 1) & 1) ^ 1;
+            const int np = min(8, n_pages - kt * 8);
+            // lane -> (page p, half cb) of this tile
+            const int p = lane / C::CB, cb = lane % C::CB;
+            const bool act = p < np && lane < 8 * C::CB;
+            const int page = act ? __ldg(pt + kt * 8 + p) : 0;
+            const int r0 = (page * A.pool.Hkv + it.hk) * kPageSize;
+            const uint32_t off = cb * C::HALF_BYTES + p * C::PAGE_BOX;
+
+            mbar_wait(&B->k_empty[st], par);
+            if (lane == 0) mbar_arrive_expect_tx(&B->k_full[st], np * C::CB * C::PAGE_BOX);
+            __syncwarp();
+            if (act) tma_load_2d(k_s + st * C::TILE_BYTES + off, tm_k, cb * 64, r0, &B->k_full[st]);
+
+            mbar_wait(&B->v_empty[st], par);
+            if (lane == 0) mbar_arrive_expect_tx(&B->v_full[st], np * C::CB * C::PAGE_BOX);
+            __syncwarp();
+            if (act) tma_load_2d(v_s + st * C::TILE_BYTES + off, tm_v, cb * 64, r0, &B->v_full[st]);
+        }
+        ++item_it;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// MMA warp
+template <int D>
+__device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B, uint8_t* tiles) {
+    using C = PrefillCfg<D>;
+    const int lane = threadIdx.x & 31;
+    const int n_items = A.hdr[HDR_N_ITEMS];
+    const uint32_t q_a = smem_u32(tiles);
+    const uint32_t k_a = q_a + C::TILE_BYTES;
+    const uint32_t v_a = q_a + C::TILE_BYTES * (1 + C::KV_STAGES);
+    const uint32_t tm = B->tmem_base;
+    constexpr uint32_t IDESC_S = make_idesc_bf16(128, 128, false);
+    constexpr uint32_t IDESC_O = make_idesc_bf16(128, D, true);
+    uint32_t item_it = 0, kv_it = 0;
+
+    auto issue_s = [&](uint32_t g) {  // S(g) = Q K^T into S slot g & 1
+        const int st = g & 1;
+        mbar_wait(&B->k_full[st], (g >> 1) & 1);
+        tc_fence_after();
+        if (lane == 0) {
+#pragma unroll
+            for (int cb = 0; cb < C::CB; ++cb)
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) {
+                    const uint32_t o = cb * C::HALF_BYTES + k4 * 32;
+                    tc_mma_ss(tm + C::TM_S + st * 128, make_smem_desc_sw128(q_a + o, 0, 1024),
+                              make_smem_desc_sw128(k_a + st * C::TILE_BYTES + o, 0, 1024), IDESC_S, (cb | k4) != 0);
+                }
+            tc_commit(&B->s_full[st]);
+            tc_commit(&B->k_empty[st]);
+        }
+        __syncwarp();
+    };
+
+    for (;;) {
+        const int ms = item_it & 1;
+        mbar_wait(&B->item_full[ms], (item_it >> 1) & 1);
+        const int id = B->mailbox[ms];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&B->item_empty[ms]);
+        if (id >= n_items) break;
+        const PrefillItem it = load_item(A, id);
+
+        mbar_wait(&B->q_full, item_it & 1);
+        issue_s(kv_it);
+        for (int kt = 0; kt < it.n_kt; ++kt) {
+            const uint32_t g = kv_it + kt;
+            const int st = g & 1;
+            if (kt + 1 < it.n_kt) {
+                issue_s(g + 1);
+            } else {
+                if (lane == 0) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
+                __syncwarp();
+            }
+            mbar_wait(&B->v_full[st], (g >> 1) & 1);
+            if (kt + 1 == it.n_kt) {  // zero V rows past the last visible key (stale or poisoned smem)
+                const int nvalid = it.l_tile - kt * kKvTile;
+                const int nz = (kKvTile - nvalid) * 8 * C::CB;
+                for (int idx = lane; idx < nz; idx += 32) {
+                    const int r = nvalid + idx / (8 * C::CB), rem = idx % (8 * C::CB);
+                    const uint32_t a = v_a + st * C::TILE_BYTES + (rem >> 3) * C::HALF_BYTES + r * 128 + ((rem & 7) << 4);
+                    asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                }
+                fence_proxy_async();
+                __syncwarp();
+            }
+            if (kt == 0) mbar_wait(&B->o_empty, (item_it & 1) ^ 1);  // previous item's epilogue has read O
+            mbar_wait(&B->p_full[st], (g >> 1) & 1);
+            tc_fence_after();
+            if (lane == 0) {
+#pragma unroll
+                for (int ks = 0; ks < 8; ++ks)  // 16 keys per MMA
+                    tc_mma_ts(tm + C::TM_O, tm + C::TM_S + st * 128 + ks * 8,
+                              make_smem_desc_sw128(v_a + st * C::TILE_BYTES + ks * 2048, C::HALF_BYTES, 1024), IDESC_O,
+                              (kt | ks) != 0);
+                tc_commit(&B->v_empty[st]);
+                tc_commit(&B->pv_done);
+            }
+            __syncwarp();
+        }
+        kv_it += it.n_kt;
+        ++item_it;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// softmax warps (4 warps, 128 threads: thread r <-> query row r <-> TMEM lane r)
+__device__ __forceinline__ float max4(float a, float b, float c, float d) { return fmaxf(fmaxf(a, b), fmaxf(c, d)); }
+
+template <int D>
+__device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBars* B, int wg_warp) {
+    using C = PrefillCfg<D>;
+    const int lane = threadIdx.x & 31;
+    const int r = wg_warp * 32 + lane;
+    const int n_items = A.hdr[HDR_N_ITEMS];
+    const uint32_t tm = B->tmem_base + ((uint32_t)(wg_warp * 32) << 16);
+    const float scale = A.scale_log2;
+    uint32_t item_it = 0, kv_it = 0;
+
+    for (;;) {
+        const int ms = item_it & 1;
+        mbar_wait(&B->item_full[ms], (item_it >> 1) & 1);
+        const int id = B->mailbox[ms];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&B->item_empty[ms]);
+        if (id >= n_items) break;
+        const PrefillItem it = load_item(A, id);
+        const int t = it.qt * kQTile + r;
+        const int limit = it.c + min(t, it.ql - 1);  // last visible key of this row (rows past the chunk mirror its last row)
+        float m_used = 0.f, l = 0.f;
+
+        for (int kt = 0; kt < it.n_kt; ++kt) {
+            const uint32_t g = kv_it + kt;
+            const int st = g & 1;
+            mbar_wait(&B->s_full[st], (g >> 1) & 1);
+            tc_fence_after();
+            uint32_t s[128];
+#pragma unroll
+            for (int c4 = 0; c4 < 4; ++c4) tmem_ld_32x32(tm + C::TM_S + st * 128 + c4 * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c4 * 32]));
+            tc_wait_ld();
+            const int n_vis = limit - kt * kKvTile + 1;  // visible columns of this tile for this row
+            if (n_vis < kKvTile) {
+#pragma unroll
+                for (int j = 0; j < 128; ++j)
+                    if (j >= n_vis) s[j] = 0xff800000u;  // -inf, by select: the score may be NaN
+            }
+            float mx = -INFINITY;
+#pragma unroll
+            for (int j = 0; j < 128; j += 4)
+                mx = fmaxf(mx, max4(__uint_as_float(s[j]), __uint_as_float(s[j + 1]), __uint_as_float(s[j + 2]),
+                                    __uint_as_float(s[j + 3])));
+            const float m_new = mx * scale;
+            if (kt == 0) {
+                m_used = m_new;  // finite: key 0 is visible to every row
+            } else {
+                const bool grow = m_new > m_used + 8.f;  // lazy rescale: P stays <= 2^8
+                if (__any_sync(0xffffffffu, grow)) {
+                    const float alpha = grow ? fast_exp2(m_used - m_new) : 1.f;
+                    mbar_wait(&B->pv_done, (g - 1) & 1);  // O holds PV(g-1)
+                    tc_fence_after();
+#pragma unroll
+                    for (int c4 = 0; c4 < D / 32; ++c4) {
+                        uint32_t o[32];
+                        tmem_ld_32x32(tm + C::TM_O + c4 * 32, o);
+                        tc_wait_ld();
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                        tmem_st_32x32(tm + C::TM_O + c4 * 32, o);
+                    }
+                    l *= alpha;
+                    if (grow) m_used = m_new;
+                }
+            }
+            float sum0 = 0.f, sum1 = 0.f;
+            uint32_t pk[64];
+#pragma unroll
+            for (int j = 0; j < 128; j += 2) {
+                const float p0 = fast_exp2(fmaf(__uint_as_float(s[j]), scale, -m_used));
+                const float p1 = fast_exp2(fmaf(__uint_as_float(s[j + 1]), scale, -m_used));
+                sum0 += p0;
+                sum1 += p1;
+                pk[j >> 1] = pack_bf16x2(p0, p1);
+            }
+            l += sum0 + sum1;
+            tmem_st_32x32(tm + C::TM_S + st * 128, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
+            tmem_st_32x32(tm + C::TM_S + st * 128 + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
+            tc_wait_st();
+            tc_fence_before();
+            mbar_arrive(&B->p_full[st]);
+        }
+        kv_it += it.n_kt;
+
+        // epilogue: out = O / l
+        mbar_wait(&B->pv_done, (kv_it - 1) & 1);
+        tc_fence_after();
+        const float inv = 1.f / l;
+        const bool valid = t < it.ql;
+        uint16_t* orow = A.out + ((size_t)(it.tok0 + t) * A.pool.Hq + it.h) * D;
+#pragma unroll
+        for (int c4 = 0; c4 < D / 32; ++c4) {
+            uint32_t o[32];
+            tmem_ld_32x32(tm + C::TM_O + c4 * 32, o);
+            tc_wait_ld();
+            if (valid) {
+#pragma unroll
+                for (int j = 0; j < 32; j += 8) {
+                    uint4 w;
+                    w.x = pack_bf16x2(__uint_as_float(o[j]) * inv, __uint_as_float(o[j + 1]) * inv);
+                    w.y = pack_bf16x2(__uint_as_float(o[j + 2]) * inv, __uint_as_float(o[j + 3]) * inv);
+                    w.z = pack_bf16x2(__uint_as_float(o[j + 4]) * inv, __uint_as_float(o[j + 5]) * inv);
+                    w.w = pack_bf16x2(__uint_as_float(o[j + 6]) * inv, __uint_as_float(o[j + 7]) * inv);
+                    *reinterpret_cast<uint4*>(orow + c4 * 32 + j) = w;
+                }
+            }
+        }
+        tc_fence_before();
+        mbar_arrive(&B->o_empty);
+        if (valid && A.lse != nullptr)
+            A.lse[(size_t)(it.tok0 + t) * A.pool.Hq + it.h] = (m_used + log2f(l)) * 0.6931471805599453f;
+        ++item_it;
+    }
+}
+
+}  // namespace tropical
