@@ -149,6 +149,7 @@ def run_ours(args, rank, world):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl")
+    tb.debug_set_mode(1 if args.mode == "split" else 0)
     s, gen_s = make_workload(args.config, rank)
     cnt = step_counts((s.num_q_heads, s.num_kv_heads, s.head_dim, s.page_size, s.q_lens, s.ctx_lens))
     peaks = load_peaks()
@@ -228,7 +229,10 @@ def run_ours(args, rank, world):
     t_roof = max(t_bytes_us, t_flops_us)
     attn_us = attn_ms * 1e3
     achieved = cnt["attn_bytes"] / (attn_us * 1e3)  # GB/s
-    cpu_us, cpu_desc, cores, _ = oracle_sample_us(s)
+    if args.no_cpu:
+        cpu_us, cpu_desc, cores = float("nan"), "skipped (--no-cpu)", 0
+    else:
+        cpu_us, cpu_desc, cores, _ = oracle_sample_us(s)
     line = {
         "metric": METRIC, "value": round(us, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 5), "higher_is_better": False,
@@ -236,7 +240,7 @@ def run_ours(args, rank, world):
         "config": {"workload": f"{args.config} ({describe(args.config)})", "replicas": world,
                    "l2": "step touches %.2f GB >> 126 MB L2, no flush needed" % (cnt["step_bytes"] / 1e9)
                    if cnt["step_bytes"] > 5e8 else "L2 flushed between steps: NO (working set fits L2; warm number)",
-                   "new_tokens_per_step": int(cnt["new_tokens"])},
+                   "new_tokens_per_step": int(cnt["new_tokens"]), "mode": args.mode},
         "tokens_per_s": round(cnt["new_tokens"] * world / (us * 1e-6), 1),
         "step_roofline": {"t_bytes_us": round(t_bytes_us, 2), "t_flops_us": round(t_flops_us, 2),
                           "t_roof_us": round(t_roof, 2), "frac": round(t_roof / us, 4),
@@ -294,6 +298,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", default="C5", choices=synth.CONFIG_NAMES)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--mode", default="fused", choices=["fused", "split"],
+                    help="fused = the product path (one persistent step kernel); split = separate prefill/decode "
+                         "launches of the same tile code, for A/B timing only")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))

@@ -162,6 +162,11 @@ int tropical_debug_attention_simt(const tropical_kv_pool_t *pool, const tropical
                                   const void *q, void *out, float *lse, float sm_scale,
                                   void *cuda_stream);
 
+/* Test / measurement hook: 0 (default) = the fused step kernel, prefill tiles and decode tiles in one
+ * persistent launch; 1 = the same tile code as separate prefill and decode
+ * launches, kept only to time the two phases apart (A/B evidence under profiles/).  Process-global. */
+void tropical_debug_set_mode(int mode);
+
 const char *tropical_status_string(int status);
 const char *tropical_last_cuda_error(void); /* thread-local text of the last CUDA failure */
 const char *tropical_version(void);

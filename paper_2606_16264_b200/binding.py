@@ -49,7 +49,7 @@ EXPORTS = (
     "tropical_kv_append", "tropical_kv_gather", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
-    "tropical_debug_attention_simt",
+    "tropical_debug_attention_simt", "tropical_debug_set_mode",
 )
 
 
@@ -86,6 +86,11 @@ def status_string(status: int) -> str:
 
 def version() -> str:
     return lib().tropical_version().decode()
+
+
+def debug_set_mode(mode: int) -> None:
+    """0 = fused step kernel (default, the product path); 1 = separate prefill / decode launches (timing A/B)."""
+    lib().tropical_debug_set_mode(ctypes.c_int(int(mode)))
 
 
 def last_launch_count() -> int:

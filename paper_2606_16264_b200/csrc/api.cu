@@ -255,6 +255,8 @@ const char* tropical_status_string(int s) {
     }
 }
 
+void tropical_debug_set_mode(int mode) { set_debug_mode(mode == 1 ? 1 : 0); }
+
 const char* tropical_last_cuda_error(void) { return g_cuda_err; }
 
 const char* tropical_version(void) { return "tropical-b200 0.1 (sm_100a)"; }

@@ -69,6 +69,74 @@ prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __
     if (warp == 0) tmem_dealloc(B->tmem_base, C::TM_COLS);
 }
 
+// ------------------------------------------------------------------------------------------------
+// The fused step kernel: ONE persistent launch, one CTA per SM, three warpgroups.
+//   WG0 (warps 0-3)  : prefill softmax / correction / epilogue    (registers grown with setmaxnreg)
+//   WG1 (warps 4-7)  : decode workers, one private TMA ring each  (HBM streaming)
+//   WG2 (warps 8-11) : warp 8 prefill TMA producer, warp 9 tcgen05 MMA issuer, 10-11 spare (registers shrunk)
+// Prefill items and decode units are popped from two ticket counters, so on every SM the tensor
+// pipe (prefill) and the HBM stream (decode) are busy at the same time for the whole step.
+constexpr int kMixedThreads = 384;
+
+template <int D>
+struct MixedCfg {
+    static constexpr int DEC_WARPS = 4;
+    static constexpr int DEC_RING = 16384;  // bytes of TMA ring per decode warp
+    static constexpr int DEC_STAGES = DEC_RING / DecodeCfg<D>::STAGE_BYTES;
+    static constexpr int BAR_BYTES = 1024;
+    static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_WARPS * DEC_RING + BAR_BYTES + 1024;
+};
+
+struct MixedBars {
+    PrefillBars p;
+    uint64_t dec_full[32];
+};
+
+template <int D>
+__global__ void __launch_bounds__(kMixedThreads, 1)
+mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap tm_q,
+             const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
+    using C = PrefillCfg<D>;
+    using M = MixedCfg<D>;
+    static_assert(sizeof(MixedBars) <= M::BAR_BYTES, "barrier block");
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* rings = tiles + C::SMEM_TILES;
+    MixedBars* B = reinterpret_cast<MixedBars*>(rings + M::DEC_WARPS * M::DEC_RING);
+    const int warp = threadIdx.x >> 5, wg = warp >> 2;
+    if (threadIdx.x == 0) {
+        tma_prefetch_desc(&tm_q);
+        tma_prefetch_desc(&tm_k);
+        tma_prefetch_desc(&tm_v);
+        prefill_init_bars(&B->p);
+        for (int i = 0; i < M::DEC_WARPS * M::DEC_STAGES; ++i) mbar_init(&B->dec_full[i], 1);
+        fence_mbar_init();
+    }
+    if (warp == 0) {
+        tmem_alloc(&B->p.tmem_base, C::TM_COLS);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    if (wg == 0) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
+        prefill_softmax<D>(PA, &B->p, warp);
+    } else if (wg == 1) {
+        const int dw = warp - 4;
+        uint32_t it = 0;
+        decode_warp_worker<D, M::DEC_STAGES>(DA, &tm_k, &tm_v, rings + dw * M::DEC_RING,
+                                             &B->dec_full[dw * M::DEC_STAGES], it);
+    } else {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+        if (warp == 8) prefill_producer<D>(PA, &B->p, tiles, &tm_q, &tm_k, &tm_v);
+        else if (warp == 9) prefill_mma<D>(PA, &B->p, tiles);
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(B->p.tmem_base, C::TM_COLS);
+}
+
 template <int D>
 __global__ void __launch_bounds__(128) combine_kernel(CombineArgs A) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -92,6 +160,9 @@ size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q) 
     return make_layout(Hq, Hkv, D, num_reqs, total_q).total;
 }
 
+static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches (A/B timing only)
+void set_debug_mode(int mode) { g_mode = mode; }
+
 template <int D>
 static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
                                   float scale_log2, void* workspace, cudaStream_t stream, int* launches) {
@@ -113,17 +184,45 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
         !encode_q_map(&tm_q, q, b.total_q, pool.Hq, D))
         return cudaErrorInvalidValue;
 
-    // A3: prefill tiles (q_i >= 2) on tcgen05
-    {
-        PrefillArgs PA;
-        PA.pool = pool;
-        PA.b = b;
-        PA.out = (uint16_t*)out;
-        PA.lse = lse;
-        PA.scale_log2 = scale_log2;
-        PA.hdr = P.hdr;
-        PA.ticket = P.hdr + HDR_TICKET_PREFILL;
-        PA.items = P.items;
+    PrefillArgs PA;
+    PA.pool = pool;
+    PA.b = b;
+    PA.out = (uint16_t*)out;
+    PA.lse = lse;
+    PA.scale_log2 = scale_log2;
+    PA.hdr = P.hdr;
+    PA.ticket = P.hdr + HDR_TICKET_PREFILL;
+    PA.items = P.items;
+
+    DecodeArgs A;
+    A.pool = pool;
+    A.b = b;
+    A.q = (const uint16_t*)q;
+    A.out = (uint16_t*)out;
+    A.lse = lse;
+    A.scale_log2 = scale_log2;
+    A.hdr = P.hdr;
+    A.ticket = P.hdr + HDR_TICKET_DECODE;
+    A.req_info = P.req_info;
+    A.units = P.units;
+    A.part_ml = (float2*)(ws + w.part_ml);
+    A.part_o = (float*)(ws + w.part_o);
+
+    if (g_mode == 0) {
+        // A3 + A4 in one persistent launch
+        const size_t smem = MixedCfg<D>::SMEM;
+        static bool attr_m = false;
+        if (!attr_m) {
+            e = cudaFuncSetAttribute(mixed_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            attr_m = true;
+        }
+        mixed_kernel<D><<<num_sms(), kMixedThreads, smem, stream>>>(PA, A, tm_q, tm_k, tm_v);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        ++*launches;
+    } else {
+        // A3: prefill tiles (q_i >= 2) on tcgen05
         const size_t smem_p = (size_t)PrefillCfg<D>::SMEM_TILES + sizeof(PrefillBars) + 1024;
         static bool attr_p = false;
         if (!attr_p) {
@@ -139,32 +238,19 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
             if (e != cudaSuccess) return e;
             ++*launches;
         }
-    }
-
-    DecodeArgs A;
-    A.pool = pool;
-    A.b = b;
-    A.q = (const uint16_t*)q;
-    A.out = (uint16_t*)out;
-    A.lse = lse;
-    A.scale_log2 = scale_log2;
-    A.hdr = P.hdr;
-    A.ticket = P.hdr + HDR_TICKET_DECODE;
-    A.req_info = P.req_info;
-    A.units = P.units;
-    A.part_ml = (float2*)(ws + w.part_ml);
-    A.part_o = (float*)(ws + w.part_o);
-    const size_t smem = (size_t)kDecodeWarps * kDecodeStages * DecodeCfg<D>::STAGE_BYTES + 1024 + 256;
-    static bool attr_done = false;
-    if (!attr_done) {
-        e = cudaFuncSetAttribute(decode_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        // A4: decode tiles
+        const size_t smem = (size_t)kDecodeWarps * kDecodeStages * DecodeCfg<D>::STAGE_BYTES + 1024 + 256;
+        static bool attr_done = false;
+        if (!attr_done) {
+            e = cudaFuncSetAttribute(decode_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            attr_done = true;
+        }
+        decode_kernel<D><<<2 * num_sms(), kDecodeWarps * 32, smem, stream>>>(A, tm_k, tm_v);
+        e = cudaGetLastError();
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        ++*launches;
     }
-    decode_kernel<D><<<2 * num_sms(), kDecodeWarps * 32, smem, stream>>>(A, tm_k, tm_v);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    ++*launches;
 
     CombineArgs Cb;
     Cb.pool = pool;

@@ -222,6 +222,23 @@ def test_product_path_matches_simt_cross_check():
     assert np.abs(a - b).max() <= 2e-2 and np.abs(la - lb).max() <= 2e-3
 
 
+def test_split_launch_mode_matches_fused():
+    """The A/B timing mode (separate prefill / decode launches) runs the same tile code: same bits."""
+    s = _step(16, 16, 2, 128, [300, 1, 1, 1, 40], [0, 777, 4097, 15, 130])
+    dev = DeviceStep(s)
+    dev.step()
+    a = bits(dev.out).copy()
+    tb.debug_set_mode(1)
+    try:
+        dev.out.zero_()
+        dev.attention()
+        torch.cuda.synchronize()
+        b = bits(dev.out).copy()
+    finally:
+        tb.debug_set_mode(0)
+    assert np.array_equal(a, b)
+
+
 # ------------------------------------------------------------------ end-to-end host entry point
 def test_step_host_equals_device_path():
     import paper_2606_16264_b200 as tb
