@@ -191,6 +191,7 @@ def run_ours(args, rank, world):
         torch.cuda.synchronize()
     sampler.stop_flag = True
     sampler.join()
+    roles = tb.debug_read_profile(dev.workspace) if args.mode == "fused" else None
     if world > 1:
         t = torch.tensor([total_ms], device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -256,6 +257,7 @@ def run_ours(args, rank, world):
         "gpu_launches": int(launches_per_step) * args.steps,
         "clocks": sampler.summary(),
         "gen_seconds": round(gen_s, 1),
+        "role_finish_us": {k: round(v / 1e3, 1) for k, v in roles.items()} if roles else None,
     }
     print(json.dumps(line))
 

@@ -167,6 +167,12 @@ int tropical_debug_attention_simt(const tropical_kv_pool_t *pool, const tropical
  * launches, kept only to time the two phases apart (A/B evidence under profiles/).  Process-global. */
 void tropical_debug_set_mode(int mode);
 
+/* Measurement hook: role timestamps of the LAST fused step kernel that ran with this workspace
+ * (globaltimer nanoseconds): out_ns[0] kernel start (earliest CTA), [1] prefill queue drained (latest
+ * softmax warp), [2] latest dedicated decode warp done, [3] latest late-joining decode warp done.
+ * Copies 32 bytes device->host and synchronises the stream.  out_ns is [host]. */
+int tropical_debug_read_profile(const void *workspace, uint64_t *out_ns, void *cuda_stream);
+
 const char *tropical_status_string(int status);
 const char *tropical_last_cuda_error(void); /* thread-local text of the last CUDA failure */
 const char *tropical_version(void);

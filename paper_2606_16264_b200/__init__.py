@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     KVPool,
     TropicalError,
     debug_attention_simt,
+    debug_read_profile,
     debug_set_mode,
     kv_append,
     kv_gather,

@@ -49,7 +49,7 @@ EXPORTS = (
     "tropical_kv_append", "tropical_kv_gather", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
-    "tropical_debug_attention_simt", "tropical_debug_set_mode",
+    "tropical_debug_attention_simt", "tropical_debug_set_mode", "tropical_debug_read_profile",
 )
 
 
@@ -74,7 +74,8 @@ def lib():
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
     for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_mixed_attention", "tropical_step_host",
-                 "tropical_step_cost", "tropical_last_launch_count", "tropical_debug_attention_simt"):
+                 "tropical_step_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
+                 "tropical_debug_read_profile"):
         getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L
@@ -91,6 +92,16 @@ def version() -> str:
 def debug_set_mode(mode: int) -> None:
     """0 = fused step kernel (default, the product path); 1 = separate prefill / decode launches (timing A/B)."""
     lib().tropical_debug_set_mode(ctypes.c_int(int(mode)))
+
+
+def debug_read_profile(workspace: torch.Tensor, stream=None):
+    """Role timestamps (ns, relative to kernel start) of the last fused step kernel run with `workspace`:
+    dict(prefill_done, decode_done, late_decode_done); 0 = that role never ran."""
+    out = (ctypes.c_uint64 * 4)()
+    _check(lib().tropical_debug_read_profile(_ptr(_aligned(workspace)), out, _stream(stream)), "debug_read_profile")
+    t0 = int(out[0])
+    rel = lambda v: int(v) - t0 if int(v) else 0
+    return {"prefill_done": rel(out[1]), "decode_done": rel(out[2]), "late_decode_done": rel(out[3])}
 
 
 def last_launch_count() -> int:

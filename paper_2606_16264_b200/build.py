@@ -38,7 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc] + NVCC_FLAGS + ["-I", INCLUDE, "-o", tmp] + sources()
+    extra = os.environ.get("TROPICAL_NVCC_EXTRA", "").split()  # e.g. -DTROPICAL_DEBUG_WAIT (names a timed-out mbarrier wait)
+    cmd = [nvcc] + NVCC_FLAGS + extra + ["-I", INCLUDE, "-o", tmp] + sources()
     res = subprocess.run(cmd, capture_output=True, text=True)
     log = res.stdout + res.stderr
     with open(os.path.join(HERE, "build.log"), "w") as f:

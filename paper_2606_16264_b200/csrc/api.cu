@@ -255,6 +255,16 @@ const char* tropical_status_string(int s) {
     }
 }
 
+int tropical_debug_read_profile(const void* workspace, uint64_t* out_ns, void* cuda_stream) {
+    if (workspace == nullptr || out_ns == nullptr) return TROPICAL_ERR_INVALID_ARG;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaMemcpyAsync(out_ns, (const char*)workspace + profile_offset_bytes(), 4 * sizeof(uint64_t),
+                                    cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return cuda_fail(e, "read_profile");
+    return TROPICAL_OK;
+}
+
 void tropical_debug_set_mode(int mode) { set_debug_mode(mode == 1 ? 1 : 0); }
 
 const char* tropical_last_cuda_error(void) { return g_cuda_err; }

@@ -4,6 +4,7 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
 
 namespace tropical {
 
@@ -80,12 +81,21 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
     return ok != 0;
 }
 // Bounded wait: a protocol bug traps (launch failure) instead of hanging the GPU box.
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0, int aux = 0) {
     if (mbar_try_wait(bar, parity)) return;
     long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > 4000000000LL) __trap();  // ~2 s at 1.9 GHz
+        if (clock64() - t0 > 4000000000LL) {  // ~2 s at 1.9 GHz
+#ifdef TROPICAL_DEBUG_WAIT
+            if ((threadIdx.x & 31) == 0) printf("mbar timeout: block %d warp %d tag %d parity %u aux %d\n", blockIdx.x, threadIdx.x >> 5, tag, parity, aux);
+            long long t1 = clock64();
+            while (clock64() - t1 < 1500000000LL) {}  // let every stuck warp report before the trap
+#endif
+            __trap();
+        }
     }
+    (void)tag;
+    (void)aux;
 }
 
 __device__ __forceinline__ void fence_proxy_async() {

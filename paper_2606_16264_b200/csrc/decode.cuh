@@ -1,12 +1,20 @@
 // decode.cuh -- SURVEY.md 8(a) row A4: decode tiles (split-K flash decoding over pages).
 //
-// One WARP is one decode worker.  It pops a unit (request, kv head, head block, page range),
-// streams the unit's K and V page-heads HBM -> shared memory with TMA (two 64-column
-// SWIZZLE_128B boxes per 16 x d page-head, i.e. whole 4 KiB contiguous blocks of the HND pool,
-// landed bank-conflict-free for ldmatrix) through a private NSTAGE-deep mbarrier ring, and
-// consumes them with warp-level tensor-core MMAs whose M rows are the (up to 8) q heads of the
-// kv group: S = Q K^T (m16n8k16, fp32), online softmax in registers (quad shuffles), O += P V.
-// HBM-bound: each K/V byte is read once; arithmetic per byte is the same for MHA and GQA.
+// One WARP is one decode worker.  It pops a unit (request, kv head, head block, page range) and
+// streams the unit's K and V page-heads HBM -> shared memory with TMA (64-column SWIZZLE_128B
+// boxes, i.e. whole 4 KiB contiguous page-head blocks of the HND pool, landed bank-conflict-free
+// for ldmatrix) through a private ring of page-head sized stages -- K(p), V(p), K(p+1), V(p+1), ...,
+// one mbarrier each -- that is kept full: a stage is refilled as soon as the warp has read it, so
+// (ring - 1) page-heads are in flight per warp while one is consumed.
+// The math runs on warp-level tensor-core MMAs in the TRANSPOSED orientation, so the 16 keys of a
+// page are the M rows and the (up to 8) q heads of the kv group are the N columns:
+//     S^T[16 keys x 8 heads] = K[16 x d] Q^T[d x 8]          (A = K page via ldmatrix, B = q registers)
+//     O^T[d x 8 heads]      += V^T[d x 16 keys] P^T[16 x 8]  (A = V page via ldmatrix.trans,
+//                                                             B = P^T via movmatrix of the S^T fragment)
+// No accumulator row is padding (an m16n8k16 tile with heads as M would waste rows 8-15), which
+// halves the MMA count and the accumulator registers.  Online softmax in registers, max over keys
+// by shuffles across the 8 row groups.  HBM-bound: each K/V byte is read once; arithmetic per byte
+// is the same for MHA and GQA.
 // Results: final bf16 row when the request has one split, else fp32 partial (m, l, o) for A5.
 #pragma once
 #include "common.cuh"
@@ -18,9 +26,10 @@ template <int D>
 struct DecodeCfg {
     static constexpr int CB = D / 64;                 // 64-column swizzle blocks per row
     static constexpr int HALF_BYTES = 16 * 128;       // one TMA box: 16 rows x 128 B
-    static constexpr int PAGE_BYTES = CB * HALF_BYTES;  // K (or V) of one page-head
-    static constexpr int STAGE_BYTES = 2 * PAGE_BYTES;  // K + V
+    static constexpr int PAGE_BYTES = CB * HALF_BYTES;  // K (or V) of one page-head = one ring stage
 };
+
+constexpr int kMaxDecodeStages = 32;  // mbarriers reserved per decode warp
 
 struct DecodeArgs {
     PoolDesc pool;
@@ -37,21 +46,40 @@ struct DecodeArgs {
     float* part_o;
 };
 
-// ring: this warp's NSTAGE * STAGE_BYTES bytes (1024-aligned); full: NSTAGE mbarriers (count 1);
-// it: running stage counter of this warp (persists across units so barrier parities stay consistent).
-template <int D, int NSTAGE>
+// Ring state of one decode warp; persists across units so barrier parities stay consistent.
+struct DecodeRing {
+    uint8_t* base;     // nst * PAGE_BYTES bytes, 1024-aligned
+    uint64_t* full;    // nst mbarriers (count 1)
+    int nst;           // stages
+    int c_slot;        // next stage to consume (== next stage to fill when nothing is in flight)
+    uint32_t c_phase;  // parity of c_slot's current use
+    int i_slot;        // next stage to fill
+};
+
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
+    uint32_t d;
+    asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
+    return d;
+}
+
+template <int D>
 __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CUtensorMap* tm_k, const CUtensorMap* tm_v,
-                                                   uint8_t* ring, uint64_t* full, uint32_t& it) {
+                                                   DecodeRing& R) {
     using C = DecodeCfg<D>;
     const int lane = threadIdx.x & 31;
     const int row = lane >> 2, cq = (lane & 3) * 2;
     const int g = A.pool.Hq / A.pool.Hkv;
     const int n_units = A.hdr[HDR_N_UNITS];
-    const uint32_t ring_s = smem_u32(ring);
+    const uint32_t ring_s = smem_u32(R.base);
     // ldmatrix lane addressing (row within 8x8 matrix r8, matrix id mi)
     const int mi = lane >> 3, r8 = lane & 7;
-    const int k_key = (mi >> 1) * 8 + r8, k_chunk_off = mi & 1;   // K: matrices (keys lo/hi) x (chunk, chunk+1)
-    const int v_key = (mi & 1) * 8 + r8, v_chunk_off = mi >> 1;   // V (trans): (keys lo/hi) x (chunk, chunk+1)
+    const int k_key = (mi & 1) * 8 + r8, k_chunk_off = mi >> 1;  // K as A: (keys lo/hi) x (chunk, chunk+1)
+    const int v_key = (mi >> 1) * 8 + r8, v_chunk_off = mi & 1;  // V^T as A (trans): (chunk, chunk+1) x (keys lo/hi)
+    // Swizzled byte offset of this lane's ldmatrix row inside a stage.  Chunk c of row r sits at
+    // r*128 + ((c ^ (r & 7)) << 4); c = 2*i + off with off in {0,1}, so (c ^ x) = (2*i) ^ (off ^ x): the
+    // per-instruction part is an XOR with a compile-time constant on top of one per-lane register.
+    const uint32_t k_lane = k_key * 128 + ((k_chunk_off ^ (k_key & 7)) << 4);
+    const uint32_t v_lane = v_key * 128 + ((v_chunk_off ^ (v_key & 7)) << 4);
 
     for (;;) {
         int u = 0;
@@ -66,83 +94,100 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
         const int nh = min(kHeadBlock, g - hb * kHeadBlock);
         const int* pt = A.b.page_table + (size_t)req * A.b.stride + p0;
 
-        // Q fragments (A operand rows = heads of the group; rows >= nh and rows 8..15 are zero)
-        uint32_t qa[D / 16][2];
+        // Q^T fragments (B operand: column = head of the group; heads >= nh are zero)
+        uint32_t qb[D / 16][2];
         {
             const uint16_t* qrow = A.q + ((size_t)tok * A.pool.Hq + h0 + row) * D;
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
-                qa[ks][0] = row < nh ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + cq) : 0u;
-                qa[ks][1] = row < nh ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + 8 + cq) : 0u;
+                qb[ks][0] = row < nh ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + cq) : 0u;
+                qb[ks][1] = row < nh ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + 8 + cq) : 0u;
             }
         }
-        float o[D / 8][4];
+        // O^T accumulators: o[db][0,1] = d row (db*16 + row) x heads (cq, cq+1); o[db][2,3] = d row + 8
+        float o[D / 16][4];
 #pragma unroll
-        for (int nt = 0; nt < D / 8; ++nt) o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f;
-        float m = -INFINITY, l = 0.f;
+        for (int db = 0; db < D / 16; ++db) o[db][0] = o[db][1] = o[db][2] = o[db][3] = 0.f;
+        float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;  // heads cq, cq+1 (l: this lane's keys only)
 
-        int ptv = 0;
-        uint32_t it_issue = it;
-        auto issue = [&](int pi) {  // whole warp calls; lane 0 issues the TMA boxes of page pi of this unit
-            if ((pi & 31) == 0) ptv = (pi + lane < np) ? __ldg(pt + pi + lane) : 0;
+        // ---- stage issue: sub-stage j = K (j even) or V (j odd) of page j >> 1
+        const int n_sub = 2 * np;
+        int issued = 0, ptv = 0;
+        auto issue_one = [&]() {  // whole warp calls; lane 0 issues the boxes of sub-stage `issued`
+            const int pi = issued >> 1;
+            if ((issued & 63) == 0) ptv = (pi + lane < np) ? __ldg(pt + pi + lane) : 0;
             const int page = __shfl_sync(0xffffffffu, ptv, pi & 31);
             if (lane == 0) {
-                const int st = it_issue % NSTAGE;
-                uint8_t* dst = ring + st * C::STAGE_BYTES;
+                uint8_t* dst = R.base + R.i_slot * C::PAGE_BYTES;
+                uint64_t* bar = R.full + R.i_slot;
                 const int r0 = (page * A.pool.Hkv + kvh) * kPageSize;
-                mbar_arrive_expect_tx(full + st, C::STAGE_BYTES);
+                const CUtensorMap* tm = (issued & 1) ? tm_v : tm_k;
+                mbar_arrive_expect_tx(bar, C::PAGE_BYTES);
 #pragma unroll
-                for (int cb = 0; cb < C::CB; ++cb) {
-                    tma_load_2d(dst + cb * C::HALF_BYTES, tm_k, cb * 64, r0, full + st);
-                    tma_load_2d(dst + C::PAGE_BYTES + cb * C::HALF_BYTES, tm_v, cb * 64, r0, full + st);
-                }
+                for (int cb = 0; cb < C::CB; ++cb) tma_load_2d(dst + cb * C::HALF_BYTES, tm, cb * 64, r0, bar);
             }
-            ++it_issue;
+            R.i_slot = (R.i_slot + 1 == R.nst) ? 0 : R.i_slot + 1;
+            ++issued;
         };
-        const int pre = min(NSTAGE - 1, np);
-        for (int i = 0; i < pre; ++i) issue(i);
+        auto consume_advance = [&]() {
+            if (++R.c_slot == R.nst) { R.c_slot = 0; R.c_phase ^= 1; }
+        };
+        {
+            const int pre = min(R.nst, n_sub);
+            for (int i = 0; i < pre; ++i) issue_one();
+        }
 
         for (int p = 0; p < np; ++p) {
-            if (p + NSTAGE - 1 < np) issue(p + NSTAGE - 1);
-            const int st = it % NSTAGE;
-            mbar_wait(full + st, (it / NSTAGE) & 1);
-            ++it;
-            const uint32_t kbase = ring_s + st * C::STAGE_BYTES;
-            const uint32_t vbase = kbase + C::PAGE_BYTES;
-
-            // S = Q K^T for the 16 keys of this page (two n-tiles of 8 keys)
-            float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+            // ---------------- S^T = K Q^T for the 16 keys of this page
+            mbar_wait(R.full + R.c_slot, R.c_phase, 201);
+            const uint32_t kbase = ring_s + R.c_slot * C::PAGE_BYTES;
+            float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
-                const int chunk = (ks & 3) * 2 + k_chunk_off;
-                const uint32_t addr = kbase + (ks >> 2) * C::HALF_BYTES + k_key * 128 + ((chunk ^ (k_key & 7)) << 4);
-                uint32_t b00, b01, b10, b11;
-                ldmatrix_x4(addr, b00, b01, b10, b11);
-                mma_bf16_16816(s0, qa[ks][0], 0u, qa[ks][1], 0u, b00, b01);
-                mma_bf16_16816(s1, qa[ks][0], 0u, qa[ks][1], 0u, b10, b11);
+                const uint32_t addr = ((kbase + k_lane) ^ (uint32_t)((ks & 3) * 32)) + (ks >> 2) * C::HALF_BYTES;
+                uint32_t a0, a1, a2, a3;
+                ldmatrix_x4(addr, a0, a1, a2, a3);
+                if (ks & 1) mma_bf16_16816(sb, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
+                else mma_bf16_16816(sa, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
             }
-            const int nvalid = L - (p0 + p) * kPageSize;  // >= 1 by construction of the unit
-            float v00 = (cq < nvalid) ? s0[0] * A.scale_log2 : -INFINITY;
-            float v01 = (cq + 1 < nvalid) ? s0[1] * A.scale_log2 : -INFINITY;
-            float v10 = (cq + 8 < nvalid) ? s1[0] * A.scale_log2 : -INFINITY;
-            float v11 = (cq + 9 < nvalid) ? s1[1] * A.scale_log2 : -INFINITY;
-            float mx = fmaxf(fmaxf(v00, v01), fmaxf(v10, v11));
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
-            const float m_new = fmaxf(m, mx);  // finite: key 0 of the page is valid
-            const float alpha = fast_exp2(m - m_new);
-            v00 = fast_exp2(v00 - m_new);
-            v01 = fast_exp2(v01 - m_new);
-            v10 = fast_exp2(v10 - m_new);
-            v11 = fast_exp2(v11 - m_new);
-            l = l * alpha + ((v00 + v01) + (v10 + v11));
-            if (__any_sync(0xffffffffu, m_new > m)) {
-#pragma unroll
-                for (int nt = 0; nt < D / 8; ++nt) { o[nt][0] *= alpha; o[nt][1] *= alpha; }
-            }
-            m = m_new;
-            const uint32_t pa0 = pack_bf16x2(v00, v01), pa2 = pack_bf16x2(v10, v11);
+            __syncwarp();  // every lane has read the K stage
+            consume_advance();
+            if (issued < n_sub) issue_one();
 
+            const int nvalid = L - (p0 + p) * kPageSize;  // >= 1 by construction of the unit
+            // sa/sb[0,1]: key `row`, heads cq, cq+1;  [2,3]: key row + 8
+            const bool klo = row < nvalid, khi = row + 8 < nvalid;
+            float v00 = klo ? (sa[0] + sb[0]) * A.scale_log2 : -INFINITY;
+            float v01 = klo ? (sa[1] + sb[1]) * A.scale_log2 : -INFINITY;
+            float v10 = khi ? (sa[2] + sb[2]) * A.scale_log2 : -INFINITY;
+            float v11 = khi ? (sa[3] + sb[3]) * A.scale_log2 : -INFINITY;
+            float mx0 = fmaxf(v00, v10), mx1 = fmaxf(v01, v11);
+#pragma unroll
+            for (int off = 4; off < 32; off <<= 1) {
+                mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, off));
+                mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, off));
+            }
+            const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);  // finite: key 0 of the page is valid
+            const float al0 = fast_exp2(m0 - mn0), al1 = fast_exp2(m1 - mn1);
+            v00 = fast_exp2(v00 - mn0);
+            v10 = fast_exp2(v10 - mn0);
+            v01 = fast_exp2(v01 - mn1);
+            v11 = fast_exp2(v11 - mn1);
+            l0 = l0 * al0 + (v00 + v10);
+            l1 = l1 * al1 + (v01 + v11);
+            if (__any_sync(0xffffffffu, (mn0 > m0) | (mn1 > m1))) {
+#pragma unroll
+                for (int db = 0; db < D / 16; ++db) { o[db][0] *= al0; o[db][1] *= al1; o[db][2] *= al0; o[db][3] *= al1; }
+            }
+            m0 = mn0;
+            m1 = mn1;
+            // P^T as B operand: transpose the two 8x8 (key x head) bf16 blocks of the S^T fragment
+            const uint32_t pb0 = movmatrix_trans(pack_bf16x2(v00, v01));
+            const uint32_t pb1 = movmatrix_trans(pack_bf16x2(v10, v11));
+
+            // ---------------- O^T += V^T P^T
+            mbar_wait(R.full + R.c_slot, R.c_phase, 202);
+            const uint32_t vbase = ring_s + R.c_slot * C::PAGE_BYTES;
             if (nvalid < kPageSize) {  // ragged last page: unused slots may hold NaN bits; 0 * NaN = NaN in the MMA
                 const int nz = (kPageSize - nvalid) * 8 * C::CB;
                 for (int idx = lane; idx < nz; idx += 32) {
@@ -152,37 +197,62 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
                 }
                 __syncwarp();
             }
-            // O += P V
 #pragma unroll
-            for (int n2 = 0; n2 < D / 16; ++n2) {
-                const int chunk = ((n2 * 2) & 7) + v_chunk_off;
-                const uint32_t addr = vbase + ((n2 * 2) >> 3) * C::HALF_BYTES + v_key * 128 + ((chunk ^ (v_key & 7)) << 4);
-                uint32_t b0, b1, b2, b3;
-                ldmatrix_x4_trans(addr, b0, b1, b2, b3);
-                mma_bf16_16816(o[2 * n2], pa0, 0u, pa2, 0u, b0, b1);
-                mma_bf16_16816(o[2 * n2 + 1], pa0, 0u, pa2, 0u, b2, b3);
+            for (int db = 0; db < D / 16; ++db) {
+                const uint32_t addr = ((vbase + v_lane) ^ (uint32_t)((db & 3) * 32)) + (db >> 2) * C::HALF_BYTES;
+                uint32_t a0, a1, a2, a3;
+                ldmatrix_x4_trans(addr, a0, a1, a2, a3);
+                mma_bf16_16816(o[db], a0, a1, a2, a3, pb0, pb1);
             }
             if (nvalid < kPageSize) fence_proxy_async();  // generic zero-fill before the next TMA refill
-            __syncwarp();  // every lane is done with this stage before lane 0 refills it
+            __syncwarp();  // every lane is done with the V stage
+            consume_advance();
+            if (issued < n_sub) issue_one();
         }
 
-        l += __shfl_xor_sync(0xffffffffu, l, 1);
-        l += __shfl_xor_sync(0xffffffffu, l, 2);
+#pragma unroll
+        for (int off = 4; off < 32; off <<= 1) {
+            l0 += __shfl_xor_sync(0xffffffffu, l0, off);
+            l1 += __shfl_xor_sync(0xffffffffu, l1, off);
+        }
         const int nsplit = A.req_info[req].z;
-        if (row < nh) {
-            if (nsplit == 1) {
-                const float inv = 1.f / l;
-                uint16_t* orow = A.out + ((size_t)tok * A.pool.Hq + h0 + row) * D + cq;
+        // this lane owns heads cq, cq+1 and d rows {db*16 + row, db*16 + row + 8}
+        if (nsplit == 1) {
+            const float i0 = 1.f / l0, i1 = 1.f / l1;
+            __nv_bfloat16* ob = reinterpret_cast<__nv_bfloat16*>(A.out) + ((size_t)tok * A.pool.Hq + h0) * D;
 #pragma unroll
-                for (int nt = 0; nt < D / 8; ++nt)
-                    *reinterpret_cast<uint32_t*>(orow + nt * 8) = pack_bf16x2(o[nt][0] * inv, o[nt][1] * inv);
-                if (A.lse != nullptr && cq == 0)
-                    A.lse[(size_t)tok * A.pool.Hq + h0 + row] = (m + log2f(l)) * 0.6931471805599453f;
-            } else {
-                float* prow = A.part_o + ((size_t)u * kHeadBlock + row) * D + cq;
+            for (int db = 0; db < D / 16; ++db) {
+                const int d0 = db * 16 + row;
+                if (cq < nh) {
+                    ob[(size_t)cq * D + d0] = __float2bfloat16_rn(o[db][0] * i0);
+                    ob[(size_t)cq * D + d0 + 8] = __float2bfloat16_rn(o[db][2] * i0);
+                }
+                if (cq + 1 < nh) {
+                    ob[(size_t)(cq + 1) * D + d0] = __float2bfloat16_rn(o[db][1] * i1);
+                    ob[(size_t)(cq + 1) * D + d0 + 8] = __float2bfloat16_rn(o[db][3] * i1);
+                }
+            }
+            if (A.lse != nullptr && row == 0) {
+                if (cq < nh) A.lse[(size_t)tok * A.pool.Hq + h0 + cq] = (m0 + log2f(l0)) * 0.6931471805599453f;
+                if (cq + 1 < nh) A.lse[(size_t)tok * A.pool.Hq + h0 + cq + 1] = (m1 + log2f(l1)) * 0.6931471805599453f;
+            }
+        } else {
+            float* pb = A.part_o + (size_t)u * kHeadBlock * D;
 #pragma unroll
-                for (int nt = 0; nt < D / 8; ++nt) *reinterpret_cast<float2*>(prow + nt * 8) = make_float2(o[nt][0], o[nt][1]);
-                if (cq == 0) A.part_ml[(size_t)u * kHeadBlock + row] = make_float2(m, l);
+            for (int db = 0; db < D / 16; ++db) {
+                const int d0 = db * 16 + row;
+                if (cq < nh) {
+                    pb[cq * D + d0] = o[db][0];
+                    pb[cq * D + d0 + 8] = o[db][2];
+                }
+                if (cq + 1 < nh) {
+                    pb[(cq + 1) * D + d0] = o[db][1];
+                    pb[(cq + 1) * D + d0 + 8] = o[db][3];
+                }
+            }
+            if (row == 0) {
+                if (cq < nh) A.part_ml[(size_t)u * kHeadBlock + cq] = make_float2(m0, l0);
+                if (cq + 1 < nh) A.part_ml[(size_t)u * kHeadBlock + cq + 1] = make_float2(m1, l1);
             }
         }
     }

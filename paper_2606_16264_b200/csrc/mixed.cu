@@ -12,7 +12,29 @@
 namespace tropical {
 
 constexpr int kDecodeWarps = 4;
-constexpr int kDecodeStages = 3;
+constexpr int kDecodeRingBytes = 24576;  // per decode warp: 6 page-head stages at d = 128
+
+__device__ __forceinline__ DecodeRing make_ring(uint8_t* base, uint64_t* bars, int nst) {
+    DecodeRing R;
+    R.base = base;
+    R.full = bars;
+    R.nst = nst;
+    R.c_slot = 0;
+    R.c_phase = 0;
+    R.i_slot = 0;
+    return R;
+}
+
+// role finish times (globaltimer ns) for the A/B evidence under profiles/: hdr[HDR_PROF ...] as u64
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void prof_mark(const int* hdr, int which, bool is_min) {
+    unsigned long long* p = reinterpret_cast<unsigned long long*>(const_cast<int*>(hdr) + HDR_PROF) + which;
+    if (is_min) atomicMin(p, global_ns()); else atomicMax(p, global_ns());
+}
 
 template <int D>
 __global__ void __launch_bounds__(kDecodeWarps * 32, 2)
@@ -20,19 +42,19 @@ decode_kernel(DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __gr
     using C = DecodeCfg<D>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kDecodeWarps * kDecodeStages * C::STAGE_BYTES);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kDecodeWarps * kDecodeRingBytes);
+    constexpr int NST = kDecodeRingBytes / C::PAGE_BYTES;
+    static_assert(NST <= kMaxDecodeStages, "stage barriers");
+    const int warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tm_k);
         tma_prefetch_desc(&tm_v);
-        for (int i = 0; i < kDecodeWarps * kDecodeStages; ++i) mbar_init(bars + i, 1);
+        for (int i = 0; i < kDecodeWarps * NST; ++i) mbar_init(bars + i, 1);
         fence_mbar_init();
     }
     __syncthreads();
-    uint32_t it = 0;
-    decode_warp_worker<D, kDecodeStages>(A, &tm_k, &tm_v, smem + warp * kDecodeStages * C::STAGE_BYTES,
-                                         bars + warp * kDecodeStages, it);
-    (void)lane;
+    DecodeRing R = make_ring(smem + warp * kDecodeRingBytes, bars + warp * NST, NST);
+    decode_warp_worker<D>(A, &tm_k, &tm_v, R);
 }
 
 
@@ -70,26 +92,31 @@ prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __
 }
 
 // ------------------------------------------------------------------------------------------------
-// The fused step kernel: ONE persistent launch, one CTA per SM, three warpgroups.
-//   WG0 (warps 0-3)  : prefill softmax / correction / epilogue    (registers grown with setmaxnreg)
-//   WG1 (warps 4-7)  : decode workers, one private TMA ring each  (HBM streaming)
-//   WG2 (warps 8-11) : warp 8 prefill TMA producer, warp 9 tcgen05 MMA issuer, 10-11 spare (registers shrunk)
+// The fused step kernel: ONE persistent launch, one CTA per SM, four warpgroups (512 threads, the whole
+// register file re-divided between the roles with setmaxnreg).
+//   WG0 (warps 0-3)   : prefill softmax / correction / epilogue (224 regs); when the prefill queue is empty
+//                       these warps become decode workers too, with rings carved out of the (now idle)
+//                       prefill tile memory
+//   WG1 (warps 4-7)   : decode workers, one private TMA ring each (HBM streaming, 120 regs)
+//   WG2 (warps 8-11)  : warp 8 prefill TMA producer, warp 9 tcgen05 MMA issuer, 10-11 idle (48 regs)
+//   WG3 (warps 12-15) : decode workers (120 regs)
 // Prefill items and decode units are popped from two ticket counters, so on every SM the tensor
 // pipe (prefill) and the HBM stream (decode) are busy at the same time for the whole step.
-constexpr int kMixedThreads = 384;
+constexpr int kMixedThreads = 512;
 
 template <int D>
 struct MixedCfg {
-    static constexpr int DEC_WARPS = 4;
-    static constexpr int DEC_RING = 16384;  // bytes of TMA ring per decode warp
-    static constexpr int DEC_STAGES = DEC_RING / DecodeCfg<D>::STAGE_BYTES;
-    static constexpr int BAR_BYTES = 1024;
+    static constexpr int DEC_WARPS = 8;
+    static constexpr int DEC_RING = 12288;                                  // bytes of TMA ring per dedicated decode warp
+    static constexpr int DEC_STAGES = DEC_RING / DecodeCfg<D>::PAGE_BYTES;
+    static constexpr int LATE_RING = PrefillCfg<D>::SMEM_TILES / 4;         // WG0 after the prefill queue is empty
+    static constexpr int LATE_STAGES = LATE_RING / DecodeCfg<D>::PAGE_BYTES;
+    static constexpr int N_DEC_BARS = DEC_WARPS * DEC_STAGES + 4 * LATE_STAGES;
+    static constexpr int BAR_BYTES = 2048;
     static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_WARPS * DEC_RING + BAR_BYTES + 1024;
-};
-
-struct MixedBars {
-    PrefillBars p;
-    uint64_t dec_full[32];
+    static_assert(DEC_STAGES <= kMaxDecodeStages && LATE_STAGES <= kMaxDecodeStages, "stage barriers");
+    static_assert(LATE_RING % 1024 == 0 && DEC_RING % 1024 == 0, "ring alignment");
+    static_assert(sizeof(PrefillBars) + N_DEC_BARS * 8 <= BAR_BYTES, "barrier block");
 };
 
 template <int D>
@@ -98,43 +125,52 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
              const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
     using C = PrefillCfg<D>;
     using M = MixedCfg<D>;
-    static_assert(sizeof(MixedBars) <= M::BAR_BYTES, "barrier block");
     extern __shared__ uint8_t smem_raw[];
     uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* rings = tiles + C::SMEM_TILES;
-    MixedBars* B = reinterpret_cast<MixedBars*>(rings + M::DEC_WARPS * M::DEC_RING);
+    PrefillBars* PB = reinterpret_cast<PrefillBars*>(rings + M::DEC_WARPS * M::DEC_RING);
+    uint64_t* dec_full = reinterpret_cast<uint64_t*>(PB + 1);
     const int warp = threadIdx.x >> 5, wg = warp >> 2;
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
         tma_prefetch_desc(&tm_v);
-        prefill_init_bars(&B->p);
-        for (int i = 0; i < M::DEC_WARPS * M::DEC_STAGES; ++i) mbar_init(&B->dec_full[i], 1);
+        prefill_init_bars(PB);
+        for (int i = 0; i < M::N_DEC_BARS; ++i) mbar_init(dec_full + i, 1);
         fence_mbar_init();
+        prof_mark(PA.hdr, 0, true);
     }
     if (warp == 0) {
-        tmem_alloc(&B->p.tmem_base, C::TM_COLS);
+        tmem_alloc(&PB->tmem_base, C::TM_COLS);
         tmem_relinquish();
     }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     if (wg == 0) {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
-        prefill_softmax<D>(PA, &B->p, warp);
-    } else if (wg == 1) {
-        const int dw = warp - 4;
-        uint32_t it = 0;
-        decode_warp_worker<D, M::DEC_STAGES>(DA, &tm_k, &tm_v, rings + dw * M::DEC_RING,
-                                             &B->dec_full[dw * M::DEC_STAGES], it);
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+        prefill_softmax<D>(PA, PB, warp);
+        // The terminating ticket was seen after the last item's final PV completed: every TMA load into the
+        // tile memory has been consumed, and the producer issues nothing more.  Reuse it for decode rings.
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 1, false);
+        DecodeRing R = make_ring(tiles + warp * M::LATE_RING, dec_full + M::DEC_WARPS * M::DEC_STAGES + warp * M::LATE_STAGES,
+                                 M::LATE_STAGES);
+        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
+    } else if (wg == 2) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
+        if (warp == 8) prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k, &tm_v);
+        else if (warp == 9) prefill_mma<D>(PA, PB, tiles);
     } else {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
-        if (warp == 8) prefill_producer<D>(PA, &B->p, tiles, &tm_q, &tm_k, &tm_v);
-        else if (warp == 9) prefill_mma<D>(PA, &B->p, tiles);
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 120;");
+        const int dw = (wg == 1) ? warp - 4 : warp - 8;
+        DecodeRing R = make_ring(rings + dw * M::DEC_RING, dec_full + dw * M::DEC_STAGES, M::DEC_STAGES);
+        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) tmem_dealloc(B->p.tmem_base, C::TM_COLS);
+    if (warp == 0) tmem_dealloc(PB->tmem_base, C::TM_COLS);
 }
 
 template <int D>
@@ -159,6 +195,8 @@ static int num_sms() {
 size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q) {
     return make_layout(Hq, Hkv, D, num_reqs, total_q).total;
 }
+
+size_t profile_offset_bytes() { return make_layout(1, 1, 64, 1, 1).hdr + HDR_PROF * sizeof(int); }
 
 static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches (A/B timing only)
 void set_debug_mode(int mode) { g_mode = mode; }
@@ -239,7 +277,7 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
             ++*launches;
         }
         // A4: decode tiles
-        const size_t smem = (size_t)kDecodeWarps * kDecodeStages * DecodeCfg<D>::STAGE_BYTES + 1024 + 256;
+        const size_t smem = (size_t)kDecodeWarps * kDecodeRingBytes + 1024 + 1024;
         static bool attr_done = false;
         if (!attr_done) {
             e = cudaFuncSetAttribute(decode_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

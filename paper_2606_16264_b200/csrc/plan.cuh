@@ -14,7 +14,8 @@ constexpr int kTargetUnits = 9472;   // ~8 decode units per resident decode warp
 constexpr int kMinSplitPages = 8;    // never split finer than 128 tokens
 
 enum { HDR_N_ITEMS = 0, HDR_N_UNITS = 1, HDR_SPLIT_PAGES = 2, HDR_TICKET_PREFILL = 3, HDR_TICKET_DECODE = 4,
-       HDR_N_COMBINE = 5, HDR_INTS = 64 };
+       HDR_N_COMBINE = 5, HDR_PROF = 16 /* 4 x u64: kernel start (min), prefill end, WG1 decode end, WG0 decode end (max) */,
+       HDR_INTS = 64 };
 
 // req_info[i] = {kind, unit_base, nsplit, item_base}; kind 0 skip, 1 decode, 2 prefill
 struct WorkspaceLayout {
@@ -127,6 +128,9 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         P.hdr[HDR_SPLIT_PAGES] = split;
         P.hdr[HDR_TICKET_PREFILL] = 0;
         P.hdr[HDR_TICKET_DECODE] = 0;
+        unsigned long long* prof = reinterpret_cast<unsigned long long*>(P.hdr + HDR_PROF);
+        prof[0] = ~0ull;
+        prof[1] = prof[2] = prof[3] = 0ull;
     }
     __syncthreads();  // req_info visible to the whole block (same-block global writes + barrier)
 

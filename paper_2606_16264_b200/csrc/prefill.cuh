@@ -14,8 +14,9 @@
 // handed to the other roles through a 2-deep shared-memory mailbox):
 //   producer warp : TMA. Q tile (3-D map, 2 boxes) and, per KV tile, the 8 page-heads of K and of V
 //                   (2-D map, one 64-col x 16-row SW128 box per page-head half, issued by 16 lanes in
-//                   parallel) into 2-stage K and V rings.  The HND pool makes every box one
-//                   contiguous 2 KiB run of HBM/L2.
+//                   parallel) into ONE 3-slot ring filled in the order the MMA warp consumes tiles
+//                   (K0, K1, V0, K2, V1, ...).  The HND pool makes every box one contiguous 2 KiB
+//                   run of HBM/L2.
 //   MMA warp      : one elected lane issues S(kt+1) ahead of PV(kt) so the tensor pipe works on
 //                   the next scores while the softmax warps work on the current ones.
 //   softmax warps : 4 warps, thread r owns query row r (TMEM lane r): no shuffles.
@@ -36,8 +37,8 @@ struct PrefillCfg {
     static constexpr int HALF_BYTES = kKvTile * 128;     // one half of a 128-row tile: 16 KiB
     static constexpr int TILE_BYTES = CB * HALF_BYTES;   // Q tile / K tile / V tile
     static constexpr int PAGE_BOX = kPageSize * 128;     // one TMA box: 16 rows x 128 B
-    static constexpr int KV_STAGES = 2;
-    static constexpr int SMEM_TILES = TILE_BYTES * (1 + 2 * KV_STAGES);
+    static constexpr int KV_SLOTS = 3;                   // one ring for K and V tiles, filled in consumption order
+    static constexpr int SMEM_TILES = TILE_BYTES * (1 + KV_SLOTS);
     // TMEM columns: S slot 0 at 0, S slot 1 at 128, O at 256
     static constexpr uint32_t TM_S = 0, TM_O = 256, TM_COLS = 512;
 };
@@ -46,7 +47,7 @@ struct PrefillCfg {
 struct PrefillBars {
     uint64_t item_full[2], item_empty[2];
     uint64_t q_full, q_empty;
-    uint64_t k_full[2], k_empty[2], v_full[2], v_empty[2];
+    uint64_t kv_full[3], kv_empty[3];
     uint64_t s_full[2], p_full[2];
     uint64_t pv_done, o_empty;
     int mailbox[2];
@@ -90,12 +91,12 @@ __device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
     for (int i = 0; i < 2; ++i) {
         mbar_init(&B->item_full[i], 1);
         mbar_init(&B->item_empty[i], 5);  // MMA lane 0 + lane 0 of each softmax warp
-        mbar_init(&B->k_full[i], 1);
-        mbar_init(&B->k_empty[i], 1);
-        mbar_init(&B->v_full[i], 1);
-        mbar_init(&B->v_empty[i], 1);
         mbar_init(&B->s_full[i], 1);
         mbar_init(&B->p_full[i], 128);
+    }
+    for (int i = 0; i < 3; ++i) {
+        mbar_init(&B->kv_full[i], 1);
+        mbar_init(&B->kv_empty[i], 1);
     }
     mbar_init(&B->q_full, 1);
     mbar_init(&B->q_empty, 1);
@@ -113,12 +114,13 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
     const int lane = threadIdx.x & 31;
     const int n_items = A.hdr[HDR_N_ITEMS];
     uint8_t* q_s = tiles;
-    uint8_t* k_s = tiles + C::TILE_BYTES;
-    uint8_t* v_s = tiles + C::TILE_BYTES * (1 + C::KV_STAGES);
-    uint32_t item_it = 0, kv_it = 0;
+    uint8_t* ring = tiles + C::TILE_BYTES;
+    uint32_t item_it = 0;
+    int slot = 0;
+    uint32_t phase = 0;  // parity of the current use of `slot`
     for (;;) {
         const int ms = item_it & 1;
-        mbar_wait(&B->item_empty[ms], ((item_it >> 1) & 1) ^ 1);
+        mbar_wait(&B->item_empty[ms], ((item_it >> 1) & 1) ^ 1, 101, item_it);
         int id = 0;
         if (lane == 0) {
             id = atomicAdd(A.ticket, 1);
@@ -130,7 +132,7 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
         const PrefillItem it = load_item(A, id);
         const int* pt = A.b.page_table + (size_t)it.req * A.b.stride;
 
-        mbar_wait(&B->q_empty, (item_it & 1) ^ 1);
+        mbar_wait(&B->q_empty, (item_it & 1) ^ 1, 102, item_it);
         if (lane == 0) {
             mbar_arrive_expect_tx(&B->q_full, C::TILE_BYTES);
 #pragma unroll
@@ -138,26 +140,24 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
                 tma_load_3d(q_s + cb * C::HALF_BYTES, tm_q, cb * 64, it.h, it.tok0 + it.qt * kQTile, &B->q_full);
         }
         const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
-        for (int kt = 0; kt < it.n_kt; ++kt, ++kv_it) {
-            const int st = kv_it & 1;
-            const uint32_t par = ((kv_it >> 1) & 1) ^ 1;
+        // tiles in the order the MMA warp consumes them: K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)
+        auto load_tile = [&](int kt, const CUtensorMap* tm) {
             const int np = min(8, n_pages - kt * 8);
-            // lane -> (page p, half cb) of this tile
-            const int p = lane / C::CB, cb = lane % C::CB;
+            const int p = lane / C::CB, cb = lane % C::CB;  // lane -> (page p, half cb) of this tile
             const bool act = p < np && lane < 8 * C::CB;
             const int page = act ? __ldg(pt + kt * 8 + p) : 0;
             const int r0 = (page * A.pool.Hkv + it.hk) * kPageSize;
             const uint32_t off = cb * C::HALF_BYTES + p * C::PAGE_BOX;
-
-            mbar_wait(&B->k_empty[st], par);
-            if (lane == 0) mbar_arrive_expect_tx(&B->k_full[st], np * C::CB * C::PAGE_BOX);
+            mbar_wait(&B->kv_empty[slot], phase ^ 1, 103, item_it * 100000 + kt * 1000 + slot * 100 + it.n_kt);
+            if (lane == 0) mbar_arrive_expect_tx(&B->kv_full[slot], np * C::CB * C::PAGE_BOX);
             __syncwarp();
-            if (act) tma_load_2d(k_s + st * C::TILE_BYTES + off, tm_k, cb * 64, r0, &B->k_full[st]);
-
-            mbar_wait(&B->v_empty[st], par);
-            if (lane == 0) mbar_arrive_expect_tx(&B->v_full[st], np * C::CB * C::PAGE_BOX);
-            __syncwarp();
-            if (act) tma_load_2d(v_s + st * C::TILE_BYTES + off, tm_v, cb * 64, r0, &B->v_full[st]);
+            if (act) tma_load_2d(ring + slot * C::TILE_BYTES + off, tm, cb * 64, r0, &B->kv_full[slot]);
+            if (++slot == C::KV_SLOTS) { slot = 0; phase ^= 1; }
+        };
+        load_tile(0, tm_k);
+        for (int kt = 0; kt < it.n_kt; ++kt) {
+            if (kt + 1 < it.n_kt) load_tile(kt + 1, tm_k);
+            load_tile(kt, tm_v);
         }
         ++item_it;
     }
@@ -171,42 +171,48 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
     const int lane = threadIdx.x & 31;
     const int n_items = A.hdr[HDR_N_ITEMS];
     const uint32_t q_a = smem_u32(tiles);
-    const uint32_t k_a = q_a + C::TILE_BYTES;
-    const uint32_t v_a = q_a + C::TILE_BYTES * (1 + C::KV_STAGES);
+    const uint32_t ring_a = q_a + C::TILE_BYTES;
     const uint32_t tm = B->tmem_base;
     constexpr uint32_t IDESC_S = make_idesc_bf16(128, 128, false);
     constexpr uint32_t IDESC_O = make_idesc_bf16(128, D, true);
     uint32_t item_it = 0, kv_it = 0;
+    int slot = 0;
+    uint32_t phase = 0;
+    auto advance = [&]() {
+        if (++slot == C::KV_SLOTS) { slot = 0; phase ^= 1; }
+    };
 
-    auto issue_s = [&](uint32_t g) {  // S(g) = Q K^T into S slot g & 1
+    auto issue_s = [&](uint32_t g) {  // S(g) = Q K^T into S slot g & 1; consumes the next ring tile (a K tile)
         const int st = g & 1;
-        mbar_wait(&B->k_full[st], (g >> 1) & 1);
+        mbar_wait(&B->kv_full[slot], phase, 104, item_it * 100000 + g * 100 + slot);
         tc_fence_after();
         if (lane == 0) {
+            const uint32_t k_a = ring_a + slot * C::TILE_BYTES;
 #pragma unroll
             for (int cb = 0; cb < C::CB; ++cb)
 #pragma unroll
                 for (int k4 = 0; k4 < 4; ++k4) {
                     const uint32_t o = cb * C::HALF_BYTES + k4 * 32;
                     tc_mma_ss(tm + C::TM_S + st * 128, make_smem_desc_sw128(q_a + o, 0, 1024),
-                              make_smem_desc_sw128(k_a + st * C::TILE_BYTES + o, 0, 1024), IDESC_S, (cb | k4) != 0);
+                              make_smem_desc_sw128(k_a + o, 0, 1024), IDESC_S, (cb | k4) != 0);
                 }
             tc_commit(&B->s_full[st]);
-            tc_commit(&B->k_empty[st]);
+            tc_commit(&B->kv_empty[slot]);
         }
         __syncwarp();
+        advance();
     };
 
     for (;;) {
         const int ms = item_it & 1;
-        mbar_wait(&B->item_full[ms], (item_it >> 1) & 1);
+        mbar_wait(&B->item_full[ms], (item_it >> 1) & 1, 105, item_it);
         const int id = B->mailbox[ms];
         __syncwarp();
         if (lane == 0) mbar_arrive(&B->item_empty[ms]);
         if (id >= n_items) break;
         const PrefillItem it = load_item(A, id);
 
-        mbar_wait(&B->q_full, item_it & 1);
+        mbar_wait(&B->q_full, item_it & 1, 106, item_it);
         issue_s(kv_it);
         for (int kt = 0; kt < it.n_kt; ++kt) {
             const uint32_t g = kv_it + kt;
@@ -217,31 +223,32 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
                 if (lane == 0) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
                 __syncwarp();
             }
-            mbar_wait(&B->v_full[st], (g >> 1) & 1);
+            mbar_wait(&B->kv_full[slot], phase, 107, item_it * 100000 + kt * 1000 + slot * 100 + it.n_kt);  // the next ring tile is V(kt)
+            const uint32_t v_a = ring_a + slot * C::TILE_BYTES;
             if (kt + 1 == it.n_kt) {  // zero V rows past the last visible key (stale or poisoned smem)
                 const int nvalid = it.l_tile - kt * kKvTile;
                 const int nz = (kKvTile - nvalid) * 8 * C::CB;
                 for (int idx = lane; idx < nz; idx += 32) {
                     const int r = nvalid + idx / (8 * C::CB), rem = idx % (8 * C::CB);
-                    const uint32_t a = v_a + st * C::TILE_BYTES + (rem >> 3) * C::HALF_BYTES + r * 128 + ((rem & 7) << 4);
+                    const uint32_t a = v_a + (rem >> 3) * C::HALF_BYTES + r * 128 + ((rem & 7) << 4);
                     asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
                 }
                 fence_proxy_async();
                 __syncwarp();
             }
-            if (kt == 0) mbar_wait(&B->o_empty, (item_it & 1) ^ 1);  // previous item's epilogue has read O
-            mbar_wait(&B->p_full[st], (g >> 1) & 1);
+            if (kt == 0) mbar_wait(&B->o_empty, (item_it & 1) ^ 1, 108, item_it * 100000 + id);  // previous item's epilogue has read O
+            mbar_wait(&B->p_full[st], (g >> 1) & 1, 109, item_it * 100000 + kt * 1000 + it.n_kt);
             tc_fence_after();
             if (lane == 0) {
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks)  // 16 keys per MMA
                     tc_mma_ts(tm + C::TM_O, tm + C::TM_S + st * 128 + ks * 8,
-                              make_smem_desc_sw128(v_a + st * C::TILE_BYTES + ks * 2048, C::HALF_BYTES, 1024), IDESC_O,
-                              (kt | ks) != 0);
-                tc_commit(&B->v_empty[st]);
+                              make_smem_desc_sw128(v_a + ks * 2048, C::HALF_BYTES, 1024), IDESC_O, (kt | ks) != 0);
+                tc_commit(&B->kv_empty[slot]);
                 tc_commit(&B->pv_done);
             }
             __syncwarp();
+            advance();
         }
         kv_it += it.n_kt;
         ++item_it;
@@ -264,7 +271,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
 
     for (;;) {
         const int ms = item_it & 1;
-        mbar_wait(&B->item_full[ms], (item_it >> 1) & 1);
+        mbar_wait(&B->item_full[ms], (item_it >> 1) & 1, 110, item_it);
         const int id = B->mailbox[ms];
         __syncwarp();
         if (lane == 0) mbar_arrive(&B->item_empty[ms]);
@@ -277,7 +284,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
         for (int kt = 0; kt < it.n_kt; ++kt) {
             const uint32_t g = kv_it + kt;
             const int st = g & 1;
-            mbar_wait(&B->s_full[st], (g >> 1) & 1);
+            mbar_wait(&B->s_full[st], (g >> 1) & 1, 111, item_it * 100000 + kt * 1000 + it.n_kt);
             tc_fence_after();
             uint32_t s[128];
 #pragma unroll
@@ -301,7 +308,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
                 const bool grow = m_new > m_used + 8.f;  // lazy rescale: P stays <= 2^8
                 if (__any_sync(0xffffffffu, grow)) {
                     const float alpha = grow ? fast_exp2(m_used - m_new) : 1.f;
-                    mbar_wait(&B->pv_done, (g - 1) & 1);  // O holds PV(g-1)
+                    mbar_wait(&B->pv_done, (g - 1) & 1, 112, item_it * 100000 + kt * 1000 + it.n_kt);  // O holds PV(g-1)
                     tc_fence_after();
 #pragma unroll
                     for (int c4 = 0; c4 < D / 32; ++c4) {
@@ -331,12 +338,17 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
             tmem_st_32x32(tm + C::TM_S + st * 128 + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
             tc_wait_st();
             tc_fence_before();
+            // Observe EVERY phase of pv_done in order (a parity wait is only safe when the waiter is at most one
+            // phase behind): PV(g-1) here -- long complete, and PV(g) cannot start before P(g) is posted below --
+            // and PV(last) in the epilogue.  Skipping phases let a short item's epilogue pass its wait on a
+            // stale phase while the MMA warp was still waiting for that item's first V tile.
+            if (kt > 0) mbar_wait(&B->pv_done, (g - 1) & 1, 114, item_it * 100000 + kt * 1000 + it.n_kt);
             mbar_arrive(&B->p_full[st]);
         }
         kv_it += it.n_kt;
 
         // epilogue: out = O / l
-        mbar_wait(&B->pv_done, (kv_it - 1) & 1);
+        mbar_wait(&B->pv_done, (kv_it - 1) & 1, 113, item_it * 100000 + id);
         tc_fence_after();
         const float inv = 1.f / l;
         const bool valid = t < it.ql;
