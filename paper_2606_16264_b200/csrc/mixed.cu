@@ -58,7 +58,7 @@ decode_kernel(DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __gr
 }
 
 
-constexpr int kPrefillThreads = 192;  // warps 0-3 softmax, warp 4 TMA producer, warp 5 MMA issuer
+constexpr int kPrefillThreads = 224;  // warps 0-3 softmax, warp 4 K producer, warp 5 MMA issuer, warp 6 V producer
 
 template <int D>
 __global__ void __launch_bounds__(kPrefillThreads, 1)
@@ -84,8 +84,9 @@ prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __
     __syncthreads();
     tc_fence_after();
     if (warp < 4) prefill_softmax<D>(A, B, warp);
-    else if (warp == 4) prefill_producer<D>(A, B, tiles, &tm_q, &tm_k, &tm_v);
-    else prefill_mma<D>(A, B, tiles);
+    else if (warp == 4) prefill_producer<D>(A, B, tiles, &tm_q, &tm_k);
+    else if (warp == 5) prefill_mma<D>(A, B, tiles);
+    else prefill_producer_v<D>(A, B, tiles, &tm_v);
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(B->tmem_base, C::TM_COLS);
@@ -98,7 +99,7 @@ prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __
 //                       these warps become decode workers too, with rings carved out of the (now idle)
 //                       prefill tile memory
 //   WG1 (warps 4-7)   : decode workers, one private TMA ring each (HBM streaming, 120 regs)
-//   WG2 (warps 8-11)  : warp 8 prefill TMA producer, warp 9 tcgen05 MMA issuer, 10-11 idle (48 regs)
+//   WG2 (warps 8-11)  : warp 8 prefill Q/K TMA producer, warp 9 tcgen05 MMA issuer, warp 10 V producer (48 regs)
 //   WG3 (warps 12-15) : decode workers (120 regs)
 // Prefill items and decode units are popped from two ticket counters, so on every SM the tensor
 // pipe (prefill) and the HBM stream (decode) are busy at the same time for the whole step.
@@ -159,8 +160,9 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
     } else if (wg == 2) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
-        if (warp == 8) prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k, &tm_v);
+        if (warp == 8) prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k);
         else if (warp == 9) prefill_mma<D>(PA, PB, tiles);
+        else if (warp == 10) prefill_producer_v<D>(PA, PB, tiles, &tm_v);
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 120;");
         const int dw = (wg == 1) ? warp - 4 : warp - 8;

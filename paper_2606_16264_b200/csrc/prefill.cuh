@@ -10,13 +10,13 @@
 //     O += P V            tcgen05.mma, A = P (TMEM), B = V (smem, MN-major SW128), fp32 in TMEM
 // and finally out = O / l (bf16), lse = ln2 * (m + log2 l).
 //
-// Three warp roles, all persistent over the item queue (tickets popped by the producer and
+// Warp roles, all persistent over the item queue (tickets popped by the producer and
 // handed to the other roles through a 2-deep shared-memory mailbox):
-//   producer warp : TMA. Q tile (3-D map, 2 boxes) and, per KV tile, the 8 page-heads of K and of V
-//                   (2-D map, one 64-col x 16-row SW128 box per page-head half, issued by 16 lanes in
-//                   parallel) into ONE 3-slot ring filled in the order the MMA warp consumes tiles
-//                   (K0, K1, V0, K2, V1, ...).  The HND pool makes every box one contiguous 2 KiB
-//                   run of HBM/L2.
+//   producer warps: TMA. Q tile (3-D map, 2 boxes) and, per KV tile, the 8 page-heads of K and of V
+//                   (2-D map, one 64-col x 16-row SW128 box per page-head half) into ONE 3-slot ring
+//                   filled in the order the MMA warp consumes tiles (K0, K1, V0, K2, V1, ...); one warp
+//                   issues the K tiles, a second one the V tiles.  The HND pool makes every box one
+//                   contiguous 2 KiB run of HBM/L2.
 //   MMA warp      : one elected lane issues S(kt+1) ahead of PV(kt) so the tensor pipe works on
 //                   the next scores while the softmax warps work on the current ones.
 //   softmax warps : 4 warps, thread r owns query row r (TMEM lane r): no shuffles.
@@ -90,7 +90,7 @@ __device__ __forceinline__ PrefillItem load_item(const PrefillArgs& A, int id) {
 __device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
     for (int i = 0; i < 2; ++i) {
         mbar_init(&B->item_full[i], 1);
-        mbar_init(&B->item_empty[i], 5);  // MMA lane 0 + lane 0 of each softmax warp
+        mbar_init(&B->item_empty[i], 6);  // lane 0 of: MMA warp, V producer warp, each softmax warp
         mbar_init(&B->s_full[i], 1);
         mbar_init(&B->p_full[i], 128);
     }
@@ -105,22 +105,50 @@ __device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// producer warp
+// producer warps.  Ring entries follow the MMA warp's consumption order K0, K1, V0, K2, V1, ..., K(n-1),
+// V(n-2), V(n-1); both producers walk that sequence and each fills the entries of its own kind, so K and V
+// tiles are issued in parallel (a 128-key tile is 16 TMA boxes: one warp issuing all 32 of an iteration was
+// the prefill role's bottleneck).
+struct RingCursor {
+    int slot;
+    uint32_t phase;  // parity of the current use of `slot`
+    __device__ __forceinline__ void advance(int nslots) {
+        if (++slot == nslots) { slot = 0; phase ^= 1; }
+    }
+};
+
+// One KV tile (8 page-heads) of item `it` into the cursor's slot: lane -> (page p, half cb), one box per lane.
+template <int D>
+__device__ __forceinline__ void prefill_load_tile(const PrefillArgs& A, PrefillBars* B, uint8_t* ring,
+                                                  const PrefillItem& it, const int* pt, int n_pages, int kt,
+                                                  const CUtensorMap* tm, const RingCursor& cur, int lane) {
+    using C = PrefillCfg<D>;
+    const int np = min(8, n_pages - kt * 8);
+    const int p = lane / C::CB, cb = lane % C::CB;
+    const bool act = p < np && lane < 8 * C::CB;
+    const int page = act ? __ldg(pt + kt * 8 + p) : 0;
+    const int r0 = (page * A.pool.Hkv + it.hk) * kPageSize;
+    const uint32_t off = cb * C::HALF_BYTES + p * C::PAGE_BOX;
+    mbar_wait(&B->kv_empty[cur.slot], cur.phase ^ 1, 103);
+    if (lane == 0) mbar_arrive_expect_tx(&B->kv_full[cur.slot], np * C::CB * C::PAGE_BOX);
+    __syncwarp();
+    if (act) tma_load_2d(ring + cur.slot * C::TILE_BYTES + off, tm, cb * 64, r0, &B->kv_full[cur.slot]);
+}
+
+// warp A: pops the item tickets, loads Q and the K tiles
 template <int D>
 __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBars* B, uint8_t* tiles,
-                                                 const CUtensorMap* tm_q, const CUtensorMap* tm_k,
-                                                 const CUtensorMap* tm_v) {
+                                                 const CUtensorMap* tm_q, const CUtensorMap* tm_k) {
     using C = PrefillCfg<D>;
     const int lane = threadIdx.x & 31;
     const int n_items = A.hdr[HDR_N_ITEMS];
     uint8_t* q_s = tiles;
     uint8_t* ring = tiles + C::TILE_BYTES;
     uint32_t item_it = 0;
-    int slot = 0;
-    uint32_t phase = 0;  // parity of the current use of `slot`
+    RingCursor cur = {0, 0};
     for (;;) {
         const int ms = item_it & 1;
-        mbar_wait(&B->item_empty[ms], ((item_it >> 1) & 1) ^ 1, 101, item_it);
+        mbar_wait(&B->item_empty[ms], ((item_it >> 1) & 1) ^ 1, 101);
         int id = 0;
         if (lane == 0) {
             id = atomicAdd(A.ticket, 1);
@@ -132,7 +160,7 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
         const PrefillItem it = load_item(A, id);
         const int* pt = A.b.page_table + (size_t)it.req * A.b.stride;
 
-        mbar_wait(&B->q_empty, (item_it & 1) ^ 1, 102, item_it);
+        mbar_wait(&B->q_empty, (item_it & 1) ^ 1, 102);
         if (lane == 0) {
             mbar_arrive_expect_tx(&B->q_full, C::TILE_BYTES);
 #pragma unroll
@@ -140,24 +168,44 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
                 tma_load_3d(q_s + cb * C::HALF_BYTES, tm_q, cb * 64, it.h, it.tok0 + it.qt * kQTile, &B->q_full);
         }
         const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
-        // tiles in the order the MMA warp consumes them: K0, K1, V0, K2, V1, ..., K(n-1), V(n-2), V(n-1)
-        auto load_tile = [&](int kt, const CUtensorMap* tm) {
-            const int np = min(8, n_pages - kt * 8);
-            const int p = lane / C::CB, cb = lane % C::CB;  // lane -> (page p, half cb) of this tile
-            const bool act = p < np && lane < 8 * C::CB;
-            const int page = act ? __ldg(pt + kt * 8 + p) : 0;
-            const int r0 = (page * A.pool.Hkv + it.hk) * kPageSize;
-            const uint32_t off = cb * C::HALF_BYTES + p * C::PAGE_BOX;
-            mbar_wait(&B->kv_empty[slot], phase ^ 1, 103, item_it * 100000 + kt * 1000 + slot * 100 + it.n_kt);
-            if (lane == 0) mbar_arrive_expect_tx(&B->kv_full[slot], np * C::CB * C::PAGE_BOX);
-            __syncwarp();
-            if (act) tma_load_2d(ring + slot * C::TILE_BYTES + off, tm, cb * 64, r0, &B->kv_full[slot]);
-            if (++slot == C::KV_SLOTS) { slot = 0; phase ^= 1; }
-        };
-        load_tile(0, tm_k);
+        prefill_load_tile<D>(A, B, ring, it, pt, n_pages, 0, tm_k, cur, lane);
+        cur.advance(C::KV_SLOTS);
         for (int kt = 0; kt < it.n_kt; ++kt) {
-            if (kt + 1 < it.n_kt) load_tile(kt + 1, tm_k);
-            load_tile(kt, tm_v);
+            if (kt + 1 < it.n_kt) {
+                prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt + 1, tm_k, cur, lane);
+                cur.advance(C::KV_SLOTS);
+            }
+            cur.advance(C::KV_SLOTS);  // V(kt): the other producer's entry
+        }
+        ++item_it;
+    }
+}
+
+// warp B: the V tiles of the same item sequence (item ids come through the mailbox)
+template <int D>
+__device__ __forceinline__ void prefill_producer_v(const PrefillArgs& A, PrefillBars* B, uint8_t* tiles,
+                                                   const CUtensorMap* tm_v) {
+    using C = PrefillCfg<D>;
+    const int lane = threadIdx.x & 31;
+    const int n_items = A.hdr[HDR_N_ITEMS];
+    uint8_t* ring = tiles + C::TILE_BYTES;
+    uint32_t item_it = 0;
+    RingCursor cur = {0, 0};
+    for (;;) {
+        const int ms = item_it & 1;
+        mbar_wait(&B->item_full[ms], (item_it >> 1) & 1, 115);
+        const int id = B->mailbox[ms];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&B->item_empty[ms]);
+        if (id >= n_items) break;
+        const PrefillItem it = load_item(A, id);
+        const int* pt = A.b.page_table + (size_t)it.req * A.b.stride;
+        const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
+        cur.advance(C::KV_SLOTS);  // K0
+        for (int kt = 0; kt < it.n_kt; ++kt) {
+            if (kt + 1 < it.n_kt) cur.advance(C::KV_SLOTS);  // K(kt+1)
+            prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt, tm_v, cur, lane);
+            cur.advance(C::KV_SLOTS);
         }
         ++item_it;
     }
