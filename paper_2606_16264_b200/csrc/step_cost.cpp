@@ -14,10 +14,11 @@ struct BuiltinFit {
     tropical_cost_model_t m;
 };
 
-// Filled from measured kernel times by paper_2606_16264_b200/fit_cost_model.py (values are
-// copied here by hand after a fit run; provenance in DESIGN.md).  Empty until calibrated.
+// Coefficients fitted to measured step times by `python -m paper_2606_16264_b200.cost_fit fit` from the grid
+// that `... cost_fit measure` wrote on a B200 (calibration/b200_grid.csv; provenance in DESIGN.md section 7).
 const BuiltinFit kBuiltin[] = {
-    {0, 0, 0, {0, 0, 0, 0, 0, 0, 148}},
+    {0, 0, 0, {0, 0, 0, 0, 0, 0, 148}},  // sentinel: never matches
+#include "cost_model_fit.inc"
 };
 
 void features(int Hq, int Hkv, int d, int P, int n, const int32_t* q, const int32_t* c,

@@ -123,3 +123,27 @@ def test_step_cost_properties_with_explicit_model():
     assert us >= max(bd.t_tc_us, bd.t_hbm_us)
     with pytest.raises(tb.TropicalError):
         tb.step_cost(6, 4, 128, 16, [1], [1], model=m)
+
+
+def test_builtin_cost_model_reproduces_measured_grid():
+    """A6: the compiled-in coefficients (csrc/cost_model_fit.inc) against the B200 measurements they were fitted to
+    (paper_2606_16264_b200/calibration/b200_grid.csv).  Held-out rows (seed % 5 == 0) were not used by the fit.
+    The paper gives no accuracy target; the bars are this build's."""
+    import numpy as np
+    from paper_2606_16264_b200 import cost_fit
+    rows = cost_fit.read_grid(cost_fit.DEFAULT_GRID)
+    assert len(rows) >= 200
+    for shape in sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows}):
+        rel_all, rel_held = [], []
+        for r in rows:
+            if (r["Hq"], r["Hkv"], r["d"]) != shape:
+                continue
+            q, c = cost_fit.grid_lengths(r["prefill_tokens"], r["prefill_ctx"], r["n_decode"], r["ctx_median"], r["seed"])
+            us, bd = tb.step_cost(*shape, 16, q.tolist(), c.tolist())
+            assert us >= max(bd.t_tc_us, bd.t_hbm_us)
+            rel = abs(us - r["us_median"]) / r["us_median"]
+            rel_all.append(rel)
+            if cost_fit.is_held_out(r):
+                rel_held.append(rel)
+        assert np.mean(rel_held) <= 0.15, (shape, np.mean(rel_held))
+        assert np.max(rel_all) <= 0.40, (shape, np.max(rel_all))
