@@ -167,6 +167,20 @@ int tropical_debug_attention_simt(const tropical_kv_pool_t *pool, const tropical
  * launches, kept only to time the two phases apart (A/B evidence under profiles/).  Process-global. */
 void tropical_debug_set_mode(int mode);
 
+/* Test hook: cap the number of CTAs of the persistent step kernel (0 = one per SM, the default), so that small
+ * test batches put MANY tiles through each CTA's queues (multi-item sequencing of every role).  Process-global. */
+void tropical_debug_set_grid(int num_ctas);
+
+/* Test hook: force the decode split size in pages (multiple of 8; 0 = automatic, from the step's page count), so
+ * that small test batches exercise multi-block decode units.  Process-global. */
+void tropical_debug_set_split_pages(int pages);
+
+/* Measurement hook, only in builds compiled with -DTROPICAL_WAIT_PROF (else TROPICAL_ERR_UNSUPPORTED): cycles spent
+ * in and calls of every mbarrier wait of the step kernel, summed over warps, indexed by the wait's tag (the numbers
+ * next to the mbar_wait calls in csrc/).  cycles/calls are [host] arrays of n <= 512 entries; reset != 0 zeroes
+ * the device counters after the read.  Synchronises the device. */
+int tropical_debug_wait_profile(uint64_t *cycles, uint64_t *calls, int32_t n, int32_t reset);
+
 /* Measurement hook: role timestamps of the LAST fused step kernel that ran with this workspace
  * (globaltimer nanoseconds): out_ns[0] kernel start (earliest CTA), [1] prefill queue drained (latest
  * softmax warp), [2] latest dedicated decode warp done, [3] latest late-joining decode warp done.

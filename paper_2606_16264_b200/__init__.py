@@ -13,6 +13,9 @@ from .binding import (  # noqa: F401
     debug_attention_simt,
     debug_read_profile,
     debug_set_mode,
+    debug_set_grid,
+    debug_set_split_pages,
+    debug_wait_profile,
     kv_append,
     kv_gather,
     last_launch_count,

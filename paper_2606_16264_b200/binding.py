@@ -49,7 +49,7 @@ EXPORTS = (
     "tropical_kv_append", "tropical_kv_gather", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
-    "tropical_debug_attention_simt", "tropical_debug_set_mode", "tropical_debug_read_profile",
+    "tropical_debug_attention_simt", "tropical_debug_set_mode", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile",
 )
 
 
@@ -92,6 +92,27 @@ def version() -> str:
 def debug_set_mode(mode: int) -> None:
     """0 = fused step kernel (default, the product path); 1 = separate prefill / decode launches (timing A/B)."""
     lib().tropical_debug_set_mode(ctypes.c_int(int(mode)))
+
+
+def debug_set_grid(num_ctas: int) -> None:
+    """Test hook: cap the CTAs of the persistent step kernel (0 = one per SM)."""
+    lib().tropical_debug_set_grid(ctypes.c_int(int(num_ctas)))
+
+
+def debug_set_split_pages(pages: int) -> None:
+    """Test hook: force the decode split size in pages (0 = automatic)."""
+    lib().tropical_debug_set_split_pages(ctypes.c_int(int(pages)))
+
+
+def debug_wait_profile(reset: bool = True):
+    """{tag: (cycles, calls)} of the step kernel's mbarrier waits; None unless built with -DTROPICAL_WAIT_PROF."""
+    cyc = (ctypes.c_uint64 * 512)()
+    cnt = (ctypes.c_uint64 * 512)()
+    rc = lib().tropical_debug_wait_profile(cyc, cnt, ctypes.c_int32(512), ctypes.c_int32(1 if reset else 0))
+    if rc == 2:
+        return None
+    _check(rc, "tropical_debug_wait_profile")
+    return {t: (int(cyc[t]), int(cnt[t])) for t in range(512) if cnt[t]}
 
 
 def debug_read_profile(workspace: torch.Tensor, stream=None):

@@ -267,6 +267,17 @@ int tropical_debug_read_profile(const void* workspace, uint64_t* out_ns, void* c
 
 void tropical_debug_set_mode(int mode) { set_debug_mode(mode == 1 ? 1 : 0); }
 
+void tropical_debug_set_grid(int num_ctas) { set_debug_grid(num_ctas); }
+
+void tropical_debug_set_split_pages(int pages) { set_debug_split_pages(pages); }
+
+int tropical_debug_wait_profile(uint64_t* cycles, uint64_t* calls, int32_t n, int32_t reset) {
+    if (cycles == nullptr || calls == nullptr || n <= 0) return TROPICAL_ERR_INVALID_ARG;
+    const int got = read_wait_profile((unsigned long long*)cycles, (unsigned long long*)calls, n, reset);
+    if (got < 0) return cuda_fail(cudaGetLastError(), "wait_profile");
+    return got == 0 ? TROPICAL_ERR_UNSUPPORTED : TROPICAL_OK;
+}
+
 const char* tropical_last_cuda_error(void) { return g_cuda_err; }
 
 const char* tropical_version(void) { return "tropical-b200 0.1 (sm_100a)"; }

@@ -80,23 +80,48 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+#ifdef TROPICAL_WAIT_PROF
+// Measurement build only (-DTROPICAL_WAIT_PROF): cycles and calls of every mbar_wait, by tag (lane 0 of each warp).
+static __device__ unsigned long long g_wait_cycles[512];
+static __device__ unsigned long long g_wait_calls[512];
+#endif
+
 // Bounded wait: a protocol bug traps (launch failure) instead of hanging the GPU box.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0, int aux = 0) {
-    if (mbar_try_wait(bar, parity)) return;
-    long long t0 = clock64();
-    while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > 4000000000LL) {  // ~2 s at 1.9 GHz
-#ifdef TROPICAL_DEBUG_WAIT
-            if ((threadIdx.x & 31) == 0) printf("mbar timeout: block %d warp %d tag %d parity %u aux %d\n", blockIdx.x, threadIdx.x >> 5, tag, parity, aux);
-            long long t1 = clock64();
-            while (clock64() - t1 < 1500000000LL) {}  // let every stuck warp report before the trap
+#ifdef TROPICAL_WAIT_PROF
+    const long long tp = clock64();
 #endif
-            __trap();
+    if (!mbar_try_wait(bar, parity)) {
+        long long t0 = clock64();
+        while (!mbar_try_wait(bar, parity)) {
+            if (clock64() - t0 > 4000000000LL) {  // ~2 s at 1.9 GHz
+#ifdef TROPICAL_DEBUG_WAIT
+                if ((threadIdx.x & 31) == 0) printf("mbar timeout: block %d warp %d tag %d parity %u aux %d\n", blockIdx.x, threadIdx.x >> 5, tag, parity, aux);
+                long long t1 = clock64();
+                while (clock64() - t1 < 1500000000LL) {}  // let every stuck warp report before the trap
+#endif
+                __trap();
+            }
         }
     }
+#ifdef TROPICAL_WAIT_PROF
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&g_wait_cycles[tag & 511], (unsigned long long)(clock64() - tp));
+        atomicAdd(&g_wait_calls[tag & 511], 1ull);
+    }
+#endif
     (void)tag;
     (void)aux;
 }
+
+// position in a ring of mbarrier-guarded shared-memory slots
+struct RingCursor {
+    int slot;
+    uint32_t phase;  // parity of the current use of `slot`
+    __device__ __forceinline__ void advance(int nslots) {
+        if (++slot == nslots) { slot = 0; phase ^= 1; }
+    }
+};
 
 __device__ __forceinline__ void fence_proxy_async() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -201,6 +226,51 @@ __device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&r
         : "memory");
 }
 
+__device__ __forceinline__ void tmem_st_32x32_x16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+        ::"r"(taddr),
+          "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+
+// 32 lanes x 8 consecutive 32-bit columns (decode tiles: one thread per key / per d row, 8 heads)
+__device__ __forceinline__ void tmem_ld_32x32_x8(uint32_t taddr, uint32_t (&r)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st_32x32_x8(uint32_t taddr, const uint32_t (&r)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                 : "memory");
+}
+
+// ---------------------------------------------------------------- warpgroup-scope helpers (decode softmax)
+__device__ __forceinline__ float warp_max_f32(float v) {  // one CREDUX on sm_100a
+    float m;
+    asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(m) : "f"(v));
+    return m;
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("barrier.cta.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+// OR of a predicate over the `nthreads` threads that meet at named barrier `id`
+__device__ __forceinline__ bool named_bar_or(int id, int nthreads, bool pred) {
+    uint32_t r;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %3, 0;\n\t"
+        "barrier.cta.red.or.pred q, %1, %2, p;\n\t"
+        "selp.u32 %0, 1, 0, q;\n\t}"
+        : "=r"(r)
+        : "r"(id), "r"(nthreads), "r"((uint32_t)pred)
+        : "memory");
+    return r != 0;
+}
+
 // K-major / MN-major SWIZZLE_128B shared-memory matrix descriptor (sm_100 format, version 1).
 //   bits [0,14) start>>4, [16,30) LBO>>4, [32,46) SBO>>4, [46,48) version=1, [61,64) layout (2 = SW128)
 __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
@@ -213,15 +283,21 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t saddr, uint32_
     return d;
 }
 // kind::f16 instruction descriptor: bf16 x bf16 -> f32, M x N, A K-major, B K-major or MN-major
-__host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, bool b_mn_major) {
+__host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, bool b_mn_major, bool a_mn_major = false) {
     return (1u << 4)                       // c_format = F32
            | (1u << 7)                     // a_format = BF16
            | (1u << 10)                    // b_format = BF16
-           | (0u << 15)                    // a_major  = K
+           | ((a_mn_major ? 1u : 0u) << 15)
            | ((b_mn_major ? 1u : 0u) << 16)
            | ((uint32_t)(N >> 3) << 17)
            | ((uint32_t)(M >> 4) << 24);
 }
+
+// Broadcast lane 0's value: tells the compiler the result is warp-uniform, so operands of the uniform-datapath
+// instructions (UTCHMMA, UTCBAR, UTMALDG) built from it need no per-lane "waterfall" loop (ELECT / R2UR.BROADCAST /
+// BRA.U.ANY around every instruction: ~150 cycles per tcgen05.mma, measured in profiles/r1c_notes.md).
+__device__ __forceinline__ uint32_t uni(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
+__device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;

@@ -17,6 +17,9 @@ cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, cons
 cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
                                    float scale_log2, void* workspace, cudaStream_t stream, int* launches);
 void set_debug_mode(int mode);
+void set_debug_grid(int num_ctas);
+void set_debug_split_pages(int pages);
+int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset);
 size_t profile_offset_bytes();
 size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q);
 

@@ -4,6 +4,7 @@
 
 #include "common.cuh"
 #include "decode.cuh"
+#include "decode_tc.cuh"
 #include "kernels.h"
 #include "plan.cuh"
 #include "prefill.cuh"
@@ -94,50 +95,57 @@ prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __
 
 // ------------------------------------------------------------------------------------------------
 // The fused step kernel: ONE persistent launch, one CTA per SM, four warpgroups (512 threads, the whole
-// register file re-divided between the roles with setmaxnreg).
-//   WG0 (warps 0-3)   : prefill softmax / correction / epilogue (224 regs); when the prefill queue is empty
-//                       these warps become decode workers too, with rings carved out of the (now idle)
-//                       prefill tile memory
-//   WG1 (warps 4-7)   : decode workers, one private TMA ring each (HBM streaming, 120 regs)
-//   WG2 (warps 8-11)  : warp 8 prefill Q/K TMA producer, warp 9 tcgen05 MMA issuer, warp 10 V producer (48 regs)
-//   WG3 (warps 12-15) : decode workers (120 regs)
-// Prefill items and decode units are popped from two ticket counters, so on every SM the tensor
-// pipe (prefill) and the HBM stream (decode) are busy at the same time for the whole step.
+// register file re-divided between the roles with setmaxnreg).  Two tcgen05 pipelines run side by side on
+// every SM, each fed by its own ticket queue:
+//   WG0 (warps 0-3)   : prefill softmax / correction / epilogue                           (224 regs)
+//   WG2 (warps 8-10)  : prefill K producer (TMA), prefill MMA issuer, prefill V producer   (48 regs)
+//   WG1 (warps 4-7)   : decode softmax warpgroup (thread = key)                            (80 regs)
+//   WG3 (warps 12-13) : decode producer (TMA), decode MMA issuer                           (48 regs)
+// so the tensor pipe (prefill tiles) and the HBM stream (decode blocks) are busy together for the whole step.
+// When the prefill queue is empty, WG0 and warps 8-9 turn into a SECOND decode pipeline whose ring is the
+// (now idle) prefill tile memory: decode-heavy steps then have 192 KiB of K/V in flight per SM.
 constexpr int kMixedThreads = 512;
 
 template <int D>
 struct MixedCfg {
-    static constexpr int DEC_WARPS = 8;
-    static constexpr int DEC_RING = 12288;                                  // bytes of TMA ring per dedicated decode warp
-    static constexpr int DEC_STAGES = DEC_RING / DecodeCfg<D>::PAGE_BYTES;
-    static constexpr int LATE_RING = PrefillCfg<D>::SMEM_TILES / 4;         // WG0 after the prefill queue is empty
-    static constexpr int LATE_STAGES = LATE_RING / DecodeCfg<D>::PAGE_BYTES;
-    static constexpr int N_DEC_BARS = DEC_WARPS * DEC_STAGES + 4 * LATE_STAGES;
+    using DC = DecTcCfg<D>;
+    static constexpr int DEC_UNITS = 5;                                     // 16 KiB ring units of the decode pipeline
+    static constexpr int DEC_RING = DEC_UNITS * DC::UNIT_BYTES;
+    static constexpr int DEC_AUX = 2 * DC::QT_BYTES + 2 * DC::PT_BYTES;     // double-buffered Q^T and P^T tiles
+    static constexpr int LATE_UNITS = (PrefillCfg<D>::SMEM_TILES - DEC_AUX) / DC::UNIT_BYTES;  // second pipe, after prefill
     static constexpr int BAR_BYTES = 2048;
-    static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_WARPS * DEC_RING + BAR_BYTES + 1024;
-    static_assert(DEC_STAGES <= kMaxDecodeStages && LATE_STAGES <= kMaxDecodeStages, "stage barriers");
-    static_assert(LATE_RING % 1024 == 0 && DEC_RING % 1024 == 0, "ring alignment");
-    static_assert(sizeof(PrefillBars) + N_DEC_BARS * 8 <= BAR_BYTES, "barrier block");
+    // d = 64: the V^T operand is padded to M = 128 by pointing its second half one ring unit further (rows 64-127
+    // of O^T are never read); keep that read inside the allocation for the last ring unit as well
+    static constexpr int TAIL_PAD = (D == 64) ? 4096 : 0;
+    static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_RING + DEC_AUX + BAR_BYTES + TAIL_PAD + 1024;
+    static constexpr uint32_t TM_DEC = 384;                                 // decode TMEM columns 384..447 (prefill: 0..383)
+    static_assert(LATE_UNITS <= kDecMaxUnits && DEC_UNITS <= kDecMaxUnits, "ring barriers");
+    static_assert(sizeof(PrefillBars) + 2 * sizeof(DecBars) <= BAR_BYTES, "barrier block");
+    static_assert(SMEM <= 232448, "shared memory per CTA");
 };
 
 template <int D>
 __global__ void __launch_bounds__(kMixedThreads, 1)
-mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap tm_q,
+mixed_kernel(PrefillArgs PA, DecTcArgs DA, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_qd,
              const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
     using C = PrefillCfg<D>;
     using M = MixedCfg<D>;
+    using DC = DecTcCfg<D>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint8_t* rings = tiles + C::SMEM_TILES;
-    PrefillBars* PB = reinterpret_cast<PrefillBars*>(rings + M::DEC_WARPS * M::DEC_RING);
-    uint64_t* dec_full = reinterpret_cast<uint64_t*>(PB + 1);
-    const int warp = threadIdx.x >> 5, wg = warp >> 2;
+    uint8_t* dring = tiles + C::SMEM_TILES;
+    uint8_t* daux = dring + M::DEC_RING;
+    PrefillBars* PB = reinterpret_cast<PrefillBars*>(daux + M::DEC_AUX);
+    DecBars* DB = reinterpret_cast<DecBars*>(PB + 1);
+    const int warp = uni((int)(threadIdx.x >> 5)), wg = warp >> 2;
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tm_q);
+        tma_prefetch_desc(&tm_qd);
         tma_prefetch_desc(&tm_k);
         tma_prefetch_desc(&tm_v);
         prefill_init_bars(PB);
-        for (int i = 0; i < M::N_DEC_BARS; ++i) mbar_init(dec_full + i, 1);
+        dec_init_bars(DB);
+        dec_init_bars(DB + 1);
         fence_mbar_init();
         prof_mark(PA.hdr, 0, true);
     }
@@ -148,31 +156,58 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    const uint32_t tmem = PB->tmem_base;
+    DecPipe P1;  // the dedicated decode pipeline
+    P1.ring = dring;
+    P1.nunits = M::DEC_UNITS;
+    P1.qt = daux;
+    P1.pt = daux + 2 * DC::QT_BYTES;
+    P1.B = DB;
+    P1.tm = tmem + M::TM_DEC;
+    P1.bar_id = 1;
+    DecPipe P2;  // the late pipeline: prefill tile memory and TMEM columns, once the prefill queue is empty
+    P2.ring = tiles;
+    P2.nunits = M::LATE_UNITS;
+    P2.qt = tiles + M::LATE_UNITS * DC::UNIT_BYTES;
+    P2.pt = P2.qt + 2 * DC::QT_BYTES;
+    P2.B = DB + 1;
+    P2.tm = tmem;
+    P2.bar_id = 2;
+
     if (wg == 0) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         prefill_softmax<D>(PA, PB, warp);
-        // The terminating ticket was seen after the last item's final PV completed: every TMA load into the
-        // tile memory has been consumed, and the producer issues nothing more.  Reuse it for decode rings.
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 1, false);
-        DecodeRing R = make_ring(tiles + warp * M::LATE_RING, dec_full + M::DEC_WARPS * M::DEC_STAGES + warp * M::LATE_STAGES,
-                                 M::LATE_STAGES);
-        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
+        // Every prefill MMA has completed (the last epilogue read its O), so every TMA load into the tile
+        // memory has been consumed: hand the memory to the late decode pipeline.
+        named_bar_sync(3, 192);
+        dec_softmax<D>(DA, P2, warp);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
+    } else if (wg == 1) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
+        dec_softmax<D>(DA, P1, warp - 4);
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
     } else if (wg == 2) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
-        if (warp == 8) prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k);
-        else if (warp == 9) prefill_mma<D>(PA, PB, tiles);
-        else if (warp == 10) prefill_producer_v<D>(PA, PB, tiles, &tm_v);
+        if (warp == 8) {
+            prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k);
+            named_bar_sync(3, 192);
+            dec_producer<D>(DA, P2, &tm_qd, &tm_k, &tm_v);
+        } else if (warp == 9) {
+            prefill_mma<D>(PA, PB, tiles);
+            named_bar_sync(3, 192);
+            dec_mma<D>(DA, P2);
+        } else if (warp == 10) {
+            prefill_producer_v<D>(PA, PB, tiles, &tm_v);
+        }
     } else {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 120;");
-        const int dw = (wg == 1) ? warp - 4 : warp - 8;
-        DecodeRing R = make_ring(rings + dw * M::DEC_RING, dec_full + dw * M::DEC_STAGES, M::DEC_STAGES);
-        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
-        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
+        if (warp == 12) dec_producer<D>(DA, P1, &tm_qd, &tm_k, &tm_v);
+        else if (warp == 13) dec_mma<D>(DA, P1);
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) tmem_dealloc(PB->tmem_base, C::TM_COLS);
+    if (warp == 0) tmem_dealloc(tmem, C::TM_COLS);
 }
 
 template <int D>
@@ -202,6 +237,27 @@ size_t profile_offset_bytes() { return make_layout(1, 1, 64, 1, 1).hdr + HDR_PRO
 
 static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches (A/B timing only)
 void set_debug_mode(int mode) { g_mode = mode; }
+static int g_grid_cap = 0;  // test hook: 0 = one CTA per SM
+int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset) {
+#ifdef TROPICAL_WAIT_PROF
+    if (n > 512) n = 512;
+    if (cudaMemcpyFromSymbol(cycles, g_wait_cycles, n * sizeof(unsigned long long)) != cudaSuccess) return -1;
+    if (cudaMemcpyFromSymbol(calls, g_wait_calls, n * sizeof(unsigned long long)) != cudaSuccess) return -1;
+    if (reset) {
+        static unsigned long long zeros[512];
+        cudaMemcpyToSymbol(g_wait_cycles, zeros, sizeof zeros);
+        cudaMemcpyToSymbol(g_wait_calls, zeros, sizeof zeros);
+    }
+    return n;
+#else
+    (void)cycles; (void)calls; (void)n; (void)reset;
+    return 0;
+#endif
+}
+
+static int g_split_pages = 0;  // test hook: 0 = automatic
+void set_debug_split_pages(int pages) { g_split_pages = pages > 0 ? (pages + 7) / 8 * 8 : 0; }
+void set_debug_grid(int num_ctas) { g_grid_cap = num_ctas > 0 ? num_ctas : 0; }
 
 template <int D>
 static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
@@ -213,15 +269,16 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     P.req_info = (int4*)(ws + w.req_info);
     P.items = (int2*)(ws + w.items);
     P.units = (int4*)(ws + w.units);
-    plan_kernel<<<1, kPlanThreads, 0, stream>>>(b, pool.Hq, pool.Hkv, P);
+    plan_kernel<<<1, kPlanThreads, 0, stream>>>(b, pool.Hq, pool.Hkv, P, g_split_pages);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     ++*launches;
 
-    CUtensorMap tm_q, tm_k, tm_v;
+    CUtensorMap tm_q, tm_qd, tm_k, tm_v;
     const long long rows = (long long)pool.num_pages * pool.Hkv * kPageSize;
     if (!encode_pool_map(&tm_k, pool.k_pool, rows, D) || !encode_pool_map(&tm_v, pool.v_pool, rows, D) ||
-        !encode_q_map(&tm_q, q, b.total_q, pool.Hq, D))
+        !encode_q_map(&tm_q, q, b.total_q, pool.Hq, D, 1, kQTile) ||
+        !encode_q_map(&tm_qd, q, b.total_q, pool.Hq, D, kHeadBlock, 1))
         return cudaErrorInvalidValue;
 
     PrefillArgs PA;
@@ -248,6 +305,19 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     A.part_ml = (float2*)(ws + w.part_ml);
     A.part_o = (float*)(ws + w.part_o);
 
+    DecTcArgs TA;
+    TA.pool = pool;
+    TA.b = b;
+    TA.out = (uint16_t*)out;
+    TA.lse = lse;
+    TA.scale_log2 = scale_log2;
+    TA.hdr = P.hdr;
+    TA.ticket = P.hdr + HDR_TICKET_DECODE;
+    TA.req_info = P.req_info;
+    TA.units = P.units;
+    TA.part_ml = A.part_ml;
+    TA.part_o = A.part_o;
+
     if (g_mode == 0) {
         // A3 + A4 in one persistent launch
         const size_t smem = MixedCfg<D>::SMEM;
@@ -257,7 +327,7 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
             if (e != cudaSuccess) return e;
             attr_m = true;
         }
-        mixed_kernel<D><<<num_sms(), kMixedThreads, smem, stream>>>(PA, A, tm_q, tm_k, tm_v);
+        mixed_kernel<D><<<(g_grid_cap > 0 && g_grid_cap < num_sms()) ? g_grid_cap : num_sms(), kMixedThreads, smem, stream>>>(PA, TA, tm_q, tm_qd, tm_k, tm_v);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         ++*launches;

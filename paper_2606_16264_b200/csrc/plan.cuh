@@ -64,7 +64,7 @@ __device__ __forceinline__ int find_owner(const int4* __restrict__ info, int n, 
 
 constexpr int kPlanThreads = 1024;
 
-__global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P) {
+__global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split) {
     __shared__ int s_units[kPlanThreads], s_items[kPlanThreads];
     __shared__ int s_pages;
     const int tid = threadIdx.x;
@@ -84,6 +84,8 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     const long long page_heads = (long long)s_pages * Hkv * HB;
     int split = (int)((page_heads + kTargetUnits - 1) / kTargetUnits);
     if (split < kMinSplitPages) split = kMinSplitPages;
+    split = (split + 7) / 8 * 8;  // whole 128-key blocks: only a request's last unit is ragged
+    if (forced_split > 0) split = forced_split;  // test hook (workspace sizing assumes split >= 8)
 
     int my_units = 0, my_items = 0;
     for (int i = i0; i < i1; ++i) {

@@ -87,6 +87,14 @@ __device__ __forceinline__ PrefillItem load_item(const PrefillArgs& A, int id) {
     return it;
 }
 
+// the same item with every field broadcast from lane 0 (warp-uniform for the compiler: see uni())
+__device__ __forceinline__ PrefillItem load_item_uniform(const PrefillArgs& A, int id) {
+    PrefillItem it = load_item(A, id);
+    it.req = uni(it.req); it.qt = uni(it.qt); it.h = uni(it.h); it.hk = uni(it.hk);
+    it.c = uni(it.c); it.ql = uni(it.ql); it.tok0 = uni(it.tok0); it.l_tile = uni(it.l_tile); it.n_kt = uni(it.n_kt);
+    return it;
+}
+
 __device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
     for (int i = 0; i < 2; ++i) {
         mbar_init(&B->item_full[i], 1);
@@ -109,13 +117,6 @@ __device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
 // V(n-2), V(n-1); both producers walk that sequence and each fills the entries of its own kind, so K and V
 // tiles are issued in parallel (a 128-key tile is 16 TMA boxes: one warp issuing all 32 of an iteration was
 // the prefill role's bottleneck).
-struct RingCursor {
-    int slot;
-    uint32_t phase;  // parity of the current use of `slot`
-    __device__ __forceinline__ void advance(int nslots) {
-        if (++slot == nslots) { slot = 0; phase ^= 1; }
-    }
-};
 
 // One KV tile (8 page-heads) of item `it` into the cursor's slot: lane -> (page p, half cb), one box per lane.
 template <int D>
@@ -212,15 +213,15 @@ __device__ __forceinline__ void prefill_producer_v(const PrefillArgs& A, Prefill
 }
 
 // ------------------------------------------------------------------------------------------------
-// MMA warp
+// MMA warp.  All 32 lanes run the (warp-uniform) control flow; one elected lane issues the tcgen05 instructions.
 template <int D>
 __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B, uint8_t* tiles) {
     using C = PrefillCfg<D>;
     const int lane = threadIdx.x & 31;
-    const int n_items = A.hdr[HDR_N_ITEMS];
-    const uint32_t q_a = smem_u32(tiles);
+    const int n_items = uni(A.hdr[HDR_N_ITEMS]);
+    const uint32_t q_a = uni(smem_u32(tiles));
     const uint32_t ring_a = q_a + C::TILE_BYTES;
-    const uint32_t tm = B->tmem_base;
+    const uint32_t tm = uni(B->tmem_base);
     constexpr uint32_t IDESC_S = make_idesc_bf16(128, 128, false);
     constexpr uint32_t IDESC_O = make_idesc_bf16(128, D, true);
     uint32_t item_it = 0, kv_it = 0;
@@ -234,8 +235,8 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
         const int st = g & 1;
         mbar_wait(&B->kv_full[slot], phase, 104, item_it * 100000 + g * 100 + slot);
         tc_fence_after();
-        if (lane == 0) {
-            const uint32_t k_a = ring_a + slot * C::TILE_BYTES;
+        const uint32_t k_a = ring_a + slot * C::TILE_BYTES;
+        if (elect_one()) {
 #pragma unroll
             for (int cb = 0; cb < C::CB; ++cb)
 #pragma unroll
@@ -254,11 +255,11 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
     for (;;) {
         const int ms = item_it & 1;
         mbar_wait(&B->item_full[ms], (item_it >> 1) & 1, 105, item_it);
-        const int id = B->mailbox[ms];
+        const int id = uni(B->mailbox[ms]);
         __syncwarp();
         if (lane == 0) mbar_arrive(&B->item_empty[ms]);
         if (id >= n_items) break;
-        const PrefillItem it = load_item(A, id);
+        const PrefillItem it = load_item_uniform(A, id);
 
         mbar_wait(&B->q_full, item_it & 1, 106, item_it);
         issue_s(kv_it);
@@ -268,7 +269,7 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
             if (kt + 1 < it.n_kt) {
                 issue_s(g + 1);
             } else {
-                if (lane == 0) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
+                if (elect_one()) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
                 __syncwarp();
             }
             mbar_wait(&B->kv_full[slot], phase, 107, item_it * 100000 + kt * 1000 + slot * 100 + it.n_kt);  // the next ring tile is V(kt)
@@ -287,7 +288,7 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
             if (kt == 0) mbar_wait(&B->o_empty, (item_it & 1) ^ 1, 108, item_it * 100000 + id);  // previous item's epilogue has read O
             mbar_wait(&B->p_full[st], (g >> 1) & 1, 109, item_it * 100000 + kt * 1000 + it.n_kt);
             tc_fence_after();
-            if (lane == 0) {
+            if (elect_one()) {
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks)  // 16 keys per MMA
                     tc_mma_ts(tm + C::TM_O, tm + C::TM_S + st * 128 + ks * 8,
@@ -334,21 +335,29 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
             const int st = g & 1;
             mbar_wait(&B->s_full[st], (g >> 1) & 1, 111, item_it * 100000 + kt * 1000 + it.n_kt);
             tc_fence_after();
-            uint32_t s[128];
-#pragma unroll
-            for (int c4 = 0; c4 < 4; ++c4) tmem_ld_32x32(tm + C::TM_S + st * 128 + c4 * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c4 * 32]));
-            tc_wait_ld();
+            // The tile is walked twice in 32-column chunks (row maximum, then exponentials) with ROLLED loops: the
+            // second TMEM read is cheap, and the loop body stays ~150 instructions -- the fully unrolled 128-column
+            // version (~630 instructions per tile) thrashed the instruction cache that the four roles of an SM
+            // sub-partition share (55 % of this warp's samples were no-instruction stalls, profiles/r1c_c5.md).
+            const uint32_t s_col = tm + C::TM_S + st * 128;
             const int n_vis = limit - kt * kKvTile + 1;  // visible columns of this tile for this row
-            if (n_vis < kKvTile) {
-#pragma unroll
-                for (int j = 0; j < 128; ++j)
-                    if (j >= n_vis) s[j] = 0xff800000u;  // -inf, by select: the score may be NaN
-            }
+            const bool masked = __any_sync(0xffffffffu, n_vis < kKvTile);
             float mx = -INFINITY;
+#pragma unroll 1
+            for (int c4 = 0; c4 < 4; ++c4) {
+                uint32_t s[32];
+                tmem_ld_32x32(s_col + c4 * 32, s);
+                tc_wait_ld();
+                if (masked) {
 #pragma unroll
-            for (int j = 0; j < 128; j += 4)
-                mx = fmaxf(mx, max4(__uint_as_float(s[j]), __uint_as_float(s[j + 1]), __uint_as_float(s[j + 2]),
-                                    __uint_as_float(s[j + 3])));
+                    for (int j = 0; j < 32; ++j)
+                        if (c4 * 32 + j >= n_vis) s[j] = 0xff800000u;  // -inf, by select: the score may be NaN
+                }
+#pragma unroll
+                for (int j = 0; j < 32; j += 4)
+                    mx = fmaxf(mx, max4(__uint_as_float(s[j]), __uint_as_float(s[j + 1]), __uint_as_float(s[j + 2]),
+                                        __uint_as_float(s[j + 3])));
+            }
             const float m_new = mx * scale;
             if (kt == 0) {
                 m_used = m_new;  // finite: key 0 is visible to every row
@@ -358,7 +367,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
                     const float alpha = grow ? fast_exp2(m_used - m_new) : 1.f;
                     mbar_wait(&B->pv_done, (g - 1) & 1, 112, item_it * 100000 + kt * 1000 + it.n_kt);  // O holds PV(g-1)
                     tc_fence_after();
-#pragma unroll
+#pragma unroll 1
                     for (int c4 = 0; c4 < D / 32; ++c4) {
                         uint32_t o[32];
                         tmem_ld_32x32(tm + C::TM_O + c4 * 32, o);
@@ -372,18 +381,29 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
                 }
             }
             float sum0 = 0.f, sum1 = 0.f;
-            uint32_t pk[64];
+#pragma unroll 1
+            for (int c4 = 0; c4 < 4; ++c4) {
+                uint32_t s[32];
+                tmem_ld_32x32(s_col + c4 * 32, s);
+                tc_wait_ld();
+                if (masked) {
 #pragma unroll
-            for (int j = 0; j < 128; j += 2) {
-                const float p0 = fast_exp2(fmaf(__uint_as_float(s[j]), scale, -m_used));
-                const float p1 = fast_exp2(fmaf(__uint_as_float(s[j + 1]), scale, -m_used));
-                sum0 += p0;
-                sum1 += p1;
-                pk[j >> 1] = pack_bf16x2(p0, p1);
+                    for (int j = 0; j < 32; ++j)
+                        if (c4 * 32 + j >= n_vis) s[j] = 0xff800000u;
+                }
+                uint32_t pk[16];
+#pragma unroll
+                for (int j = 0; j < 32; j += 2) {
+                    const float p0 = fast_exp2(fmaf(__uint_as_float(s[j]), scale, -m_used));
+                    const float p1 = fast_exp2(fmaf(__uint_as_float(s[j + 1]), scale, -m_used));
+                    sum0 += p0;
+                    sum1 += p1;
+                    pk[j >> 1] = pack_bf16x2(p0, p1);
+                }
+                // P columns [16 c4, 16 c4 + 16) overwrite S columns this thread has already read in this pass
+                tmem_st_32x32_x16(s_col + c4 * 16, pk);
             }
             l += sum0 + sum1;
-            tmem_st_32x32(tm + C::TM_S + st * 128, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
-            tmem_st_32x32(tm + C::TM_S + st * 128 + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
             tc_wait_st();
             tc_fence_before();
             // Observe EVERY phase of pv_done in order (a parity wait is only safe when the waiter is at most one
@@ -401,7 +421,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
         const float inv = 1.f / l;
         const bool valid = t < it.ql;
         uint16_t* orow = A.out + ((size_t)(it.tok0 + t) * A.pool.Hq + it.h) * D;
-#pragma unroll
+#pragma unroll 1
         for (int c4 = 0; c4 < D / 32; ++c4) {
             uint32_t o[32];
             tmem_ld_32x32(tm + C::TM_O + c4 * 32, o);

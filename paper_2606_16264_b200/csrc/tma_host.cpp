@@ -40,13 +40,14 @@ bool encode_pool_map(CUtensorMap* map, const void* base, long long rows, int D) 
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// q viewed as 3-D bf16 [T][Hq][D]; box = 64 cols x 1 head x 128 tokens, SWIZZLE_128B.
-bool encode_q_map(CUtensorMap* map, const void* base, int T, int Hq, int D) {
+// q viewed as 3-D bf16 [T][Hq][D]; box = 64 cols x box_heads x box_tokens, SWIZZLE_128B:
+// (1 head x 128 tokens) = a prefill Q tile half, (8 heads x 1 token) = a decode Q^T half.
+bool encode_q_map(CUtensorMap* map, const void* base, int T, int Hq, int D, int box_heads, int box_tokens) {
     EncodeTiledFn enc = resolve_encode();
     if (!enc) return false;
     cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)T};
     cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
-    cuuint32_t box[3] = {64, 1, 128};
+    cuuint32_t box[3] = {64, (cuuint32_t)box_heads, (cuuint32_t)box_tokens};
     cuuint32_t estr[3] = {1, 1, 1};
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
