@@ -114,6 +114,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int ta
     (void)aux;
 }
 
+// measurement builds: total lifetime of a role (same counters as the waits, tag = role id)
+__device__ __forceinline__ long long prof_begin() {
+#ifdef TROPICAL_WAIT_PROF
+    return clock64();
+#else
+    return 0;
+#endif
+}
+__device__ __forceinline__ void prof_end(int tag, long long t0) {
+#ifdef TROPICAL_WAIT_PROF
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&g_wait_cycles[tag & 511], (unsigned long long)(clock64() - t0));
+        atomicAdd(&g_wait_calls[tag & 511], 1ull);
+    }
+#else
+    (void)tag; (void)t0;
+#endif
+}
+
 // position in a ring of mbarrier-guarded shared-memory slots
 struct RingCursor {
     int slot;

@@ -83,7 +83,7 @@ struct DecTcArgs {
 __device__ __forceinline__ void dec_init_bars(DecBars* B) {
     for (int i = 0; i < 2; ++i) {
         mbar_init(&B->unit_full[i], 1);
-        mbar_init(&B->unit_empty[i], 5);  // lane 0 of the MMA warp and of each softmax warp
+        mbar_init(&B->unit_empty[i], 6);  // lane 0 of the V producer, the MMA warp and each softmax warp
         mbar_init(&B->qt_full[i], 1);
         mbar_init(&B->qt_empty[i], 1);
         mbar_init(&B->s_full[i], 1);
@@ -125,77 +125,104 @@ __device__ __forceinline__ DecUnit dec_load_unit(const DecTcArgs& A, int u) {
     return U;
 }
 
-// ------------------------------------------------------------------------------------------------ producer
-template <int D>
-__device__ __forceinline__ void dec_producer(const DecTcArgs& A, const DecPipe& P, const CUtensorMap* tm_qd,
-                                             const CUtensorMap* tm_k, const CUtensorMap* tm_v) {
+// ------------------------------------------------------------------------------------------------ producers
+// Ring entries follow the MMA warp's consumption order K(0), K(1), V(0), K(2), V(1), ..., V(nb-1); the K producer
+// (KIND 0: pops the unit tickets, loads Q^T and the K units) and the V producer (KIND 1) both walk that sequence and
+// each fills the entries of its own kind.  One rolled loop over "steps" keeps a single copy of the issue code (the
+// roles of an SM share a 32 KiB L1.5 instruction cache); boxes are issued lane-parallel (lane = page / half).  Page
+// ids are read 32 at a time, one chunk ahead, so no global-load latency sits between two blocks.
+template <int D, int KIND>
+__device__ __noinline__ void dec_producer(const DecTcArgs& A, const DecPipe& P, const CUtensorMap* tm_qd,
+                                          const CUtensorMap* tm_kv) {
     using C = DecTcCfg<D>;
     DecBars* B = P.B;
     const int lane = threadIdx.x & 31;
-    const int n_units = A.hdr[HDR_N_UNITS];
-    const int g = A.pool.Hq / A.pool.Hkv;
+    const int n_units = uni(A.hdr[HDR_N_UNITS]);
+    const int g = uni(A.pool.Hq / A.pool.Hkv), Hkv = uni(A.pool.Hkv);
+    uint8_t* ring = P.ring;
+    const int nunits = uni(P.nunits);
     uint32_t unit_it = 0;
     RingCursor cur = {0, 0};
     for (;;) {
         const int ms = unit_it & 1;
         const uint32_t par = (unit_it >> 1) & 1;
-        mbar_wait(&B->unit_empty[ms], par ^ 1, 301);
         int u = 0;
-        if (lane == 0) {
-            u = atomicAdd(A.ticket, 1);
-            B->mailbox[ms] = u;
-            mbar_arrive(&B->unit_full[ms]);
+        if (KIND == 0) {
+            mbar_wait(&B->unit_empty[ms], par ^ 1, 301);
+            if (lane == 0) {
+                u = atomicAdd(A.ticket, 1);
+                B->mailbox[ms] = u;
+                mbar_arrive(&B->unit_full[ms]);
+            }
+            u = __shfl_sync(0xffffffffu, u, 0);
+        } else {
+            mbar_wait(&B->unit_full[ms], par, 305);
+            u = uni(B->mailbox[ms]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&B->unit_empty[ms]);
         }
-        u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= n_units) break;
         const DecUnit U = dec_load_unit(A, u);
-        const int tok = __ldg(A.b.q_offsets + U.req);
-        const int h0 = U.kvh * g + U.hb * kHeadBlock;
-        mbar_wait(&B->qt_empty[ms], par ^ 1, 302);
-        if (lane == 0) {
-            mbar_arrive_expect_tx(&B->qt_full[ms], C::CB * 1024);
-#pragma unroll
-            for (int cb = 0; cb < C::CB; ++cb)
-                tma_load_3d(P.qt + ms * C::QT_BYTES + cb * 2048, tm_qd, cb * 64, h0, tok, &B->qt_full[ms]);
-        }
         const int* pt = A.b.page_table + (size_t)U.req * A.b.stride + U.p0;
-        // ring entries follow the MMA warp's consumption order: K(0), K(1), V(0), K(2), V(1), ..., V(nb-1)
-        auto load_k = [&](int b) {  // K units of block b: 128 keys x 64 columns each
-            const int npb = min(kDecBlockPages, U.np - b * kDecBlockPages);
-            const int page = lane < npb ? __ldg(pt + b * kDecBlockPages + lane) : 0;
+        int pg_cur = lane < U.np ? __ldg(pt + lane) : 0;
+        int pg_next = 32 + lane < U.np ? __ldg(pt + 32 + lane) : 0;
+        if (KIND == 0) {
+            const int tok = uni(__ldg(A.b.q_offsets + U.req));
+            const int h0 = U.kvh * g + U.hb * kHeadBlock;
+            mbar_wait(&B->qt_empty[ms], par ^ 1, 302);
+            if (elect_one()) {
+                mbar_arrive_expect_tx(&B->qt_full[ms], C::CB * 1024);
 #pragma unroll
-            for (int cb = 0; cb < C::CB; ++cb) {
-                mbar_wait(&B->ring_empty[cur.slot], cur.phase ^ 1, 303);
-                if (lane == 0) mbar_arrive_expect_tx(&B->ring_full[cur.slot], npb * 2048);
-                __syncwarp();
-                if (lane < npb)
-                    tma_load_2d(P.ring + cur.slot * C::UNIT_BYTES + lane * 2048, tm_k, cb * 64,
-                                (page * A.pool.Hkv + U.kvh) * kPageSize, &B->ring_full[cur.slot]);
-                cur.advance(P.nunits);
+                for (int cb = 0; cb < C::CB; ++cb)
+                    tma_load_3d(P.qt + ms * C::QT_BYTES + cb * 2048, tm_qd, cb * 64, h0, tok, &B->qt_full[ms]);
             }
-        };
-        auto load_v = [&](int b) {  // V units of block b: V_KEYS keys x d columns each
-            const int npb = min(kDecBlockPages, U.np - b * kDecBlockPages);
-            const int page = lane < npb ? __ldg(pt + b * kDecBlockPages + lane) : 0;
-#pragma unroll
-            for (int j = 0; j < C::CB; ++j) {
-                const int npj = min(C::V_PAGES, npb - j * C::V_PAGES);
-                if (npj <= 0) break;
+        }
+        for (int s = 0; s <= U.nb; ++s) {
+            const int b = KIND == 0 ? s : s - 1;  // the block this producer loads in step s
+            int npb = 0;
+            if (b >= 0 && b < U.nb) {
+                npb = min(kDecBlockPages, U.np - b * kDecBlockPages);
+                if (b > 0 && (b & 3) == 0) {
+                    pg_cur = pg_next;
+                    pg_next = b * kDecBlockPages + 32 + lane < U.np ? __ldg(pt + b * kDecBlockPages + 32 + lane) : 0;
+                }
+            }
+            if (s < U.nb) {  // K units of block s: 128 keys x 64 columns each
+                if (KIND == 0) {
+                    const int page = __shfl_sync(0xffffffffu, pg_cur, ((b & 3) * kDecBlockPages + lane) & 31);
+#pragma unroll 1
+                    for (int cb = 0; cb < C::CB; ++cb) {
+                        mbar_wait(&B->ring_empty[cur.slot], cur.phase ^ 1, 303);
+                        if (lane == 0) mbar_arrive_expect_tx(&B->ring_full[cur.slot], npb * 2048);
+                        __syncwarp();
+                        if (lane < npb)
+                            tma_load_2d(ring + cur.slot * C::UNIT_BYTES + lane * 2048, tm_kv, cb * 64,
+                                        (page * Hkv + U.kvh) * kPageSize, &B->ring_full[cur.slot]);
+                        cur.advance(nunits);
+                    }
+                } else {
+                    for (int cb = 0; cb < C::CB; ++cb) cur.advance(nunits);
+                }
+            }
+            if (s > 0) {  // V units of block s - 1: V_KEYS keys x d columns each
+                const int npv = KIND == 0 ? min(kDecBlockPages, U.np - (s - 1) * kDecBlockPages) : npb;
                 const int pp = lane / C::CB, cb = lane % C::CB;
-                const int page_l = __shfl_sync(0xffffffffu, page, (j * C::V_PAGES + pp) & 31);
-                mbar_wait(&B->ring_empty[cur.slot], cur.phase ^ 1, 304);
-                if (lane == 0) mbar_arrive_expect_tx(&B->ring_full[cur.slot], npj * C::CB * 2048);
-                __syncwarp();
-                if (lane < npj * C::CB)
-                    tma_load_2d(P.ring + cur.slot * C::UNIT_BYTES + cb * (C::V_KEYS * 128) + pp * 2048, tm_v, cb * 64,
-                                (page_l * A.pool.Hkv + U.kvh) * kPageSize, &B->ring_full[cur.slot]);
-                cur.advance(P.nunits);
+#pragma unroll 1
+                for (int j = 0; j < C::CB; ++j) {
+                    const int npj = min(C::V_PAGES, npv - j * C::V_PAGES);
+                    if (npj <= 0) break;
+                    if (KIND == 1) {
+                        const int page = __shfl_sync(0xffffffffu, pg_cur, ((b & 3) * kDecBlockPages + j * C::V_PAGES + pp) & 31);
+                        mbar_wait(&B->ring_empty[cur.slot], cur.phase ^ 1, 304);
+                        if (lane == 0) mbar_arrive_expect_tx(&B->ring_full[cur.slot], npj * C::CB * 2048);
+                        __syncwarp();
+                        if (lane < npj * C::CB)
+                            tma_load_2d(ring + cur.slot * C::UNIT_BYTES + cb * (C::V_KEYS * 128) + pp * 2048, tm_kv, cb * 64,
+                                        (page * Hkv + U.kvh) * kPageSize, &B->ring_full[cur.slot]);
+                    }
+                    cur.advance(nunits);
+                }
             }
-        };
-        load_k(0);
-        for (int b = 0; b < U.nb; ++b) {
-            if (b + 1 < U.nb) load_k(b + 1);
-            load_v(b);
         }
         ++unit_it;
     }
@@ -203,7 +230,7 @@ __device__ __forceinline__ void dec_producer(const DecTcArgs& A, const DecPipe& 
 
 // ------------------------------------------------------------------------------------------------ MMA issuer
 template <int D>
-__device__ __forceinline__ void dec_mma(const DecTcArgs& A, const DecPipe& P) {
+__device__ __noinline__ void dec_mma(const DecTcArgs& A, const DecPipe& P) {
     using C = DecTcCfg<D>;
     DecBars* B = P.B;
     const int lane = threadIdx.x & 31;
@@ -227,43 +254,41 @@ __device__ __forceinline__ void dec_mma(const DecTcArgs& A, const DecPipe& P) {
         const DecUnit U = dec_load_unit(A, u);
         const uint32_t tm_o = tm_base + C::TM_OT + ms * 16;
 
-        auto issue_s = [&](int b) {  // S^T(b) = K(b) Q^T into S^T slot (blk_it + b) & 1
-            const int st = (blk_it + b) & 1;
+        mbar_wait(&B->qt_full[ms], par, 313);
+        // step s issues S^T(s) (ahead) and then PV(s - 1): one copy of each issue sequence
+        for (int s = 0; s <= U.nb; ++s) {
+            if (s < U.nb) {  // S^T(s) = K(s) Q^T into S^T slot (blk_it + s) & 1
+                const int st = (blk_it + s) & 1;
+#pragma unroll 1
+                for (int cb = 0; cb < C::CB; ++cb) {
+                    mbar_wait(&B->ring_full[cur.slot], cur.phase, 312);
+                    tc_fence_after();
+                    const uint32_t k_a = ring_a + cur.slot * C::UNIT_BYTES;
+                    const uint32_t q_a = qt_a + ms * C::QT_BYTES + cb * 2048;
+                    if (elect_one()) {
 #pragma unroll
-            for (int cb = 0; cb < C::CB; ++cb) {
-                mbar_wait(&B->ring_full[cur.slot], cur.phase, 312);
-                tc_fence_after();
-                const uint32_t k_a = ring_a + cur.slot * C::UNIT_BYTES;
-                const uint32_t q_a = qt_a + ms * C::QT_BYTES + cb * 2048;
+                        for (int k4 = 0; k4 < 4; ++k4)
+                            tc_mma_ss(tm_base + C::TM_ST + st * 16, make_smem_desc_sw128(k_a + k4 * 32, 0, 1024),
+                                      make_smem_desc_sw128(q_a + k4 * 32, 0, 1024), IDESC_S, (cb | k4) != 0);
+                        tc_commit(&B->ring_empty[cur.slot]);
+                    }
+                    __syncwarp();
+                    cur.advance(nunits);
+                }
                 if (elect_one()) {
-#pragma unroll
-                    for (int k4 = 0; k4 < 4; ++k4)
-                        tc_mma_ss(tm_base + C::TM_ST + st * 16, make_smem_desc_sw128(k_a + k4 * 32, 0, 1024),
-                                  make_smem_desc_sw128(q_a + k4 * 32, 0, 1024), IDESC_S, (cb | k4) != 0);
-                    tc_commit(&B->ring_empty[cur.slot]);
+                    tc_commit(&B->s_full[st]);
+                    if (s + 1 == U.nb) tc_commit(&B->qt_empty[ms]);  // every S^T MMA of this unit has been issued
                 }
                 __syncwarp();
-                cur.advance(nunits);
             }
-            if (elect_one()) tc_commit(&B->s_full[st]);
-            __syncwarp();
-        };
-
-        mbar_wait(&B->qt_full[ms], par, 313);
-        issue_s(0);
-        for (int b = 0; b < U.nb; ++b) {
-            if (b + 1 < U.nb) {
-                issue_s(b + 1);
-            } else {
-                if (elect_one()) tc_commit(&B->qt_empty[ms]);  // every S^T MMA of this unit has been issued
-                __syncwarp();
-            }
+            if (s == 0) continue;
+            const int b = s - 1;
             const uint32_t gb = blk_it + b;
             const int st = gb & 1;
             const int npb = min(kDecBlockPages, U.np - b * kDecBlockPages);
             const int nvalid_blk = min(kDecBlockKeys, U.key_end - b * kDecBlockKeys);
             bool first = true;
-#pragma unroll
+#pragma unroll 1
             for (int j = 0; j < C::CB; ++j) {
                 const int npj = min(C::V_PAGES, npb - j * C::V_PAGES);
                 if (npj <= 0) break;
@@ -286,13 +311,14 @@ __device__ __forceinline__ void dec_mma(const DecTcArgs& A, const DecPipe& P) {
                     first = false;
                 }
                 tc_fence_after();
+                const uint32_t p_a = pt_a + st * C::PT_BYTES + ((j * C::V_KEYS) >> 6) * 2048 + (((j * C::V_KEYS) & 63) >> 4) * 32;
                 if (elect_one()) {
 #pragma unroll
                     for (int ks = 0; ks < C::V_KEYS / 16; ++ks) {
-                        const int key0 = j * C::V_KEYS + ks * 16;
-                        const uint32_t p_a = pt_a + st * C::PT_BYTES + (key0 >> 6) * 2048 + ((key0 & 63) >> 4) * 32;
+                        // 16 keys per MMA: +32 B inside a 64-key P^T half, next half after 4 steps
+                        const uint32_t pk = p_a + (ks >> 2) * 2048 + (ks & 3) * 32;
                         tc_mma_ss(tm_o, make_smem_desc_sw128(v_a + ks * 2048, C::V_KEYS * 128, 1024),
-                                  make_smem_desc_sw128(p_a, 0, 1024), IDESC_O, (b | j | ks) != 0);
+                                  make_smem_desc_sw128(pk, 0, 1024), IDESC_O, (b | j | ks) != 0);
                     }
                     tc_commit(&B->ring_empty[cur.slot]);
                 }
@@ -312,7 +338,7 @@ __device__ __forceinline__ void dec_mma(const DecTcArgs& A, const DecPipe& P) {
 
 // ------------------------------------------------------------------------------------------------ softmax warpgroup
 template <int D>
-__device__ __forceinline__ void dec_softmax(const DecTcArgs& A, const DecPipe& P, int wg_warp) {
+__device__ __noinline__ void dec_softmax(const DecTcArgs& A, const DecPipe& P, int wg_warp) {
     using C = DecTcCfg<D>;
     DecBars* B = P.B;
     const int lane = threadIdx.x & 31;
@@ -359,7 +385,6 @@ __device__ __forceinline__ void dec_softmax(const DecTcArgs& A, const DecPipe& P
             }
             bool raise = true;  // first block of a unit: m is -inf
             if (b > 0) raise = named_bar_or(P.bar_id, 128, over);
-            bool waited = false;
             if (raise) {
                 float* rb = &B->red[gb & 1][0][0];
 #pragma unroll
@@ -377,9 +402,11 @@ __device__ __forceinline__ void dec_softmax(const DecTcArgs& A, const DecPipe& P
                     l[h] *= alpha[h];
                     m[h] = mn;
                 }
-                if (b > 0) {  // rescale O^T (this thread: d row r) once PV(b-1) has landed
+                if (b > 0) {  // rescale O^T (this thread: d row r) once PV(b-1) has landed.  The parity wait is
+                    // unambiguous although this warp does not observe every phase: s_full(gb) was seen, S^T(gb)
+                    // was issued after PV(gb-2) and tcgen05 ops complete in issue order, so at least gb-1 phases
+                    // of pv_done are complete; PV(gb) cannot be issued before p_full(gb) is posted below.
                     mbar_wait(&B->pv_done, (gb - 1) & 1, 323);
-                    waited = true;
                     tc_fence_after();
                     uint32_t o[8];
                     tmem_ld_32x32_x8(tm_o, o);
@@ -401,8 +428,6 @@ __device__ __forceinline__ void dec_softmax(const DecTcArgs& A, const DecPipe& P
                 }
             }
             fence_proxy_async();
-            // observe every phase of pv_done in order (see prefill_softmax)
-            if (b > 0 && !waited) mbar_wait(&B->pv_done, (gb - 1) & 1, 324);
             mbar_arrive(&B->p_full[st]);
         }
         blk_it += U.nb;

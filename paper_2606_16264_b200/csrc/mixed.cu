@@ -175,35 +175,39 @@ mixed_kernel(PrefillArgs PA, DecTcArgs DA, const __grid_constant__ CUtensorMap t
     P2.bar_id = 2;
 
     if (wg == 0) {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+        const long long t0 = prof_begin();
         prefill_softmax<D>(PA, PB, warp);
+        prof_end(120, t0);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 1, false);
         // Every prefill MMA has completed (the last epilogue read its O), so every TMA load into the tile
         // memory has been consumed: hand the memory to the late decode pipeline.
-        named_bar_sync(3, 192);
+        named_bar_sync(3, 224);
         dec_softmax<D>(DA, P2, warp);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
     } else if (wg == 1) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
+        const long long t0 = prof_begin();
         dec_softmax<D>(DA, P1, warp - 4);
+        prof_end(320, t0);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
     } else if (wg == 2) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
         if (warp == 8) {
             prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k);
-            named_bar_sync(3, 192);
-            dec_producer<D>(DA, P2, &tm_qd, &tm_k, &tm_v);
+            named_bar_sync(3, 224);
+            dec_producer<D, 0>(DA, P2, &tm_qd, &tm_k);
         } else if (warp == 9) {
             prefill_mma<D>(PA, PB, tiles);
-            named_bar_sync(3, 192);
+            named_bar_sync(3, 224);
             dec_mma<D>(DA, P2);
         } else if (warp == 10) {
             prefill_producer_v<D>(PA, PB, tiles, &tm_v);
+            named_bar_sync(3, 224);
+            dec_producer<D, 1>(DA, P2, &tm_qd, &tm_v);
         }
     } else {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
-        if (warp == 12) dec_producer<D>(DA, P1, &tm_qd, &tm_k, &tm_v);
-        else if (warp == 13) dec_mma<D>(DA, P1);
+        const long long t0 = prof_begin();
+        if (warp == 12) { dec_producer<D, 0>(DA, P1, &tm_qd, &tm_k); prof_end(300, t0); }
+        else if (warp == 13) { dec_mma<D>(DA, P1); prof_end(310, t0); }
+        else if (warp == 14) dec_producer<D, 1>(DA, P1, &tm_qd, &tm_v);
     }
     tc_fence_before();
     __syncthreads();

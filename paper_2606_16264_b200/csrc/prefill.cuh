@@ -142,7 +142,7 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
                                                  const CUtensorMap* tm_q, const CUtensorMap* tm_k) {
     using C = PrefillCfg<D>;
     const int lane = threadIdx.x & 31;
-    const int n_items = A.hdr[HDR_N_ITEMS];
+    const int n_items = uni(A.hdr[HDR_N_ITEMS]);
     uint8_t* q_s = tiles;
     uint8_t* ring = tiles + C::TILE_BYTES;
     uint32_t item_it = 0;
@@ -158,25 +158,23 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
         }
         id = __shfl_sync(0xffffffffu, id, 0);
         if (id >= n_items) break;
-        const PrefillItem it = load_item(A, id);
+        const PrefillItem it = load_item_uniform(A, id);
         const int* pt = A.b.page_table + (size_t)it.req * A.b.stride;
 
         mbar_wait(&B->q_empty, (item_it & 1) ^ 1, 102);
-        if (lane == 0) {
+        if (elect_one()) {
             mbar_arrive_expect_tx(&B->q_full, C::TILE_BYTES);
 #pragma unroll
             for (int cb = 0; cb < C::CB; ++cb)
                 tma_load_3d(q_s + cb * C::HALF_BYTES, tm_q, cb * 64, it.h, it.tok0 + it.qt * kQTile, &B->q_full);
         }
         const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
-        prefill_load_tile<D>(A, B, ring, it, pt, n_pages, 0, tm_k, cur, lane);
-        cur.advance(C::KV_SLOTS);
-        for (int kt = 0; kt < it.n_kt; ++kt) {
-            if (kt + 1 < it.n_kt) {
-                prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt + 1, tm_k, cur, lane);
+        for (int s = 0; s <= it.n_kt; ++s) {  // ring order K0, K1, V0, K2, V1, ...: step s = K(s), then V(s-1)
+            if (s < it.n_kt) {
+                prefill_load_tile<D>(A, B, ring, it, pt, n_pages, s, tm_k, cur, lane);
                 cur.advance(C::KV_SLOTS);
             }
-            cur.advance(C::KV_SLOTS);  // V(kt): the other producer's entry
+            if (s > 0) cur.advance(C::KV_SLOTS);  // V(s-1): the other producer's entry
         }
         ++item_it;
     }
@@ -188,25 +186,26 @@ __device__ __forceinline__ void prefill_producer_v(const PrefillArgs& A, Prefill
                                                    const CUtensorMap* tm_v) {
     using C = PrefillCfg<D>;
     const int lane = threadIdx.x & 31;
-    const int n_items = A.hdr[HDR_N_ITEMS];
+    const int n_items = uni(A.hdr[HDR_N_ITEMS]);
     uint8_t* ring = tiles + C::TILE_BYTES;
     uint32_t item_it = 0;
     RingCursor cur = {0, 0};
     for (;;) {
         const int ms = item_it & 1;
         mbar_wait(&B->item_full[ms], (item_it >> 1) & 1, 115);
-        const int id = B->mailbox[ms];
+        const int id = uni(B->mailbox[ms]);
         __syncwarp();
         if (lane == 0) mbar_arrive(&B->item_empty[ms]);
         if (id >= n_items) break;
-        const PrefillItem it = load_item(A, id);
+        const PrefillItem it = load_item_uniform(A, id);
         const int* pt = A.b.page_table + (size_t)it.req * A.b.stride;
         const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
-        cur.advance(C::KV_SLOTS);  // K0
-        for (int kt = 0; kt < it.n_kt; ++kt) {
-            if (kt + 1 < it.n_kt) cur.advance(C::KV_SLOTS);  // K(kt+1)
-            prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt, tm_v, cur, lane);
-            cur.advance(C::KV_SLOTS);
+        for (int s = 0; s <= it.n_kt; ++s) {
+            if (s < it.n_kt) cur.advance(C::KV_SLOTS);  // K(s): the other producer's entry
+            if (s > 0) {
+                prefill_load_tile<D>(A, B, ring, it, pt, n_pages, s - 1, tm_v, cur, lane);
+                cur.advance(C::KV_SLOTS);
+            }
         }
         ++item_it;
     }
@@ -231,27 +230,6 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
         if (++slot == C::KV_SLOTS) { slot = 0; phase ^= 1; }
     };
 
-    auto issue_s = [&](uint32_t g) {  // S(g) = Q K^T into S slot g & 1; consumes the next ring tile (a K tile)
-        const int st = g & 1;
-        mbar_wait(&B->kv_full[slot], phase, 104, item_it * 100000 + g * 100 + slot);
-        tc_fence_after();
-        const uint32_t k_a = ring_a + slot * C::TILE_BYTES;
-        if (elect_one()) {
-#pragma unroll
-            for (int cb = 0; cb < C::CB; ++cb)
-#pragma unroll
-                for (int k4 = 0; k4 < 4; ++k4) {
-                    const uint32_t o = cb * C::HALF_BYTES + k4 * 32;
-                    tc_mma_ss(tm + C::TM_S + st * 128, make_smem_desc_sw128(q_a + o, 0, 1024),
-                              make_smem_desc_sw128(k_a + o, 0, 1024), IDESC_S, (cb | k4) != 0);
-                }
-            tc_commit(&B->s_full[st]);
-            tc_commit(&B->kv_empty[slot]);
-        }
-        __syncwarp();
-        advance();
-    };
-
     for (;;) {
         const int ms = item_it & 1;
         mbar_wait(&B->item_full[ms], (item_it >> 1) & 1, 105, item_it);
@@ -262,16 +240,35 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
         const PrefillItem it = load_item_uniform(A, id);
 
         mbar_wait(&B->q_full, item_it & 1, 106, item_it);
-        issue_s(kv_it);
-        for (int kt = 0; kt < it.n_kt; ++kt) {
+        // step s issues S(s) (ahead) and then PV(s - 1): the tensor pipe works on the next scores while the softmax
+        // warps work on the current ones; one copy of each issue sequence (instruction-cache footprint)
+        for (int s = 0; s <= it.n_kt; ++s) {
+            if (s < it.n_kt) {  // S(g) = Q K^T into S slot g & 1; consumes the next ring tile (a K tile)
+                const uint32_t g = kv_it + s;
+                const int st = g & 1;
+                mbar_wait(&B->kv_full[slot], phase, 104, item_it * 100000 + g * 100 + slot);
+                tc_fence_after();
+                const uint32_t k_a = ring_a + slot * C::TILE_BYTES;
+                if (elect_one()) {
+#pragma unroll
+                    for (int cb = 0; cb < C::CB; ++cb)
+#pragma unroll
+                        for (int k4 = 0; k4 < 4; ++k4) {
+                            const uint32_t o = cb * C::HALF_BYTES + k4 * 32;
+                            tc_mma_ss(tm + C::TM_S + st * 128, make_smem_desc_sw128(q_a + o, 0, 1024),
+                                      make_smem_desc_sw128(k_a + o, 0, 1024), IDESC_S, (cb | k4) != 0);
+                        }
+                    tc_commit(&B->s_full[st]);
+                    tc_commit(&B->kv_empty[slot]);
+                    if (s + 1 == it.n_kt) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
+                }
+                __syncwarp();
+                advance();
+            }
+            if (s == 0) continue;
+            const int kt = s - 1;
             const uint32_t g = kv_it + kt;
             const int st = g & 1;
-            if (kt + 1 < it.n_kt) {
-                issue_s(g + 1);
-            } else {
-                if (elect_one()) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
-                __syncwarp();
-            }
             mbar_wait(&B->kv_full[slot], phase, 107, item_it * 100000 + kt * 1000 + slot * 100 + it.n_kt);  // the next ring tile is V(kt)
             const uint32_t v_a = ring_a + slot * C::TILE_BYTES;
             if (kt + 1 == it.n_kt) {  // zero V rows past the last visible key (stale or poisoned smem)
