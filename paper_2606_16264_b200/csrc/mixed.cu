@@ -214,6 +214,74 @@ mixed_kernel(PrefillArgs PA, DecTcArgs DA, const __grid_constant__ CUtensorMap t
     if (warp == 0) tmem_dealloc(tmem, C::TM_COLS);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Variant "ws" of the step kernel (debug mode 2, A/B evidence): the same prefill roles, but the decode tiles run
+// on 8 independent warp workers (warp-level mma.sync tiles of decode.cuh, a private 12 KiB TMA ring each) instead
+// of the tcgen05 decode pipelines.
+template <int D>
+struct MixedWsCfg {
+    static constexpr int DEC_WARPS = 8;
+    static constexpr int DEC_RING = 12288;
+    static constexpr int DEC_STAGES = DEC_RING / DecodeCfg<D>::PAGE_BYTES;
+    static constexpr int LATE_RING = PrefillCfg<D>::SMEM_TILES / 4;
+    static constexpr int LATE_STAGES = LATE_RING / DecodeCfg<D>::PAGE_BYTES;
+    static constexpr int N_DEC_BARS = DEC_WARPS * DEC_STAGES + 4 * LATE_STAGES;
+    static constexpr int BAR_BYTES = 2048;
+    static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_WARPS * DEC_RING + BAR_BYTES + 1024;
+    static_assert(DEC_STAGES <= kMaxDecodeStages && LATE_STAGES <= kMaxDecodeStages, "stage barriers");
+    static_assert(sizeof(PrefillBars) + N_DEC_BARS * 8 <= BAR_BYTES, "barrier block");
+};
+
+template <int D>
+__global__ void __launch_bounds__(kMixedThreads, 1)
+mixed_ws_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap tm_q,
+                const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
+    using C = PrefillCfg<D>;
+    using M = MixedWsCfg<D>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* rings = tiles + C::SMEM_TILES;
+    PrefillBars* PB = reinterpret_cast<PrefillBars*>(rings + M::DEC_WARPS * M::DEC_RING);
+    uint64_t* dec_full = reinterpret_cast<uint64_t*>(PB + 1);
+    const int warp = uni((int)(threadIdx.x >> 5)), wg = warp >> 2;
+    if (threadIdx.x == 0) {
+        tma_prefetch_desc(&tm_q);
+        tma_prefetch_desc(&tm_k);
+        tma_prefetch_desc(&tm_v);
+        prefill_init_bars(PB);
+        for (int i = 0; i < M::N_DEC_BARS; ++i) mbar_init(dec_full + i, 1);
+        fence_mbar_init();
+        prof_mark(PA.hdr, 0, true);
+    }
+    if (warp == 0) {
+        tmem_alloc(&PB->tmem_base, C::TM_COLS);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    if (wg == 0) {
+        prefill_softmax<D>(PA, PB, warp);
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 1, false);
+        DecodeRing R = make_ring(tiles + warp * M::LATE_RING, dec_full + M::DEC_WARPS * M::DEC_STAGES + warp * M::LATE_STAGES,
+                                 M::LATE_STAGES);
+        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
+    } else if (wg == 2) {
+        if (warp == 8) prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k);
+        else if (warp == 9) prefill_mma<D>(PA, PB, tiles);
+        else if (warp == 10) prefill_producer_v<D>(PA, PB, tiles, &tm_v);
+    } else {
+        const int dw = (wg == 1) ? warp - 4 : warp - 8;
+        DecodeRing R = make_ring(rings + dw * M::DEC_RING, dec_full + dw * M::DEC_STAGES, M::DEC_STAGES);
+        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(PB->tmem_base, C::TM_COLS);
+}
+
 template <int D>
 __global__ void __launch_bounds__(128) combine_kernel(CombineArgs A) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -239,7 +307,7 @@ size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q) 
 
 size_t profile_offset_bytes() { return make_layout(1, 1, 64, 1, 1).hdr + HDR_PROF * sizeof(int); }
 
-static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches (A/B timing only)
+static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches; 2: fused, tcgen05 decode pipelines (1, 2: A/B timing only)
 void set_debug_mode(int mode) { g_mode = mode; }
 static int g_grid_cap = 0;  // test hook: 0 = one CTA per SM
 int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset) {
@@ -322,8 +390,8 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     TA.part_ml = A.part_ml;
     TA.part_o = A.part_o;
 
-    if (g_mode == 0) {
-        // A3 + A4 in one persistent launch
+    if (g_mode == 2) {
+        // A3 + A4 in one persistent launch, decode tiles on the tcgen05 pipelines (A/B variant)
         const size_t smem = MixedCfg<D>::SMEM;
         static bool attr_m = false;
         if (!attr_m) {
@@ -332,6 +400,20 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
             attr_m = true;
         }
         mixed_kernel<D><<<(g_grid_cap > 0 && g_grid_cap < num_sms()) ? g_grid_cap : num_sms(), kMixedThreads, smem, stream>>>(PA, TA, tm_q, tm_qd, tm_k, tm_v);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        ++*launches;
+    } else if (g_mode == 0) {
+        // A3 + A4 in one persistent launch: the product path
+        const size_t smem = MixedWsCfg<D>::SMEM;
+        static bool attr_w = false;
+        if (!attr_w) {
+            e = cudaFuncSetAttribute(mixed_ws_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            attr_w = true;
+        }
+        mixed_ws_kernel<D><<<(g_grid_cap > 0 && g_grid_cap < num_sms()) ? g_grid_cap : num_sms(), kMixedThreads, smem, stream>>>(
+            PA, A, tm_q, tm_k, tm_v);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         ++*launches;

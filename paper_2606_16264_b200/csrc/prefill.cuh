@@ -325,69 +325,65 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
         const PrefillItem it = load_item(A, id);
         const int t = it.qt * kQTile + r;
         const int limit = it.c + min(t, it.ql - 1);  // last visible key of this row (rows past the chunk mirror its last row)
-        float m_used = 0.f, l = 0.f;
+        float m_used = -INFINITY, l = 0.f;  // the first chunk of the item raises m_used from -inf (grow_fix)
 
         for (int kt = 0; kt < it.n_kt; ++kt) {
             const uint32_t g = kv_it + kt;
             const int st = g & 1;
             mbar_wait(&B->s_full[st], (g >> 1) & 1, 111, item_it * 100000 + kt * 1000 + it.n_kt);
             tc_fence_after();
-            // The tile is walked twice in 32-column chunks (row maximum, then exponentials) with ROLLED loops: the
-            // second TMEM read is cheap, and the loop body stays ~150 instructions -- the fully unrolled 128-column
-            // version (~630 instructions per tile) thrashed the instruction cache that the four roles of an SM
-            // sub-partition share (55 % of this warp's samples were no-instruction stalls, profiles/r1c_c5.md).
+            // ONE pass over the tile in 32-column chunks, the TMEM load of the next chunk in flight while the current
+            // one is exponentiated (two register buffers).  P = exp2(s*scale - m_used) is written with the running
+            // maximum m_used of the PREVIOUS chunks; a chunk whose maximum exceeds m_used by more than 2^8 (rare after
+            // the first chunk of an item) takes grow_fix(): raise m_used, rescale O, l and the P chunks already written.
+            // Code size matters: the roles of an SM share a 32 KiB instruction cache (profiles/r1c_c5.md).
             const uint32_t s_col = tm + C::TM_S + st * 128;
             const int n_vis = limit - kt * kKvTile + 1;  // visible columns of this tile for this row
             const bool masked = __any_sync(0xffffffffu, n_vis < kKvTile);
-            float mx = -INFINITY;
+            float sum0 = 0.f, sum1 = 0.f;
+
+            auto grow_fix = [&](int c4, float cm) {  // cold path
+                const float m_new = fmaxf(m_used, cm * scale);
+                const float alpha = m_new == -INFINITY ? 1.f : fast_exp2(m_used - m_new);  // rows that do not grow: 1; first chunk of an item: 0
+                if (kt > 0) {
+                    mbar_wait(&B->pv_done, (g - 1) & 1, 112, item_it * 100000 + kt * 1000 + it.n_kt);  // O holds PV(g-1)
+                    tc_fence_after();
 #pragma unroll 1
-            for (int c4 = 0; c4 < 4; ++c4) {
-                uint32_t s[32];
-                tmem_ld_32x32(s_col + c4 * 32, s);
-                tc_wait_ld();
+                    for (int c = 0; c < D / 32; ++c) {
+                        uint32_t o[32];
+                        tmem_ld_32x32(tm + C::TM_O + c * 32, o);
+                        tc_wait_ld();
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                        tmem_st_32x32(tm + C::TM_O + c * 32, o);
+                    }
+                }
+#pragma unroll 1
+                for (int c = 0; c < c4; ++c) {  // P chunks of this tile written with the old maximum
+                    uint32_t pk[16];
+                    tmem_ld_32x32_x16(s_col + c * 16, pk);
+                    tc_wait_ld();
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) pk[j] = pack_bf16x2(bf16_lo(pk[j]) * alpha, bf16_hi(pk[j]) * alpha);
+                    tmem_st_32x32_x16(s_col + c * 16, pk);
+                }
+                l *= alpha;
+                sum0 *= alpha;
+                sum1 *= alpha;
+                m_used = m_new;
+            };
+            auto process = [&](uint32_t (&s)[32], int c4) {
                 if (masked) {
 #pragma unroll
                     for (int j = 0; j < 32; ++j)
                         if (c4 * 32 + j >= n_vis) s[j] = 0xff800000u;  // -inf, by select: the score may be NaN
                 }
+                float cm = -INFINITY;
 #pragma unroll
                 for (int j = 0; j < 32; j += 4)
-                    mx = fmaxf(mx, max4(__uint_as_float(s[j]), __uint_as_float(s[j + 1]), __uint_as_float(s[j + 2]),
+                    cm = fmaxf(cm, max4(__uint_as_float(s[j]), __uint_as_float(s[j + 1]), __uint_as_float(s[j + 2]),
                                         __uint_as_float(s[j + 3])));
-            }
-            const float m_new = mx * scale;
-            if (kt == 0) {
-                m_used = m_new;  // finite: key 0 is visible to every row
-            } else {
-                const bool grow = m_new > m_used + 8.f;  // lazy rescale: P stays <= 2^8
-                if (__any_sync(0xffffffffu, grow)) {
-                    const float alpha = grow ? fast_exp2(m_used - m_new) : 1.f;
-                    mbar_wait(&B->pv_done, (g - 1) & 1, 112, item_it * 100000 + kt * 1000 + it.n_kt);  // O holds PV(g-1)
-                    tc_fence_after();
-#pragma unroll 1
-                    for (int c4 = 0; c4 < D / 32; ++c4) {
-                        uint32_t o[32];
-                        tmem_ld_32x32(tm + C::TM_O + c4 * 32, o);
-                        tc_wait_ld();
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
-                        tmem_st_32x32(tm + C::TM_O + c4 * 32, o);
-                    }
-                    l *= alpha;
-                    if (grow) m_used = m_new;
-                }
-            }
-            float sum0 = 0.f, sum1 = 0.f;
-#pragma unroll 1
-            for (int c4 = 0; c4 < 4; ++c4) {
-                uint32_t s[32];
-                tmem_ld_32x32(s_col + c4 * 32, s);
-                tc_wait_ld();
-                if (masked) {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j)
-                        if (c4 * 32 + j >= n_vis) s[j] = 0xff800000u;
-                }
+                if (__any_sync(0xffffffffu, cm * scale > m_used + 8.f)) grow_fix(c4, cm);  // lazy: P stays <= 2^8
                 uint32_t pk[16];
 #pragma unroll
                 for (int j = 0; j < 32; j += 2) {
@@ -397,8 +393,22 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
                     sum1 += p1;
                     pk[j >> 1] = pack_bf16x2(p0, p1);
                 }
-                // P columns [16 c4, 16 c4 + 16) overwrite S columns this thread has already read in this pass
+                // P columns [16 c4, 16 c4 + 16) overwrite S columns this thread has already loaded
                 tmem_st_32x32_x16(s_col + c4 * 16, pk);
+            };
+            {
+                uint32_t sa[32], sb[32];
+                tmem_ld_32x32(s_col, sa);
+                tc_wait_ld();
+#pragma unroll 1
+                for (int h = 0; h < 2; ++h) {
+                    tmem_ld_32x32(s_col + (2 * h + 1) * 32, sb);
+                    process(sa, 2 * h);
+                    tc_wait_ld();
+                    if (h == 0) tmem_ld_32x32(s_col + 64, sa);
+                    process(sb, 2 * h + 1);
+                    if (h == 0) tc_wait_ld();
+                }
             }
             l += sum0 + sum1;
             tc_wait_st();

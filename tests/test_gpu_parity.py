@@ -223,36 +223,41 @@ def test_product_path_matches_simt_cross_check():
 
 
 def test_split_launch_mode_matches_fused():
-    """The A/B timing mode (separate prefill / decode launches; decode tiles on warp-level MMAs there) computes
-    the same step: prefill rows bit-identical (same tile code), decode rows within tolerance."""
+    """The A/B timing modes compute the same step: 1 = separate prefill / decode launches of the same tile code
+    (bit-identical), 2 = decode tiles on tcgen05 pipelines (prefill rows bit-identical, decode rows within tolerance)."""
     s = _step(16, 16, 2, 128, [300, 1, 1, 1, 40], [0, 777, 4097, 15, 130])
     dev = DeviceStep(s)
     dev.step()
     a = bits(dev.out).copy()
-    tb.debug_set_mode(1)
-    try:
-        dev.out.zero_()
-        dev.attention()
-        torch.cuda.synchronize()
-        b = bits(dev.out).copy()
-    finally:
-        tb.debug_set_mode(0)
-    assert np.array_equal(a[:300], b[:300]) and np.array_equal(a[303:], b[303:])
-    fa, fb = synth.bf16_bits_to_f32(a).astype(np.float64), synth.bf16_bits_to_f32(b).astype(np.float64)
-    assert np.abs(fa - fb).max() <= 2e-2
+    for mode in (1, 2):
+        tb.debug_set_mode(mode)
+        try:
+            dev.out.zero_()
+            dev.attention()
+            torch.cuda.synchronize()
+            b = bits(dev.out).copy()
+        finally:
+            tb.debug_set_mode(0)
+        if mode == 1:
+            assert np.array_equal(a, b)
+        assert np.array_equal(a[:300], b[:300]) and np.array_equal(a[303:], b[303:])
+        fa, fb = synth.bf16_bits_to_f32(a).astype(np.float64), synth.bf16_bits_to_f32(b).astype(np.float64)
+        assert np.abs(fa - fb).max() <= 2e-2
 
 
 # ------------------------------------------------------------------ queue sequencing: many tiles per CTA
+@pytest.mark.parametrize("mode", [0, 2])
 @pytest.mark.parametrize("split", [0, 16, 24, 64])
 @pytest.mark.parametrize("grid", [1, 2, 5])
 @pytest.mark.parametrize("shape", [(8, 1, 128), (16, 2, 128), (4, 4, 64)])
-def test_few_ctas_many_tiles_per_queue(grid, shape, split):
+def test_few_ctas_many_tiles_per_queue(grid, shape, split, mode):
     """With the step kernel capped to a few CTAs every role walks long sequences of prefill items and decode
     units (ring wrap-around, mailbox and barrier phases, TMEM slot reuse, both decode pipelines of a CTA)."""
     Hq, Hkv, d = shape
     qs = [300, 1, 1, 1, 1, 40, 1, 1, 1, 1, 1, 1]
     cs = [0, 777, 4097, 15, 130, 100, 2000, 128, 127, 1, 513, 3000]
     s = _step(20 + grid, Hq, Hkv, d, qs, cs)
+    tb.debug_set_mode(mode)  # 0 = product kernel; 2 = the tcgen05-decode variant kept for A/B timing
     tb.debug_set_grid(grid)
     tb.debug_set_split_pages(split)  # 0 = automatic (one 128-key block per unit at these sizes); else multi-block units
     try:
@@ -261,6 +266,7 @@ def test_few_ctas_many_tiles_per_queue(grid, shape, split):
         s2 = _step(30 + grid, Hq, Hkv, d, [1] * 9, [5000, 3000, 17, 900, 256, 255, 4096, 64, 2500])
         _check_step(s2)
     finally:
+        tb.debug_set_mode(0)
         tb.debug_set_grid(0)
         tb.debug_set_split_pages(0)
 
