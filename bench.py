@@ -149,7 +149,7 @@ def run_ours(args, rank, world):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl")
-    tb.debug_set_mode({"fused": 0, "split": 1, "tc": 2}[args.mode])
+    tb.debug_set_mode({"fused": 0, "split": 1}[args.mode])
     s, gen_s = make_workload(args.config, rank)
     cnt = step_counts((s.num_q_heads, s.num_kv_heads, s.head_dim, s.page_size, s.q_lens, s.ctx_lens))
     peaks = load_peaks()
@@ -300,10 +300,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", default="C5", choices=synth.CONFIG_NAMES)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="fused", choices=["fused", "split", "tc"],
+    ap.add_argument("--mode", default="fused", choices=["fused", "split"],
                     help="fused = the product path (one persistent step kernel); split = separate prefill/decode "
-                         "launches of the same tile code; tc = fused with the decode tiles on tcgen05 pipelines "
-                         "(split, tc: A/B timing only)")
+                         "launches of the same tile code, for A/B timing only")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))

@@ -163,9 +163,8 @@ int tropical_debug_attention_simt(const tropical_kv_pool_t *pool, const tropical
                                   void *cuda_stream);
 
 /* Test / measurement hook: 0 (default) = the fused step kernel, prefill tiles and decode tiles in one
- * persistent launch; 1 = the same tile code as separate prefill and decode launches; 2 = the
- * fused kernel with the decode tiles on tcgen05 pipelines (csrc/decode_tc.cuh) instead of warp workers.  1 and 2
- * exist to time design alternatives (A/B evidence under profiles/).  Process-global. */
+ * persistent launch; 1 = the same tile code as separate prefill and decode launches, kept
+ * only to time the two phases apart (A/B evidence under profiles/).  Process-global. */
 void tropical_debug_set_mode(int mode);
 
 /* Test hook: cap the number of CTAs of the persistent step kernel (0 = one per SM, the default), so that small

@@ -90,8 +90,7 @@ def version() -> str:
 
 
 def debug_set_mode(mode: int) -> None:
-    """0 = fused step kernel (default, the product path); 1 = separate prefill / decode launches; 2 = fused with
-    tcgen05 decode pipelines (1, 2: timing A/B)."""
+    """0 = fused step kernel (default, the product path); 1 = separate prefill / decode launches (timing A/B)."""
     lib().tropical_debug_set_mode(ctypes.c_int(int(mode)))
 
 

@@ -265,7 +265,7 @@ int tropical_debug_read_profile(const void* workspace, uint64_t* out_ns, void* c
     return TROPICAL_OK;
 }
 
-void tropical_debug_set_mode(int mode) { set_debug_mode(mode >= 0 && mode <= 2 ? mode : 0); }
+void tropical_debug_set_mode(int mode) { set_debug_mode(mode == 1 ? 1 : 0); }
 
 void tropical_debug_set_grid(int num_ctas) { set_debug_grid(num_ctas); }
 

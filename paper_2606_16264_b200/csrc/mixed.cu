@@ -4,7 +4,6 @@
 
 #include "common.cuh"
 #include "decode.cuh"
-#include "decode_tc.cuh"
 #include "kernels.h"
 #include "plan.cuh"
 #include "prefill.cuh"
@@ -59,7 +58,7 @@ decode_kernel(DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __gr
 }
 
 
-constexpr int kPrefillThreads = 224;  // warps 0-3 softmax, warp 4 K producer, warp 5 MMA issuer, warp 6 V producer
+constexpr int kPrefillThreads = 224;  // warps 0-3 softmax, 4 K producer, 5 MMA issuer, 6 V producer
 
 template <int D>
 __global__ void __launch_bounds__(kPrefillThreads, 1)
@@ -69,7 +68,7 @@ prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __
     extern __shared__ uint8_t smem_raw[];
     uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     PrefillBars* B = reinterpret_cast<PrefillBars*>(tiles + C::SMEM_TILES);
-    const int warp = threadIdx.x >> 5;
+    const int warp = uni((int)(threadIdx.x >> 5));
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -85,165 +84,54 @@ prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __
     __syncthreads();
     tc_fence_after();
     if (warp < 4) prefill_softmax<D>(A, B, warp);
-    else if (warp == 4) prefill_producer<D>(A, B, tiles, &tm_q, &tm_k);
+    else if (warp == 4) prefill_producer<D, 0>(A, B, tiles, &tm_q, &tm_k);
     else if (warp == 5) prefill_mma<D>(A, B, tiles);
-    else prefill_producer_v<D>(A, B, tiles, &tm_v);
+    else prefill_producer<D, 1>(A, B, tiles, &tm_q, &tm_v);
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(B->tmem_base, C::TM_COLS);
 }
 
 // ------------------------------------------------------------------------------------------------
-// The fused step kernel: ONE persistent launch, one CTA per SM, four warpgroups (512 threads, the whole
-// register file re-divided between the roles with setmaxnreg).  Two tcgen05 pipelines run side by side on
-// every SM, each fed by its own ticket queue:
-//   WG0 (warps 0-3)   : prefill softmax / correction / epilogue                           (224 regs)
-//   WG2 (warps 8-10)  : prefill K producer (TMA), prefill MMA issuer, prefill V producer   (48 regs)
-//   WG1 (warps 4-7)   : decode softmax warpgroup (thread = key)                            (80 regs)
-//   WG3 (warps 12-13) : decode producer (TMA), decode MMA issuer                           (48 regs)
-// so the tensor pipe (prefill tiles) and the HBM stream (decode blocks) are busy together for the whole step.
-// When the prefill queue is empty, WG0 and warps 8-9 turn into a SECOND decode pipeline whose ring is the
-// (now idle) prefill tile memory: decode-heavy steps then have 192 KiB of K/V in flight per SM.
+// The fused step kernel: ONE persistent launch, one CTA per SM, 16 warps, every role compiled for <= 128 registers.
+//   warps 0-3       : prefill softmax warpgroup (both query tiles of a two-tile item, alternately)
+//   warps 8, 9, 10  : prefill K producer (TMA; pops the item tickets), tcgen05 MMA issuer, V producer
+//   warps 4-7, 11-14: decode warp workers, a private TMA ring each (HBM streaming; csrc/decode.cuh)
+// Prefill items and decode units are popped from two ticket counters, so on every SM the tensor pipe (prefill) and
+// the HBM stream (decode) are busy at the same time -- the paper's multiplexing at SM granularity.  When the prefill
+// queue is empty the four softmax warps become decode workers too, with rings carved out of the (now idle) prefill
+// tile memory: a decode-heavy step then streams with 12 workers and ~220 KiB of K/V in flight per SM.
 constexpr int kMixedThreads = 512;
 
 template <int D>
 struct MixedCfg {
-    using DC = DecTcCfg<D>;
-    static constexpr int DEC_UNITS = 5;                                     // 16 KiB ring units of the decode pipeline
-    static constexpr int DEC_RING = DEC_UNITS * DC::UNIT_BYTES;
-    static constexpr int DEC_AUX = 2 * DC::QT_BYTES + 2 * DC::PT_BYTES;     // double-buffered Q^T and P^T tiles
-    static constexpr int LATE_UNITS = (PrefillCfg<D>::SMEM_TILES - DEC_AUX) / DC::UNIT_BYTES;  // second pipe, after prefill
+    static constexpr int DEC_WARPS = 8;
+    static constexpr int DEC_RING = 12288;                                  // bytes of TMA ring per dedicated decode warp
+    static constexpr int DEC_STAGES = DEC_RING / DecodeCfg<D>::PAGE_BYTES;
+    static constexpr int LATE_WARPS = 4;                                    // the softmax warps, once the prefill queue is empty
+    static constexpr int LATE_RING = PrefillCfg<D>::SMEM_TILES / LATE_WARPS / 1024 * 1024;
+    static constexpr int LATE_STAGES = LATE_RING / DecodeCfg<D>::PAGE_BYTES;
+    static constexpr int N_DEC_BARS = DEC_WARPS * DEC_STAGES + LATE_WARPS * LATE_STAGES;
     static constexpr int BAR_BYTES = 2048;
-    // d = 64: the V^T operand is padded to M = 128 by pointing its second half one ring unit further (rows 64-127
-    // of O^T are never read); keep that read inside the allocation for the last ring unit as well
-    static constexpr int TAIL_PAD = (D == 64) ? 4096 : 0;
-    static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_RING + DEC_AUX + BAR_BYTES + TAIL_PAD + 1024;
-    static constexpr uint32_t TM_DEC = 384;                                 // decode TMEM columns 384..447 (prefill: 0..383)
-    static_assert(LATE_UNITS <= kDecMaxUnits && DEC_UNITS <= kDecMaxUnits, "ring barriers");
-    static_assert(sizeof(PrefillBars) + 2 * sizeof(DecBars) <= BAR_BYTES, "barrier block");
+    static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_WARPS * DEC_RING + BAR_BYTES + 1024;
+    static_assert(DEC_STAGES <= kMaxDecodeStages && LATE_STAGES <= kMaxDecodeStages, "stage barriers");
+    static_assert(LATE_RING % 1024 == 0 && DEC_RING % 1024 == 0, "ring alignment");
+    static_assert(sizeof(PrefillBars) + N_DEC_BARS * 8 <= BAR_BYTES, "barrier block");
     static_assert(SMEM <= 232448, "shared memory per CTA");
 };
 
 template <int D>
 __global__ void __launch_bounds__(kMixedThreads, 1)
-mixed_kernel(PrefillArgs PA, DecTcArgs DA, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_qd,
+mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap tm_q,
              const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
     using C = PrefillCfg<D>;
     using M = MixedCfg<D>;
-    using DC = DecTcCfg<D>;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint8_t* dring = tiles + C::SMEM_TILES;
-    uint8_t* daux = dring + M::DEC_RING;
-    PrefillBars* PB = reinterpret_cast<PrefillBars*>(daux + M::DEC_AUX);
-    DecBars* DB = reinterpret_cast<DecBars*>(PB + 1);
-    const int warp = uni((int)(threadIdx.x >> 5)), wg = warp >> 2;
-    if (threadIdx.x == 0) {
-        tma_prefetch_desc(&tm_q);
-        tma_prefetch_desc(&tm_qd);
-        tma_prefetch_desc(&tm_k);
-        tma_prefetch_desc(&tm_v);
-        prefill_init_bars(PB);
-        dec_init_bars(DB);
-        dec_init_bars(DB + 1);
-        fence_mbar_init();
-        prof_mark(PA.hdr, 0, true);
-    }
-    if (warp == 0) {
-        tmem_alloc(&PB->tmem_base, C::TM_COLS);
-        tmem_relinquish();
-    }
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem = PB->tmem_base;
-    DecPipe P1;  // the dedicated decode pipeline
-    P1.ring = dring;
-    P1.nunits = M::DEC_UNITS;
-    P1.qt = daux;
-    P1.pt = daux + 2 * DC::QT_BYTES;
-    P1.B = DB;
-    P1.tm = tmem + M::TM_DEC;
-    P1.bar_id = 1;
-    DecPipe P2;  // the late pipeline: prefill tile memory and TMEM columns, once the prefill queue is empty
-    P2.ring = tiles;
-    P2.nunits = M::LATE_UNITS;
-    P2.qt = tiles + M::LATE_UNITS * DC::UNIT_BYTES;
-    P2.pt = P2.qt + 2 * DC::QT_BYTES;
-    P2.B = DB + 1;
-    P2.tm = tmem;
-    P2.bar_id = 2;
-
-    if (wg == 0) {
-        const long long t0 = prof_begin();
-        prefill_softmax<D>(PA, PB, warp);
-        prof_end(120, t0);
-        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 1, false);
-        // Every prefill MMA has completed (the last epilogue read its O), so every TMA load into the tile
-        // memory has been consumed: hand the memory to the late decode pipeline.
-        named_bar_sync(3, 224);
-        dec_softmax<D>(DA, P2, warp);
-        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
-    } else if (wg == 1) {
-        const long long t0 = prof_begin();
-        dec_softmax<D>(DA, P1, warp - 4);
-        prof_end(320, t0);
-        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
-    } else if (wg == 2) {
-        if (warp == 8) {
-            prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k);
-            named_bar_sync(3, 224);
-            dec_producer<D, 0>(DA, P2, &tm_qd, &tm_k);
-        } else if (warp == 9) {
-            prefill_mma<D>(PA, PB, tiles);
-            named_bar_sync(3, 224);
-            dec_mma<D>(DA, P2);
-        } else if (warp == 10) {
-            prefill_producer_v<D>(PA, PB, tiles, &tm_v);
-            named_bar_sync(3, 224);
-            dec_producer<D, 1>(DA, P2, &tm_qd, &tm_v);
-        }
-    } else {
-        const long long t0 = prof_begin();
-        if (warp == 12) { dec_producer<D, 0>(DA, P1, &tm_qd, &tm_k); prof_end(300, t0); }
-        else if (warp == 13) { dec_mma<D>(DA, P1); prof_end(310, t0); }
-        else if (warp == 14) dec_producer<D, 1>(DA, P1, &tm_qd, &tm_v);
-    }
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem, C::TM_COLS);
-}
-
-// ------------------------------------------------------------------------------------------------
-// Variant "ws" of the step kernel (debug mode 2, A/B evidence): the same prefill roles, but the decode tiles run
-// on 8 independent warp workers (warp-level mma.sync tiles of decode.cuh, a private 12 KiB TMA ring each) instead
-// of the tcgen05 decode pipelines.
-template <int D>
-struct MixedWsCfg {
-    static constexpr int DEC_WARPS = 8;
-    static constexpr int DEC_RING = 12288;
-    static constexpr int DEC_STAGES = DEC_RING / DecodeCfg<D>::PAGE_BYTES;
-    static constexpr int LATE_RING = PrefillCfg<D>::SMEM_TILES / 4;
-    static constexpr int LATE_STAGES = LATE_RING / DecodeCfg<D>::PAGE_BYTES;
-    static constexpr int N_DEC_BARS = DEC_WARPS * DEC_STAGES + 4 * LATE_STAGES;
-    static constexpr int BAR_BYTES = 2048;
-    static constexpr int SMEM = PrefillCfg<D>::SMEM_TILES + DEC_WARPS * DEC_RING + BAR_BYTES + 1024;
-    static_assert(DEC_STAGES <= kMaxDecodeStages && LATE_STAGES <= kMaxDecodeStages, "stage barriers");
-    static_assert(sizeof(PrefillBars) + N_DEC_BARS * 8 <= BAR_BYTES, "barrier block");
-};
-
-template <int D>
-__global__ void __launch_bounds__(kMixedThreads, 1)
-mixed_ws_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap tm_q,
-                const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
-    using C = PrefillCfg<D>;
-    using M = MixedWsCfg<D>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* rings = tiles + C::SMEM_TILES;
     PrefillBars* PB = reinterpret_cast<PrefillBars*>(rings + M::DEC_WARPS * M::DEC_RING);
     uint64_t* dec_full = reinterpret_cast<uint64_t*>(PB + 1);
-    const int warp = uni((int)(threadIdx.x >> 5)), wg = warp >> 2;
+    const int warp = uni((int)(threadIdx.x >> 5));
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -260,19 +148,24 @@ mixed_ws_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorM
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    if (wg == 0) {
+    if (warp < 4) {
         prefill_softmax<D>(PA, PB, warp);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 1, false);
+        // The terminating ticket was seen after the last item's final epilogue: every prefill MMA has completed, so
+        // every TMA load into the tile memory has been consumed and the producers issue nothing more.
+        named_bar_sync(1, 128);
         DecodeRing R = make_ring(tiles + warp * M::LATE_RING, dec_full + M::DEC_WARPS * M::DEC_STAGES + warp * M::LATE_STAGES,
                                  M::LATE_STAGES);
         decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
-    } else if (wg == 2) {
-        if (warp == 8) prefill_producer<D>(PA, PB, tiles, &tm_q, &tm_k);
-        else if (warp == 9) prefill_mma<D>(PA, PB, tiles);
-        else if (warp == 10) prefill_producer_v<D>(PA, PB, tiles, &tm_v);
-    } else {
-        const int dw = (wg == 1) ? warp - 4 : warp - 8;
+    } else if (warp == 8) {
+        prefill_producer<D, 0>(PA, PB, tiles, &tm_q, &tm_k);
+    } else if (warp == 9) {
+        prefill_mma<D>(PA, PB, tiles);
+    } else if (warp == 10) {
+        prefill_producer<D, 1>(PA, PB, tiles, &tm_q, &tm_v);
+    } else if (warp != 15) {
+        const int dw = warp < 8 ? warp - 4 : warp - 7;
         DecodeRing R = make_ring(rings + dw * M::DEC_RING, dec_full + dw * M::DEC_STAGES, M::DEC_STAGES);
         decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
@@ -307,7 +200,7 @@ size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q) 
 
 size_t profile_offset_bytes() { return make_layout(1, 1, 64, 1, 1).hdr + HDR_PROF * sizeof(int); }
 
-static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches; 2: fused, tcgen05 decode pipelines (1, 2: A/B timing only)
+static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches (A/B timing only)
 void set_debug_mode(int mode) { g_mode = mode; }
 static int g_grid_cap = 0;  // test hook: 0 = one CTA per SM
 int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset) {
@@ -346,11 +239,10 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     if (e != cudaSuccess) return e;
     ++*launches;
 
-    CUtensorMap tm_q, tm_qd, tm_k, tm_v;
+    CUtensorMap tm_q, tm_k, tm_v;
     const long long rows = (long long)pool.num_pages * pool.Hkv * kPageSize;
     if (!encode_pool_map(&tm_k, pool.k_pool, rows, D) || !encode_pool_map(&tm_v, pool.v_pool, rows, D) ||
-        !encode_q_map(&tm_q, q, b.total_q, pool.Hq, D, 1, kQTile) ||
-        !encode_q_map(&tm_qd, q, b.total_q, pool.Hq, D, kHeadBlock, 1))
+        !encode_q_map(&tm_q, q, b.total_q, pool.Hq, D, 1, kQTile))
         return cudaErrorInvalidValue;
 
     PrefillArgs PA;
@@ -377,21 +269,8 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     A.part_ml = (float2*)(ws + w.part_ml);
     A.part_o = (float*)(ws + w.part_o);
 
-    DecTcArgs TA;
-    TA.pool = pool;
-    TA.b = b;
-    TA.out = (uint16_t*)out;
-    TA.lse = lse;
-    TA.scale_log2 = scale_log2;
-    TA.hdr = P.hdr;
-    TA.ticket = P.hdr + HDR_TICKET_DECODE;
-    TA.req_info = P.req_info;
-    TA.units = P.units;
-    TA.part_ml = A.part_ml;
-    TA.part_o = A.part_o;
-
-    if (g_mode == 2) {
-        // A3 + A4 in one persistent launch, decode tiles on the tcgen05 pipelines (A/B variant)
+    if (g_mode == 0) {
+        // A3 + A4 in one persistent launch: the product path
         const size_t smem = MixedCfg<D>::SMEM;
         static bool attr_m = false;
         if (!attr_m) {
@@ -399,20 +278,7 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
             if (e != cudaSuccess) return e;
             attr_m = true;
         }
-        mixed_kernel<D><<<(g_grid_cap > 0 && g_grid_cap < num_sms()) ? g_grid_cap : num_sms(), kMixedThreads, smem, stream>>>(PA, TA, tm_q, tm_qd, tm_k, tm_v);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        ++*launches;
-    } else if (g_mode == 0) {
-        // A3 + A4 in one persistent launch: the product path
-        const size_t smem = MixedWsCfg<D>::SMEM;
-        static bool attr_w = false;
-        if (!attr_w) {
-            e = cudaFuncSetAttribute(mixed_ws_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            attr_w = true;
-        }
-        mixed_ws_kernel<D><<<(g_grid_cap > 0 && g_grid_cap < num_sms()) ? g_grid_cap : num_sms(), kMixedThreads, smem, stream>>>(
+        mixed_kernel<D><<<(g_grid_cap > 0 && g_grid_cap < num_sms()) ? g_grid_cap : num_sms(), kMixedThreads, smem, stream>>>(
             PA, A, tm_q, tm_k, tm_v);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -45,7 +45,7 @@ __host__ __device__ inline WorkspaceLayout make_layout(int Hq, int Hkv, int D, i
 struct PlanPtrs {
     int* hdr;
     int4* req_info;
-    int2* items;   // {req, (qtile << 16) | head}
+    int2* items;   // {req, (qtile << 16) | (pair << 15) | head}: pair = the item also carries head + 1 (same kv group)
     int4* units;   // {req, kvh | (hb << 16), page_start, page_count}
 };
 
@@ -71,6 +71,10 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     const int g = Hq / Hkv;
     const int HB = (g + kHeadBlock - 1) / kHeadBlock;
     const int n = b.num_reqs;
+    // prefill items per 128-row query tile: under GQA with an even group, two heads of a kv group share one item
+    // (and its K/V tiles in shared memory); otherwise one head per item
+    const int pair = (g % 2 == 0) ? 1 : 0;
+    const int ipt = pair ? Hq / 2 : Hq;
     const int chunk = (n + kPlanThreads - 1) / kPlanThreads;
     const int i0 = tid * chunk, i1 = min(n, i0 + chunk);
 
@@ -94,7 +98,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
             const int pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
             my_units += ((pages + split - 1) / split) * Hkv * HB;
         } else if (q > 1) {
-            my_items += ((q + kQTile - 1) / kQTile) * Hq;
+            my_items += ((q + kQTile - 1) / kQTile) * ipt;
         }
     }
     s_units[tid] = my_units;
@@ -120,7 +124,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
             ubase += info.z * Hkv * HB;
         } else if (q > 1) {
             info.x = 2;
-            ibase += ((q + kQTile - 1) / kQTile) * Hq;
+            ibase += ((q + kQTile - 1) / kQTile) * ipt;
         }
         P.req_info[i] = info;
     }
@@ -152,8 +156,8 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         const int4 info = P.req_info[i];
         const int local = e - info.w;
         const int ntile = (b.q_lens[i] + kQTile - 1) / kQTile;
-        const int qt = ntile - 1 - local / Hq;  // heaviest (most KV tiles) first
-        P.items[e] = make_int2(i, (qt << 16) | (local % Hq));
+        const int qt = ntile - 1 - local / ipt;  // heaviest (most KV tiles) first
+        P.items[e] = make_int2(i, (qt << 16) | (pair << 15) | ((local % ipt) << pair));
     }
 }
 

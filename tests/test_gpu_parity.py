@@ -223,13 +223,12 @@ def test_product_path_matches_simt_cross_check():
 
 
 def test_split_launch_mode_matches_fused():
-    """The A/B timing modes compute the same step: 1 = separate prefill / decode launches of the same tile code
-    (bit-identical), 2 = decode tiles on tcgen05 pipelines (prefill rows bit-identical, decode rows within tolerance)."""
+    """The A/B timing mode (separate prefill / decode launches) runs the same tile code: same bits."""
     s = _step(16, 16, 2, 128, [300, 1, 1, 1, 40], [0, 777, 4097, 15, 130])
     dev = DeviceStep(s)
     dev.step()
     a = bits(dev.out).copy()
-    for mode in (1, 2):
+    for mode in (1,):
         tb.debug_set_mode(mode)
         try:
             dev.out.zero_()
@@ -246,7 +245,7 @@ def test_split_launch_mode_matches_fused():
 
 
 # ------------------------------------------------------------------ queue sequencing: many tiles per CTA
-@pytest.mark.parametrize("mode", [0, 2])
+@pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("split", [0, 16, 24, 64])
 @pytest.mark.parametrize("grid", [1, 2, 5])
 @pytest.mark.parametrize("shape", [(8, 1, 128), (16, 2, 128), (4, 4, 64)])
@@ -257,7 +256,7 @@ def test_few_ctas_many_tiles_per_queue(grid, shape, split, mode):
     qs = [300, 1, 1, 1, 1, 40, 1, 1, 1, 1, 1, 1]
     cs = [0, 777, 4097, 15, 130, 100, 2000, 128, 127, 1, 513, 3000]
     s = _step(20 + grid, Hq, Hkv, d, qs, cs)
-    tb.debug_set_mode(mode)  # 0 = product kernel; 2 = the tcgen05-decode variant kept for A/B timing
+    tb.debug_set_mode(mode)  # 0 = product kernel; 1 = separate prefill / decode launches (grid cap applies to 0 only)
     tb.debug_set_grid(grid)
     tb.debug_set_split_pages(split)  # 0 = automatic (one 128-key block per unit at these sizes); else multi-block units
     try:
