@@ -70,7 +70,9 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
     const int row = lane >> 2, cq = (lane & 3) * 2;
     const int g = A.pool.Hq / A.pool.Hkv;
     const int n_units = A.hdr[HDR_N_UNITS];
-    const uint32_t ring_s = smem_u32(R.base);
+    const uint32_t ring_s = uni(smem_u32(R.base));
+    const uint32_t full_s = uni(smem_u32(R.full));
+    const int Hkv = uni(A.pool.Hkv);
     // ldmatrix lane addressing (row within 8x8 matrix r8, matrix id mi)
     const int mi = lane >> 3, r8 = lane & 7;
     const int k_key = (mi & 1) * 8 + r8, k_chunk_off = mi >> 1;  // K as A: (keys lo/hi) x (chunk, chunk+1)
@@ -88,6 +90,7 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
         if (u >= n_units) break;
         const int4 un = A.units[u];
         const int req = un.x, kvh = un.y & 0xffff, hb = un.y >> 16, p0 = un.z, np = un.w;
+        const int kvh_u = uni(kvh);
         const int L = __ldg(A.b.ctx_lens + req) + 1;
         const int tok = __ldg(A.b.q_offsets + req);
         const int h0 = kvh * g + hb * kHeadBlock;
@@ -113,19 +116,24 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
         // ---- stage issue: sub-stage j = K (j even) or V (j odd) of page j >> 1
         const int n_sub = 2 * np;
         int issued = 0, ptv = 0;
-        auto issue_one = [&]() {  // whole warp calls; lane 0 issues the boxes of sub-stage `issued`
+        auto issue_one = [&]() {  // whole warp calls; one elected lane issues the boxes of sub-stage `issued`
             const int pi = issued >> 1;
             if ((issued & 63) == 0) ptv = (pi + lane < np) ? __ldg(pt + pi + lane) : 0;
-            const int page = __shfl_sync(0xffffffffu, ptv, pi & 31);
-            if (lane == 0) {
-                uint8_t* dst = R.base + R.i_slot * C::PAGE_BYTES;
-                uint64_t* bar = R.full + R.i_slot;
-                const int r0 = (page * A.pool.Hkv + kvh) * kPageSize;
-                const CUtensorMap* tm = (issued & 1) ? tm_v : tm_k;
-                mbar_arrive_expect_tx(bar, C::PAGE_BYTES);
+            const int page = __shfl_sync(0xffffffffu, ptv, pi & 31);  // warp-uniform: no waterfall around UTMALDG
+            const uint32_t dst = ring_s + R.i_slot * C::PAGE_BYTES;
+            const uint32_t bar = full_s + R.i_slot * 8;
+            const int r0 = (page * Hkv + kvh_u) * kPageSize;
+            const CUtensorMap* tm = (issued & 1) ? tm_v : tm_k;
+            if (elect_one()) {
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((uint32_t)C::PAGE_BYTES) : "memory");
 #pragma unroll
-                for (int cb = 0; cb < C::CB; ++cb) tma_load_2d(dst + cb * C::HALF_BYTES, tm, cb * 64, r0, bar);
+                for (int cb = 0; cb < C::CB; ++cb)
+                    asm volatile(
+                        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                        ::"r"(dst + cb * C::HALF_BYTES), "l"(tm), "r"(bar), "r"(cb * 64), "r"(r0)
+                        : "memory");
             }
+            __syncwarp();
             R.i_slot = (R.i_slot + 1 == R.nst) ? 0 : R.i_slot + 1;
             ++issued;
         };
@@ -279,19 +287,29 @@ __device__ __forceinline__ void combine_row(const CombineArgs& A, int req, int h
     const int nsplit = info.z;
     const size_t u0 = (size_t)info.y + ((size_t)kvh * nsplit) * HB + hb;
     float M = -INFINITY;
+#pragma unroll 4
     for (int s = 0; s < nsplit; ++s) M = fmaxf(M, A.part_ml[(u0 + (size_t)s * HB) * kHeadBlock + r].x);
     constexpr int EPL = D / 32;
     float acc[EPL], l = 0.f;
 #pragma unroll
     for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+#pragma unroll 4
     for (int s = 0; s < nsplit; ++s) {
         const size_t u = u0 + (size_t)s * HB;
         const float2 ml = A.part_ml[u * kHeadBlock + r];
         const float w = exp2f(ml.x - M);
         l += ml.y * w;
         const float* po = A.part_o + (u * kHeadBlock + r) * D + lane * EPL;
+        if (EPL == 4) {
+            const float4 v = *reinterpret_cast<const float4*>(po);
+            acc[0] = fmaf(v.x, w, acc[0]);
+            acc[1] = fmaf(v.y, w, acc[1]);
+            acc[2] = fmaf(v.z, w, acc[2]);
+            acc[3] = fmaf(v.w, w, acc[3]);
+        } else {
 #pragma unroll
-        for (int e = 0; e < EPL; ++e) acc[e] = fmaf(po[e], w, acc[e]);
+            for (int e = 0; e < EPL; ++e) acc[e] = fmaf(po[e], w, acc[e]);
+        }
     }
     const float inv = 1.f / l;
     const int tok = A.b.q_offsets[req];

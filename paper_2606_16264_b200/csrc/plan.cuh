@@ -63,10 +63,12 @@ __device__ __forceinline__ int find_owner(const int4* __restrict__ info, int n, 
 }
 
 constexpr int kPlanThreads = 1024;
+constexpr int kPlanStagedReqs = 2048;  // per-request bases kept in shared memory for the ticket -> request search
 
 __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split) {
     __shared__ int s_units[kPlanThreads], s_items[kPlanThreads];
     __shared__ int s_pages;
+    __shared__ int s_ub[kPlanStagedReqs], s_ib[kPlanStagedReqs];
     const int tid = threadIdx.x;
     const int g = Hq / Hkv;
     const int HB = (g + kHeadBlock - 1) / kHeadBlock;
@@ -140,8 +142,28 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     }
     __syncthreads();  // req_info visible to the whole block (same-block global writes + barrier)
 
+    // ticket -> request: binary search over the per-request bases, staged in shared memory when they fit (the
+    // dependent global loads of the search made this kernel ~20 us for a few hundred requests)
+    const bool staged = n <= kPlanStagedReqs;
+    if (staged) {
+        for (int i = tid; i < n; i += kPlanThreads) {
+            const int4 v = P.req_info[i];
+            s_ub[i] = v.y;
+            s_ib[i] = v.w;
+        }
+        __syncthreads();
+    }
+    auto owner = [&](const int* base_s, int field, int e) {
+        if (!staged) return field == 1 ? find_owner<1>(P.req_info, n, e) : find_owner<3>(P.req_info, n, e);
+        int lo = 0, hi = n;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (base_s[mid] <= e) lo = mid; else hi = mid;
+        }
+        return lo;
+    };
     for (int e = tid; e < n_units; e += kPlanThreads) {
-        const int i = find_owner<1>(P.req_info, n, e);
+        const int i = owner(s_ub, 1, e);
         const int4 info = P.req_info[i];
         const int u = e - info.y;
         const int hb = u % HB;
@@ -152,7 +174,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         P.units[e] = make_int4(i, kvh | (hb << 16), p0, min(split, pages - p0));
     }
     for (int e = tid; e < n_items; e += kPlanThreads) {
-        const int i = find_owner<3>(P.req_info, n, e);
+        const int i = owner(s_ib, 3, e);
         const int4 info = P.req_info[i];
         const int local = e - info.w;
         const int ntile = (b.q_lens[i] + kQTile - 1) / kQTile;

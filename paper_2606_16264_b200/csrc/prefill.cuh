@@ -309,6 +309,7 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
 // ------------------------------------------------------------------------------------------------
 // softmax warpgroup (4 warps, 128 threads: thread r <-> query row r <-> TMEM lane r, for both query tiles)
 __device__ __forceinline__ float max4(float a, float b, float c, float d) { return fmaxf(fmaxf(a, b), fmaxf(c, d)); }
+constexpr int kPolyEvery = 4;  // every 4th pair of a chunk takes exp2_poly_x2 instead of MUFU.EX2
 
 template <int D>
 __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBars* B, int wg_warp) {
@@ -388,24 +389,52 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
                     for (int j = 0; j < 32; ++j)
                         if (c4 * 32 + j >= n_vis) s[j] = 0xff800000u;  // -inf, by select: the score may be NaN
                 }
+                // Exponentials with the CURRENT m_used (speculative) and the chunk maximum are independent instruction
+                // streams: no branch between them, so the FMNMX tree fills the MUFU latency.  If the maximum then
+                // turns out to exceed m_used by more than 2^8 (rare; always for the first chunk of an item, where
+                // m_used is -inf and the speculative values are inf / NaN), the chunk is redone from its registers.
+                uint32_t pk[16];
+                const uint64_t sc2 = f32x2_pack(scale, scale);
+                uint64_t nm2 = f32x2_pack(-m_used, -m_used);
+                uint64_t cs2 = f32x2_pack(0.f, 0.f);
+#pragma unroll
+                for (int j = 0; j < 32; j += 2) {
+                    float x0, x1;
+                    f32x2_unpack(f32x2_fma(f32x2_pack(__uint_as_float(s[j]), __uint_as_float(s[j + 1])), sc2, nm2), x0, x1);
+                    float p0, p1;
+                    if ((j >> 1) % kPolyEvery == kPolyEvery - 1) {  // a quarter of the exponentials on the FMA pipe
+                        exp2_poly_x2(x0, x1, p0, p1);
+                    } else {
+                        p0 = fast_exp2(x0);
+                        p1 = fast_exp2(x1);
+                    }
+                    cs2 = f32x2_add(cs2, f32x2_pack(p0, p1));
+                    pk[j >> 1] = pack_bf16x2(p0, p1);
+                }
                 float cm = -INFINITY;
 #pragma unroll
                 for (int j = 0; j < 32; j += 4)
                     cm = fmaxf(cm, max4(__uint_as_float(s[j]), __uint_as_float(s[j + 1]), __uint_as_float(s[j + 2]),
                                         __uint_as_float(s[j + 3])));
-                if (__any_sync(0xffffffffu, cm * scale > m_used + 8.f)) grow_fix(c4, cm);  // lazy: P stays <= 2^8
-                uint32_t pk[16];
-                const uint64_t sc2 = f32x2_pack(scale, scale), nm2 = f32x2_pack(-m_used, -m_used);
-                uint64_t acc2 = f32x2_pack(sum0, sum1);
+                if (__any_sync(0xffffffffu, cm * scale > m_used + 8.f)) {  // lazy: P stays <= 2^8
+                    grow_fix(c4, cm);
+                    nm2 = f32x2_pack(-m_used, -m_used);
+                    cs2 = f32x2_pack(0.f, 0.f);
 #pragma unroll
-                for (int j = 0; j < 32; j += 2) {
-                    float x0, x1;
-                    f32x2_unpack(f32x2_fma(f32x2_pack(__uint_as_float(s[j]), __uint_as_float(s[j + 1])), sc2, nm2), x0, x1);
-                    const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
-                    acc2 = f32x2_add(acc2, f32x2_pack(p0, p1));
-                    pk[j >> 1] = pack_bf16x2(p0, p1);
+                    for (int j = 0; j < 32; j += 2) {
+                        float x0, x1;
+                        f32x2_unpack(f32x2_fma(f32x2_pack(__uint_as_float(s[j]), __uint_as_float(s[j + 1])), sc2, nm2), x0, x1);
+                        const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
+                        cs2 = f32x2_add(cs2, f32x2_pack(p0, p1));
+                        pk[j >> 1] = pack_bf16x2(p0, p1);
+                    }
                 }
-                f32x2_unpack(acc2, sum0, sum1);
+                {
+                    float c0, c1;
+                    f32x2_unpack(cs2, c0, c1);
+                    sum0 += c0;
+                    sum1 += c1;
+                }
                 // P columns [16 c4, 16 c4 + 16) overwrite S columns this thread has already loaded
                 tmem_st_32x32_x16(s_col + c4 * 16, pk);
             };
