@@ -363,7 +363,7 @@ __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, bool b_mn_m
 
 // Broadcast lane 0's value: tells the compiler the result is warp-uniform, so operands of the uniform-datapath
 // instructions (UTCHMMA, UTCBAR, UTMALDG) built from it need no per-lane "waterfall" loop (ELECT / R2UR.BROADCAST /
-// BRA.U.ANY around every instruction: ~150 cycles per tcgen05.mma, measured in profiles/r1c_notes.md).
+// BRA.U.ANY around every instruction: ~150 cycles per tcgen05.mma, measured in profiles/r1c_c5.md).
 __device__ __forceinline__ uint32_t uni(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
 __device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 

@@ -63,12 +63,12 @@ __device__ __forceinline__ int find_owner(const int4* __restrict__ info, int n, 
 }
 
 constexpr int kPlanThreads = 1024;
-constexpr int kPlanStagedReqs = 2048;  // per-request bases kept in shared memory for the ticket -> request search
+constexpr int kPlanStagedReqs = 1024;  // per-request bases kept in shared memory for the ticket -> request search
 
 __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split) {
     __shared__ int s_units[kPlanThreads], s_items[kPlanThreads];
     __shared__ int s_pages;
-    __shared__ int s_ub[kPlanStagedReqs], s_ib[kPlanStagedReqs];
+    __shared__ int s_ub[kPlanStagedReqs], s_ib[kPlanStagedReqs], s_ns[kPlanStagedReqs], s_pg[kPlanStagedReqs];
     const int tid = threadIdx.x;
     const int g = Hq / Hkv;
     const int HB = (g + kHeadBlock - 1) / kHeadBlock;
@@ -150,6 +150,9 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
             const int4 v = P.req_info[i];
             s_ub[i] = v.y;
             s_ib[i] = v.w;
+            s_ns[i] = v.z;
+            // decode request: pages of its context; prefill request: its 128-row query tiles
+            s_pg[i] = v.x == 1 ? (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize : (b.q_lens[i] + kQTile - 1) / kQTile;
         }
         __syncthreads();
     }
@@ -164,20 +167,25 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     };
     for (int e = tid; e < n_units; e += kPlanThreads) {
         const int i = owner(s_ub, 1, e);
-        const int4 info = P.req_info[i];
-        const int u = e - info.y;
+        int ubase, nsplit, pages;
+        if (staged) {
+            ubase = s_ub[i]; nsplit = s_ns[i]; pages = s_pg[i];
+        } else {
+            const int4 info = P.req_info[i];
+            ubase = info.y; nsplit = info.z;
+            pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+        }
+        const int u = e - ubase;
         const int hb = u % HB;
-        const int s = (u / HB) % info.z;
-        const int kvh = u / (HB * info.z);
-        const int pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+        const int s = (u / HB) % nsplit;
+        const int kvh = u / (HB * nsplit);
         const int p0 = s * split;
         P.units[e] = make_int4(i, kvh | (hb << 16), p0, min(split, pages - p0));
     }
     for (int e = tid; e < n_items; e += kPlanThreads) {
         const int i = owner(s_ib, 3, e);
-        const int4 info = P.req_info[i];
-        const int local = e - info.w;
-        const int ntile = (b.q_lens[i] + kQTile - 1) / kQTile;
+        const int local = e - (staged ? s_ib[i] : P.req_info[i].w);
+        const int ntile = staged ? s_pg[i] : (b.q_lens[i] + kQTile - 1) / kQTile;
         const int qt = ntile - 1 - local / ipt;  // heaviest (most KV tiles) first
         P.items[e] = make_int2(i, (qt << 16) | (pair << 15) | ((local % ipt) << pair));
     }

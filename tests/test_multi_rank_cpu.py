@@ -1,0 +1,68 @@
+"""N > 1 path on CPU: two processes over gloo run the rank logic bench.py uses under torchrun -- every rank builds
+its own replica of the workload (same lengths, private page placement and values), steps it (here: through the
+CPU oracle, since there is no GPU), and the job's time is the maximum over ranks, its throughput the sum over
+replicas.  The data path has no collective: the only exchange is the timing reduction."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import bench
+        import oracle
+        s, _ = bench.make_workload("C1", rank)
+        ref, _, kp, _ = oracle.step(s)
+        fake_us = 100.0 + 25.0 * rank                      # rank 1 is the slow replica
+        job_us = bench.max_over_ranks(fake_us, world, "cpu")
+        info = dict(rank=rank, q=s.q_lens.tolist(), c=s.ctx_lens.tolist(), table=s.page_table.tolist(),
+                    checksum=float(np.abs(ref).sum()), pool_sum=int(kp.astype(np.int64).sum()), job_us=job_us,
+                    tps=bench.whole_job_tokens_per_s(s.total_q, world, job_us))
+        gathered = [None] * world
+        dist.all_gather_object(gathered, info)
+        if rank == 0:
+            out.put(gathered)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_run_private_replicas_and_time_is_max_over_ranks():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = out.get(timeout=180)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    a, b = sorted(got, key=lambda d: d["rank"])
+    assert a["q"] == b["q"] == [57, 1, 1, 1] and a["c"] == b["c"]          # same step shape on every rank (weak scaling)
+    assert a["table"] != b["table"] and a["checksum"] != b["checksum"]      # private pool placement and values
+    assert a["job_us"] == b["job_us"] == 125.0                              # the slowest rank sets the step time
+    assert a["tps"] == pytest.approx(2 * 60 / 125e-6)                        # whole-job aggregate over both replicas
+
+
+def test_single_rank_reduction_is_identity():
+    import bench
+    assert bench.max_over_ranks(3.5, 1, "cpu") == 3.5
+    assert bench.whole_job_tokens_per_s(60, 1, 100.0) == pytest.approx(6e5)
