@@ -44,6 +44,7 @@ struct DecodeArgs {
     const int4* units;
     float2* part_ml;
     float* part_o;
+    int* group_cnt;   // per split group (request, kv head, head block): units finished so far; zeroed by the plan kernel
 };
 
 // Ring state of one decode warp; persists across units so barrier parities stay consistent.
@@ -60,6 +61,53 @@ __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
     uint32_t d;
     asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
     return d;
+}
+
+// A5 (in-kernel): merge the split partials of the (up to 8) q heads of one split group, in split-index order -- the
+// result does not depend on which unit finished last.  Called by the warp whose unit completed the group; the
+// partials of the other units were published with __threadfence() before their counter increment, and are read
+// through L2 (ld.global.cg) here.
+template <int D>
+__device__ __noinline__ void combine_group(const DecodeArgs& A, size_t u_first, int HB, int nsplit, int nh, int tok, int h0,
+                                           int lane) {
+    // lane -> (head r = lane / 4, quarter k = lane % 4); the lane owns the float4s j * 4 + k (j < D / 16) of its head's
+    // row, so the 8 heads of the group are merged concurrently with D / 16 independent loads per split in flight
+    constexpr int J = D / 16;
+    const int r = lane >> 2, k = lane & 3;
+    if (r >= nh) return;
+    float M = -INFINITY;
+#pragma unroll 4
+    for (int s = 0; s < nsplit; ++s) M = fmaxf(M, __ldcg(&A.part_ml[(u_first + (size_t)s * HB) * kHeadBlock + r]).x);
+    float4 acc[J];
+    float l = 0.f;
+#pragma unroll
+    for (int j = 0; j < J; ++j) acc[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 2
+    for (int s = 0; s < nsplit; ++s) {
+        const size_t u = u_first + (size_t)s * HB;
+        const float2 ml = __ldcg(&A.part_ml[u * kHeadBlock + r]);
+        const float w = exp2f(ml.x - M);
+        l += ml.y * w;
+        const float4* po = reinterpret_cast<const float4*>(A.part_o + (u * kHeadBlock + r) * D) + k;
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            const float4 v = __ldcg(po + j * 4);
+            acc[j].x = fmaf(v.x, w, acc[j].x);
+            acc[j].y = fmaf(v.y, w, acc[j].y);
+            acc[j].z = fmaf(v.z, w, acc[j].z);
+            acc[j].w = fmaf(v.w, w, acc[j].w);
+        }
+    }
+    const float inv = 1.f / l;
+    uint2* orow = reinterpret_cast<uint2*>(A.out + ((size_t)tok * A.pool.Hq + h0 + r) * D) + k;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+        uint2 w;
+        w.x = pack_bf16x2(acc[j].x * inv, acc[j].y * inv);
+        w.y = pack_bf16x2(acc[j].z * inv, acc[j].w * inv);
+        orow[j * 4] = w;
+    }
+    if (A.lse != nullptr && k == 0) A.lse[(size_t)tok * A.pool.Hq + h0 + r] = (M + log2f(l)) * 0.6931471805599453f;
 }
 
 template <int D>
@@ -262,67 +310,21 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
                 if (cq < nh) A.part_ml[(size_t)u * kHeadBlock + cq] = make_float2(m0, l0);
                 if (cq + 1 < nh) A.part_ml[(size_t)u * kHeadBlock + cq + 1] = make_float2(m1, l1);
             }
+            // last unit of the split group to finish merges the group (A5)
+            const int HB = (g + kHeadBlock - 1) / kHeadBlock;
+            const int s_idx = ((u - A.req_info[req].y) / HB) % nsplit;
+            const size_t u_first = (size_t)u - (size_t)s_idx * HB;
+            __threadfence();
+            __syncwarp();
+            int done = 0;
+            if (lane == 0) done = atomicAdd(A.group_cnt + u_first, 1);
+            done = __shfl_sync(0xffffffffu, done, 0);
+            if (done == nsplit - 1) {
+                __threadfence();
+                combine_group<D>(A, u_first, HB, nsplit, nh, tok, h0, lane);
+            }
         }
     }
-}
-
-// A5: combine the split partials of one (decode request, q head) in fixed split order.
-struct CombineArgs {
-    PoolDesc pool;
-    BatchDesc b;
-    uint16_t* out;
-    float* lse;
-    const int4* req_info;
-    const float2* part_ml;
-    const float* part_o;
-};
-
-template <int D>
-__device__ __forceinline__ void combine_row(const CombineArgs& A, int req, int hq, int lane) {
-    const int4 info = A.req_info[req];
-    if (info.x != 1 || info.z <= 1) return;
-    const int g = A.pool.Hq / A.pool.Hkv;
-    const int HB = (g + kHeadBlock - 1) / kHeadBlock;
-    const int kvh = hq / g, hb = (hq % g) / kHeadBlock, r = (hq % g) % kHeadBlock;
-    const int nsplit = info.z;
-    const size_t u0 = (size_t)info.y + ((size_t)kvh * nsplit) * HB + hb;
-    float M = -INFINITY;
-#pragma unroll 4
-    for (int s = 0; s < nsplit; ++s) M = fmaxf(M, A.part_ml[(u0 + (size_t)s * HB) * kHeadBlock + r].x);
-    constexpr int EPL = D / 32;
-    float acc[EPL], l = 0.f;
-#pragma unroll
-    for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
-#pragma unroll 4
-    for (int s = 0; s < nsplit; ++s) {
-        const size_t u = u0 + (size_t)s * HB;
-        const float2 ml = A.part_ml[u * kHeadBlock + r];
-        const float w = exp2f(ml.x - M);
-        l += ml.y * w;
-        const float* po = A.part_o + (u * kHeadBlock + r) * D + lane * EPL;
-        if (EPL == 4) {
-            const float4 v = *reinterpret_cast<const float4*>(po);
-            acc[0] = fmaf(v.x, w, acc[0]);
-            acc[1] = fmaf(v.y, w, acc[1]);
-            acc[2] = fmaf(v.z, w, acc[2]);
-            acc[3] = fmaf(v.w, w, acc[3]);
-        } else {
-#pragma unroll
-            for (int e = 0; e < EPL; ++e) acc[e] = fmaf(po[e], w, acc[e]);
-        }
-    }
-    const float inv = 1.f / l;
-    const int tok = A.b.q_offsets[req];
-    uint16_t* orow = A.out + ((size_t)tok * A.pool.Hq + hq) * D + lane * EPL;
-    if (EPL == 4) {
-        uint2 w;
-        w.x = pack_bf16x2(acc[0] * inv, acc[1] * inv);
-        w.y = pack_bf16x2(acc[2] * inv, acc[3] * inv);
-        *reinterpret_cast<uint2*>(orow) = w;
-    } else {
-        *reinterpret_cast<uint32_t*>(orow) = pack_bf16x2(acc[0] * inv, acc[1] * inv);
-    }
-    if (A.lse != nullptr && lane == 0) A.lse[(size_t)tok * A.pool.Hq + hq] = (M + log2f(l)) * 0.6931471805599453f;
 }
 
 }  // namespace tropical

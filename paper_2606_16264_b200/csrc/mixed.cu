@@ -175,14 +175,6 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
     if (warp == 0) tmem_dealloc(PB->tmem_base, C::TM_COLS);
 }
 
-template <int D>
-__global__ void __launch_bounds__(128) combine_kernel(CombineArgs A) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long n = (long long)A.b.num_reqs * A.pool.Hq;
-    for (long long r = (long long)blockIdx.x * 4 + warp; r < n; r += (long long)gridDim.x * 4)
-        combine_row<D>(A, (int)(r / A.pool.Hq), (int)(r % A.pool.Hq), lane);
-}
-
 static int g_num_sms = 0;
 static int num_sms() {
     if (g_num_sms == 0) {
@@ -234,6 +226,7 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     P.req_info = (int4*)(ws + w.req_info);
     P.items = (int2*)(ws + w.items);
     P.units = (int4*)(ws + w.units);
+    P.group_cnt = (int*)(ws + w.group_cnt);
     plan_kernel<<<1, kPlanThreads, 0, stream>>>(b, pool.Hq, pool.Hkv, P, g_split_pages);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -268,6 +261,7 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     A.units = P.units;
     A.part_ml = (float2*)(ws + w.part_ml);
     A.part_o = (float*)(ws + w.part_o);
+    A.group_cnt = P.group_cnt;
 
     if (g_mode == 0) {
         // A3 + A4 in one persistent launch: the product path
@@ -314,23 +308,6 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
         ++*launches;
     }
 
-    CombineArgs Cb;
-    Cb.pool = pool;
-    Cb.b = b;
-    Cb.out = (uint16_t*)out;
-    Cb.lse = lse;
-    Cb.req_info = P.req_info;
-    Cb.part_ml = A.part_ml;
-    Cb.part_o = A.part_o;
-    long long rows_c = (long long)b.num_reqs * pool.Hq;
-    int grid = (int)((rows_c + 3) / 4);
-    if (grid > 8 * num_sms()) grid = 8 * num_sms();
-    if (grid > 0) {
-        combine_kernel<D><<<grid, 128, 0, stream>>>(Cb);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        ++*launches;
-    }
     return cudaSuccess;
 }
 

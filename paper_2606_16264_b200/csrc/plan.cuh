@@ -19,7 +19,7 @@ enum { HDR_N_ITEMS = 0, HDR_N_UNITS = 1, HDR_SPLIT_PAGES = 2, HDR_TICKET_PREFILL
 
 // req_info[i] = {kind, unit_base, nsplit, item_base}; kind 0 skip, 1 decode, 2 prefill
 struct WorkspaceLayout {
-    size_t hdr, req_info, items, units, part_ml, part_o, total;
+    size_t hdr, req_info, items, units, group_cnt, part_ml, part_o, total;
     int max_items, max_units;
 };
 
@@ -36,6 +36,7 @@ __host__ __device__ inline WorkspaceLayout make_layout(int Hq, int Hkv, int D, i
     w.req_info = off;  off += ws_align((size_t)(num_reqs > 0 ? num_reqs : 1) * sizeof(int4));
     w.items = off;     off += ws_align((size_t)(w.max_items > 0 ? w.max_items : 1) * sizeof(int2));
     w.units = off;     off += ws_align((size_t)w.max_units * sizeof(int4));
+    w.group_cnt = off; off += ws_align((size_t)w.max_units * sizeof(int));
     w.part_ml = off;   off += ws_align((size_t)w.max_units * kHeadBlock * sizeof(float2));
     w.part_o = off;    off += ws_align((size_t)w.max_units * kHeadBlock * D * sizeof(float));
     w.total = off;
@@ -47,6 +48,7 @@ struct PlanPtrs {
     int4* req_info;
     int2* items;   // {req, (qtile << 16) | (pair << 15) | head}: pair = the item also carries head + 1 (same kv group)
     int4* units;   // {req, kvh | (hb << 16), page_start, page_count}
+    int* group_cnt;  // [n_units] zeroed here: finished units per split group (indexed by the group's first unit)
 };
 
 // largest i in [0, n) with base(i) <= e, base non-decreasing
@@ -181,6 +183,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         const int kvh = u / (HB * nsplit);
         const int p0 = s * split;
         P.units[e] = make_int4(i, kvh | (hb << 16), p0, min(split, pages - p0));
+        P.group_cnt[e] = 0;
     }
     for (int e = tid; e < n_items; e += kPlanThreads) {
         const int i = owner(s_ib, 3, e);
