@@ -213,18 +213,26 @@ def run_ours(args, rank, world):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record(stream)
-    for k in range(args.steps):
+    for k in range(args.steps):  # the timed region: exactly K steps, nothing but the two library calls per step
         if flush:
             flush_buf.fill_(k & 0xff)
-        if flush:
             st_evs[k][0].record(stream)
-        one_step(evs[k])
+        one_step()
         if flush:
             st_evs[k][1].record(stream)
     e1.record(stream)
     torch.cuda.synchronize()
     total_ms = sum(a.elapsed_time(b) for a, b in st_evs) if flush else e0.elapsed_time(e1)
-    attn_ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps
+    # second pass, same steps: an event between the append and the attention call isolates the attention launches
+    # for the per-kernel roofline (kept out of the timed region: the event breaks the plan kernel's overlap with
+    # the append)
+    n_k = min(args.steps, 50)
+    for k in range(n_k):
+        if flush:
+            flush_buf.fill_(k & 0xff)
+        one_step(evs[k])
+    torch.cuda.synchronize()
+    attn_ms = sum(a.elapsed_time(b) for a, b in evs[:n_k]) / n_k
     if total_ms < 400:  # keep the GPU busy long enough for the clock sampler to see it under load
         t_end = time.perf_counter() + 0.4
         while time.perf_counter() < t_end:

@@ -14,6 +14,10 @@ __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc
                                                         const uint4* __restrict__ k_new,
                                                         const uint4* __restrict__ v_new) {
     constexpr int CH = D / 8;  // 16-byte chunks per row
+    // Programmatic dependent launch: a following kernel that opted in (the plan kernel of tropical_mixed_attention,
+    // which reads only q_lens / ctx_lens) may start while this one is still copying; every other kernel keeps
+    // normal stream order.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const long long total = (long long)b.total_q * pool.Hkv * CH * 2;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {

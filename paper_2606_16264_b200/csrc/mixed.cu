@@ -227,8 +227,20 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     P.items = (int2*)(ws + w.items);
     P.units = (int4*)(ws + w.units);
     P.group_cnt = (int*)(ws + w.group_cnt);
-    plan_kernel<<<1, kPlanThreads, 0, stream>>>(b, pool.Hq, pool.Hkv, P, g_split_pages);
-    cudaError_t e = cudaGetLastError();
+    // The plan reads only the step's metadata and writes only the workspace: launched with programmatic stream
+    // serialization it overlaps the tail of a preceding tropical_kv_append (whose kernel triggers early); after any
+    // other kernel it starts in normal stream order.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1);
+    cfg.blockDim = dim3(kPlanThreads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, plan_kernel, b, pool.Hq, pool.Hkv, P, g_split_pages);
     if (e != cudaSuccess) return e;
     ++*launches;
 
