@@ -1,0 +1,59 @@
+"""chunked prefill on growing prior context (PAPER.md:159 chunked prefill on multiplexing workers;
+P:46: later chunks cost more because they attend to more context).  A 2048-token chunk on 0 / 2048 / 4096 /
+8192 tokens of prior context, beside a decode batch: parity against the oracle on sampled rows (bottom-right causal
+alignment at scale, reading S3) and monotone growth of both the measured step time and the predicted step cost."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_16264_b200 as tb
+import synth
+from tests.gpu_harness import MAX_ABS_TOL, MEAN_ABS_TOL, DeviceStep, bits
+
+pytestmark = pytest.mark.gpu
+
+HQ, HKV, D = 40, 40, 128  # the 13B-like shape of C4 (chunk size 2048: P:181)
+
+
+def _time_us(dev, n=10):
+    for _ in range(3):
+        dev.append()
+        dev.attention()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n):
+        dev.append()
+        dev.attention()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e3 / n
+
+
+def test_chunk_cost_grows_with_chunk_index_and_matches_oracle():
+    rng = np.random.default_rng(40)
+    dec_ctx = np.clip(np.rint(np.exp(np.log(1000) + 0.9 * rng.standard_normal(32))), 64, 4096).astype(int).tolist()
+    times, preds = [], []
+    for c in (0, 2048, 4096, 8192):
+        q = [2048] + [1] * 32
+        ctx = [c] + dec_ctx
+        s = synth.make_step(np.random.default_rng(41), HQ, HKV, D, 16, q, ctx, values="tiled")
+        kp, vp = s.copy_pools()
+        oracle.kv_append(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new)
+        dev = DeviceStep(s)
+        out, lse = dev.step()
+        assert np.array_equal(bits(dev.k_pool), kp) and np.array_equal(bits(dev.v_pool), vp)
+        rows = [(0, t) for t in (0, 1, 127, 128, 129, 1000, 2046, 2047)] + [(i, 0) for i in (1, 7, 32)]
+        ref, ref_lse = oracle.attention_rows(kp, vp, s.q, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, rows)
+        idx = np.array([int(s.q_offsets[i]) + t for i, t in rows])
+        err = np.abs(out[idx] - ref)
+        assert err.max() <= MAX_ABS_TOL and err.mean() <= MEAN_ABS_TOL, (c, err.max(), err.mean())
+        assert np.abs(lse[idx] - ref_lse).max() <= 2e-3
+        times.append(_time_us(dev))
+        preds.append(tb.step_cost(HQ, HKV, D, 16, q, ctx)[0])
+        del dev
+    assert all(b > a for a, b in zip(times, times[1:])), times      # measured: later chunks cost more
+    assert all(b > a for a, b in zip(preds, preds[1:])), preds      # and the predictor says so too
+    for t, p in zip(times, preds):
+        assert abs(p - t) / t <= 0.35, (times, preds)
