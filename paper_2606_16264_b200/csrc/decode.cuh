@@ -211,32 +211,43 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
             if (issued < n_sub) issue_one();
 
             const int nvalid = L - (p0 + p) * kPageSize;  // >= 1 by construction of the unit
-            // sa/sb[0,1]: key `row`, heads cq, cq+1;  [2,3]: key row + 8
-            const bool klo = row < nvalid, khi = row + 8 < nvalid;
-            float v00 = klo ? (sa[0] + sb[0]) * A.scale_log2 : -INFINITY;
-            float v01 = klo ? (sa[1] + sb[1]) * A.scale_log2 : -INFINITY;
-            float v10 = khi ? (sa[2] + sb[2]) * A.scale_log2 : -INFINITY;
-            float v11 = khi ? (sa[3] + sb[3]) * A.scale_log2 : -INFINITY;
-            float mx0 = fmaxf(v00, v10), mx1 = fmaxf(v01, v11);
-#pragma unroll
-            for (int off = 4; off < 32; off <<= 1) {
-                mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, off));
-                mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, off));
+            // sa/sb[0,1]: key `row`, heads cq, cq+1;  [2,3]: key row + 8.  Scores relative to the running reference
+            // maximum m (shared by the 8 row groups of a head): x = s * scale - m.
+            float s00 = sa[0] + sb[0], s01 = sa[1] + sb[1], s10 = sa[2] + sb[2], s11 = sa[3] + sb[3];
+            if (nvalid < kPageSize) {  // ragged last page: mask by select (the score of an unused slot may be NaN)
+                if (row >= nvalid) { s00 = -INFINITY; s01 = -INFINITY; }
+                if (row + 8 >= nvalid) { s10 = -INFINITY; s11 = -INFINITY; }
             }
-            const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);  // finite: key 0 of the page is valid
-            const float al0 = fast_exp2(m0 - mn0), al1 = fast_exp2(m1 - mn1);
-            v00 = fast_exp2(v00 - mn0);
-            v10 = fast_exp2(v10 - mn0);
-            v01 = fast_exp2(v01 - mn1);
-            v11 = fast_exp2(v11 - mn1);
-            l0 = l0 * al0 + (v00 + v10);
-            l1 = l1 * al1 + (v01 + v11);
-            if (__any_sync(0xffffffffu, (mn0 > m0) | (mn1 > m1))) {
+            float v00 = fmaf(s00, A.scale_log2, -m0), v01 = fmaf(s01, A.scale_log2, -m1);
+            float v10 = fmaf(s10, A.scale_log2, -m0), v11 = fmaf(s11, A.scale_log2, -m1);
+            // Lazy maximum: m is raised (shuffle reduction over the 16 keys, rescale of O and l) only when some score
+            // of the page exceeds it by more than 2^8 -- always on the first page of a unit (m = -inf), rarely after.
+            if (__any_sync(0xffffffffu, fmaxf(fmaxf(v00, v01), fmaxf(v10, v11)) > 8.f)) {
+                float mx0 = fmaxf(s00, s10) * A.scale_log2, mx1 = fmaxf(s01, s11) * A.scale_log2;
+#pragma unroll
+                for (int off = 4; off < 32; off <<= 1) {
+                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, off));
+                    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, off));
+                }
+                const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);  // finite: key 0 of the page is valid
+                const float al0 = fast_exp2(m0 - mn0), al1 = fast_exp2(m1 - mn1);
+                l0 *= al0;
+                l1 *= al1;
 #pragma unroll
                 for (int db = 0; db < D / 16; ++db) { o[db][0] *= al0; o[db][1] *= al1; o[db][2] *= al0; o[db][3] *= al1; }
+                m0 = mn0;
+                m1 = mn1;
+                v00 = fmaf(s00, A.scale_log2, -m0);
+                v01 = fmaf(s01, A.scale_log2, -m1);
+                v10 = fmaf(s10, A.scale_log2, -m0);
+                v11 = fmaf(s11, A.scale_log2, -m1);
             }
-            m0 = mn0;
-            m1 = mn1;
+            v00 = fast_exp2(v00);
+            v10 = fast_exp2(v10);
+            v01 = fast_exp2(v01);
+            v11 = fast_exp2(v11);
+            l0 += v00 + v10;
+            l1 += v01 + v11;
             // P^T as B operand: transpose the two 8x8 (key x head) bf16 blocks of the S^T fragment
             const uint32_t pb0 = movmatrix_trans(pack_bf16x2(v00, v01));
             const uint32_t pb1 = movmatrix_trans(pack_bf16x2(v10, v11));
