@@ -9,6 +9,10 @@ from .binding import (  # noqa: F401
     CostBreakdown,
     CostModel,
     KVPool,
+    SIM_COLOCATED,
+    SIM_DISAGGREGATED,
+    SIM_MULTIPLEXED,
+    SimConfig,
     TropicalError,
     debug_attention_simt,
     debug_read_profile,
@@ -21,6 +25,7 @@ from .binding import (  # noqa: F401
     last_launch_count,
     lib,
     mixed_attention,
+    sim_run,
     status_string,
     step_cost,
     step_host,

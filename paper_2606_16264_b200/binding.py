@@ -45,11 +45,41 @@ class CostBreakdown(ctypes.Structure):
                 ("decode_units", ctypes.c_int64)]
 
 
+class SimRequest(ctypes.Structure):
+    _fields_ = [("arrival_us", ctypes.c_double), ("prompt_len", ctypes.c_int32), ("output_len", ctypes.c_int32)]
+
+
+class SimConfig(ctypes.Structure):
+    """include/tropical_sim.h: tropical_sim_config_t."""
+    _fields_ = [("policy", ctypes.c_int32), ("num_workers", ctypes.c_int32), ("num_prefill_workers", ctypes.c_int32),
+                ("chunk_tokens", ctypes.c_int32), ("ttft_slo_us", ctypes.c_double), ("tpot_slo_us", ctypes.c_double),
+                ("decode_guard", ctypes.c_double), ("hbm_watermark", ctypes.c_double),
+                ("kv_capacity_tokens", ctypes.c_int64), ("migrate_us_per_token", ctypes.c_double),
+                ("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+                ("page_size", ctypes.c_int32), ("num_layers", ctypes.c_int32), ("attn", CostModel),
+                ("linear_us_per_token", ctypes.c_double), ("iter_overhead_us", ctypes.c_double)]
+
+
+class SimResult(ctypes.Structure):
+    _fields_ = [("ttft_us", ctypes.c_double), ("tpot_us", ctypes.c_double), ("first_token_us", ctypes.c_double),
+                ("finish_us", ctypes.c_double), ("prefill_worker", ctypes.c_int32), ("decode_worker", ctypes.c_int32),
+                ("multiplexed", ctypes.c_int32)]
+
+
+class SimSummary(ctypes.Structure):
+    _fields_ = [("attainment", ctypes.c_double), ("ttft_mean_us", ctypes.c_double), ("ttft_p90_us", ctypes.c_double),
+                ("tpot_mean_us", ctypes.c_double), ("tpot_p90_us", ctypes.c_double), ("makespan_us", ctypes.c_double),
+                ("iterations", ctypes.c_int64), ("multiplexed_prefills", ctypes.c_int64)]
+
+
+SIM_COLOCATED, SIM_DISAGGREGATED, SIM_MULTIPLEXED = 0, 1, 2
+
 EXPORTS = (
     "tropical_kv_append", "tropical_kv_gather", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
     "tropical_debug_attention_simt", "tropical_debug_set_mode", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile",
+    "tropical_sim_run",
 )
 
 
@@ -297,3 +327,14 @@ def step_cost(num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int
         return None, bd
     _check(rc, "tropical_step_cost")
     return us.value, bd
+
+
+def sim_run(config: SimConfig, requests: Sequence[tuple]):
+    """Scheduler simulation (include/tropical_sim.h).  requests: (arrival_us, prompt_len, output_len) sorted by
+    arrival.  Returns (list of SimResult, SimSummary).  Host only; works without a GPU."""
+    n = len(requests)
+    reqs = (SimRequest * max(n, 1))(*[SimRequest(float(a), int(p), int(o)) for a, p, o in requests])
+    res = (SimResult * max(n, 1))()
+    summ = SimSummary()
+    _check(lib().tropical_sim_run(ctypes.byref(config), ctypes.c_int32(n), reqs, res, ctypes.byref(summ)), "tropical_sim_run")
+    return [res[i] for i in range(n)], summ

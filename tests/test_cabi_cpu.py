@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared_functions():
-    text = open(os.path.join(ROOT, "include", "tropical.h")).read()
+    text = open(os.path.join(ROOT, "include", "tropical.h")).read() + open(os.path.join(ROOT, "include", "tropical_sim.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(tropical_[a-z_0-9]+)\s*\(", text)))
 
