@@ -288,3 +288,34 @@ def test_step_host_equals_device_path():
     assert np.array_equal(bits(dev.k_pool), kp)
     assert np.abs(h_lse.numpy() - ref_lse).max() <= 2e-3
     assert tb.last_launch_count() >= 2
+
+
+# ------------------------------------------------------------------ head-group shapes and seeded random batches
+@pytest.mark.parametrize("Hq,Hkv", [(6, 2), (2, 1), (16, 1), (48, 3), (64, 1), (5, 5), (12, 4)])
+@pytest.mark.parametrize("d", [64, 128])
+def test_head_group_shapes(Hq, Hkv, d):
+    """g = Hq / Hkv odd (one query tile per item), g = 2 (pairs), g = 16 / 64 (several 8-head decode blocks per kv head),
+    MHA with an odd head count: same step, every shape against the oracle."""
+    s = _step(50 + Hq + Hkv, Hq, Hkv, d, [130, 1, 1, 1, 40], [5, 777, 2100, 15, 130])
+    _check_step(s)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_seeded_random_batches(seed):
+    """Random mixes of skipped / decode / prefill requests (lengths around page, tile and split edges), random head
+    configuration, requests in random order."""
+    rng = np.random.default_rng(1000 + seed)
+    Hkv = int(rng.choice([1, 2, 4]))
+    g = int(rng.choice([1, 2, 3, 4, 8]))
+    d = int(rng.choice([64, 128]))
+    n = int(rng.integers(1, 12))
+    edges = np.array([0, 1, 2, 15, 16, 17, 31, 127, 128, 129, 255, 256, 257, 383, 700])
+    qs, cs = [], []
+    for _ in range(n):
+        kind = rng.integers(0, 4)
+        q = 0 if kind == 0 else 1 if kind == 1 else int(rng.choice(edges[2:])) + int(rng.integers(0, 3))
+        c = int(rng.choice(edges)) + int(rng.integers(0, 3)) + (int(rng.integers(0, 3000)) if kind == 1 else 0)
+        qs.append(q)
+        cs.append(c)
+    s = synth.make_step(rng, Hkv * g, Hkv, d, 16, qs, cs)
+    _check_step(s)
