@@ -319,3 +319,29 @@ def test_seeded_random_batches(seed):
         cs.append(c)
     s = synth.make_step(rng, Hkv * g, Hkv, d, 16, qs, cs)
     _check_step(s)
+
+
+def test_step_is_cuda_graph_capturable_and_idempotent():
+    """The step has no host sync and mutates none of its metadata: append + attention captured once in a CUDA graph
+    replays to the same bits (tensor maps are kernel parameters; the plan kernel's dependent launch is captured)."""
+    s = _step(17, 8, 2, 128, [200, 1, 1, 1, 33], [56, 700, 2049, 17, 0])
+    ref, _, kp, vp = oracle.step(s)
+    dev = DeviceStep(s)
+    dev.step()                                  # eager run: also warms one-time function attributes
+    eager = bits(dev.out).copy()
+    dev.out.zero_()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            dev.append()
+            dev.attention()
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(3):
+        dev.out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(bits(dev.out), eager)
+    assert np.array_equal(bits(dev.k_pool), kp) and np.array_equal(bits(dev.v_pool), vp)
+    assert errors(dev.out_f64(), ref)[0] <= MAX_ABS_TOL
