@@ -126,6 +126,15 @@ static __device__ unsigned long long g_wait_cycles[512];
 static __device__ unsigned long long g_wait_calls[512];
 #endif
 
+#ifdef TROPICAL_DEBUG_WAIT
+// Debug build (-DTROPICAL_DEBUG_WAIT): a wait that times out records (tag, block, warp, parity, aux) of the FIRST
+// stuck waiter, raises g_wait_abort so that every other wait falls through, and the kernel runs to its end with
+// garbage results; tropical_debug_wait_profile(...) then reports the record (cycles[0..4]).
+static __device__ int g_wait_abort;
+static __device__ int g_wait_abort_info[8];
+static __device__ int* g_wait_stuck;  // host-mapped [16][3] (readable after a fault): per warp of block 0, the wait it was in (tag, parity, aux)
+#endif
+
 // Bounded wait: a protocol bug traps (launch failure) instead of hanging the GPU box.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0, int aux = 0) {
 #ifdef TROPICAL_WAIT_PROF
@@ -134,14 +143,37 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int ta
     if (!mbar_try_wait(bar, parity)) {
         long long t0 = clock64();
         while (!mbar_try_wait(bar, parity)) {
-            if (clock64() - t0 > 4000000000LL) {  // ~2 s at 1.9 GHz
 #ifdef TROPICAL_DEBUG_WAIT
-                if ((threadIdx.x & 31) == 0) printf("mbar timeout: block %d warp %d tag %d parity %u aux %d\n", blockIdx.x, threadIdx.x >> 5, tag, parity, aux);
-                long long t1 = clock64();
-                while (clock64() - t1 < 1500000000LL) {}  // let every stuck warp report before the trap
-#endif
-                __trap();
+            if (*(volatile int*)&g_wait_abort) {
+                if ((threadIdx.x & 31) == 0 && blockIdx.x == 0 && g_wait_stuck != nullptr &&
+                    g_wait_stuck[(threadIdx.x >> 5) * 3] == 0) {
+                    g_wait_stuck[(threadIdx.x >> 5) * 3 + 1] = (int)parity;
+                    g_wait_stuck[(threadIdx.x >> 5) * 3 + 2] = aux;
+                    g_wait_stuck[(threadIdx.x >> 5) * 3] = tag;
+                    __threadfence_system();
+                }
+                break;
             }
+            if (clock64() - t0 > 400000000LL) {  // ~0.2 s
+                if ((threadIdx.x & 31) == 0 && atomicCAS(&g_wait_abort, 0, 1) == 0) {
+                    g_wait_abort_info[0] = tag;
+                    g_wait_abort_info[1] = blockIdx.x;
+                    g_wait_abort_info[2] = threadIdx.x >> 5;
+                    g_wait_abort_info[3] = (int)parity;
+                    g_wait_abort_info[4] = aux;
+                    if (g_wait_stuck != nullptr && blockIdx.x == 0) {
+                        g_wait_stuck[(threadIdx.x >> 5) * 3 + 1] = (int)parity;
+                        g_wait_stuck[(threadIdx.x >> 5) * 3 + 2] = aux;
+                        g_wait_stuck[(threadIdx.x >> 5) * 3] = tag;
+                        g_wait_stuck[48] = 1;
+                    }
+                    __threadfence_system();
+                }
+                break;
+            }
+#else
+            if (clock64() - t0 > 4000000000LL) __trap();  // ~2 s at 1.9 GHz
+#endif
         }
     }
 #ifdef TROPICAL_WAIT_PROF

@@ -195,6 +195,20 @@ size_t profile_offset_bytes() { return make_layout(1, 1, 64, 1, 1).hdr + HDR_PRO
 static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches (A/B timing only)
 void set_debug_mode(int mode) { g_mode = mode; }
 static int g_grid_cap = 0;  // test hook: 0 = one CTA per SM
+#ifdef TROPICAL_DEBUG_WAIT
+static volatile int* g_stuck_host = nullptr;
+static void debug_wait_setup() {
+    if (g_stuck_host != nullptr) return;
+    int* h = nullptr;
+    if (cudaHostAlloc((void**)&h, 64 * sizeof(int), cudaHostAllocMapped) != cudaSuccess) return;
+    for (int i = 0; i < 64; ++i) h[i] = 0;
+    int* d = nullptr;
+    if (cudaHostGetDevicePointer((void**)&d, h, 0) != cudaSuccess) return;
+    cudaMemcpyToSymbol(g_wait_stuck, &d, sizeof d);
+    g_stuck_host = h;
+}
+#endif
+
 int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset) {
 #ifdef TROPICAL_WAIT_PROF
     if (n > 512) n = 512;
@@ -204,6 +218,30 @@ int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int
         static unsigned long long zeros[512];
         cudaMemcpyToSymbol(g_wait_cycles, zeros, sizeof zeros);
         cudaMemcpyToSymbol(g_wait_calls, zeros, sizeof zeros);
+    }
+    return n;
+#elif defined(TROPICAL_DEBUG_WAIT)
+    if (g_stuck_host != nullptr) {  // host-mapped: readable even after the kernel faulted
+        for (int i = 0; i < n; ++i) { cycles[i] = 0; calls[i] = 0; }
+        cycles[0] = (unsigned long long)g_stuck_host[48];
+        for (int w = 0; w < 16 && 16 + w * 3 + 2 < n; ++w)
+            for (int k = 0; k < 3; ++k) cycles[16 + w * 3 + k] = (unsigned long long)(long long)g_stuck_host[w * 3 + k];
+        calls[0] = 1;
+        if (reset) for (int i = 0; i < 64; ++i) g_stuck_host[i] = 0;
+        return n;
+    }
+    // debug build: cycles[0] = abort flag, cycles[1..5] = tag, block, warp, parity, aux of the first stuck wait
+    int flag = 0, info[8] = {0};
+    if (cudaMemcpyFromSymbol(&flag, g_wait_abort, sizeof flag) != cudaSuccess) return -1;
+    if (cudaMemcpyFromSymbol(info, g_wait_abort_info, sizeof info) != cudaSuccess) return -1;
+    for (int i = 0; i < n; ++i) { cycles[i] = 0; calls[i] = 0; }
+    cycles[0] = (unsigned long long)flag;
+    for (int i = 0; i < 5 && i + 1 < n; ++i) cycles[i + 1] = (unsigned long long)(long long)info[i];
+    calls[0] = 1;
+    (void)0;
+    if (reset) {
+        const int zero = 0;
+        cudaMemcpyToSymbol(g_wait_abort, &zero, sizeof zero);
     }
     return n;
 #else
@@ -275,6 +313,9 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     A.part_o = (float*)(ws + w.part_o);
     A.group_cnt = P.group_cnt;
 
+#ifdef TROPICAL_DEBUG_WAIT
+    debug_wait_setup();
+#endif
     if (g_mode == 0) {
         // A3 + A4 in one persistent launch: the product path
         const size_t smem = MixedCfg<D>::SMEM;
