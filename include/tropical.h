@@ -175,10 +175,14 @@ void tropical_debug_set_grid(int num_ctas);
  * that small test batches exercise multi-block decode units.  Process-global. */
 void tropical_debug_set_split_pages(int pages);
 
-/* Measurement hook, only in builds compiled with -DTROPICAL_WAIT_PROF (else TROPICAL_ERR_UNSUPPORTED): cycles spent
- * in and calls of every mbarrier wait of the step kernel, summed over warps, indexed by the wait's tag (the numbers
- * next to the mbar_wait calls in csrc/).  cycles/calls are [host] arrays of n <= 512 entries; reset != 0 zeroes
- * the device counters after the read.  Synchronises the device. */
+/* Measurement / debugging hook, only in special builds (else TROPICAL_ERR_UNSUPPORTED).  Synchronises the device.
+ *  -DTROPICAL_WAIT_PROF: cycles spent in and calls of every mbarrier wait of the step kernel, summed over warps,
+ *    indexed by the wait's tag (the numbers next to the mbar_wait calls in csrc/); reset != 0 zeroes the counters.
+ *  -DTROPICAL_DEBUG_WAIT: instead of trapping after ~2 s, a wait that is stuck for ~0.2 s raises an abort flag that
+ *    lets every wait fall through (the step finishes with garbage); cycles[0] = that flag and, for warp w of CTA 0,
+ *    cycles[16 + 3 w .. + 2] = tag, parity and aux value of the wait it was stuck in.  The record lives in
+ *    host-mapped memory, so it can be read even when the kernel faulted afterwards.
+ * cycles / calls are [host] arrays of n <= 512 entries. */
 int tropical_debug_wait_profile(uint64_t *cycles, uint64_t *calls, int32_t n, int32_t reset);
 
 /* Measurement hook: role timestamps of the LAST fused step kernel that ran with this workspace

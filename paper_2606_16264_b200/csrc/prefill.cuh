@@ -18,7 +18,9 @@
 //                   MMA warp consumes tiles (K0, V0, K1, V1, ...); one warp issues the K tiles, a second one the V
 //                   tiles.  The HND pool makes every box one contiguous 2 KiB run of HBM/L2.
 //   MMA warp      : one elected lane issues, per KV tile, {PV_A(kt), S_A(kt+1)} when P_A(kt) is posted and then
-//                   {PV_B(kt), S_B(kt+1)} when P_B(kt) is; all operands of the issue are warp-uniform (common.cuh uni()).
+//                   {PV_B(kt), S_B(kt+1)} when P_B(kt) is; a one-tile item (MHA, odd groups) alternates between the
+//                   two S slots instead and issues S(kt+1) ahead of PV(kt).  All operands of the issue are
+//                   warp-uniform (common.cuh uni()).
 //   softmax WG    : 4 warps, thread r owns query row r (TMEM lane r) of BOTH query tiles: no shuffles.  It alternates
 //                   between the tiles, so the tensor pipe runs PV_A(kt), S_A(kt+1) while it exponentiates S_B(kt).
 //                   (Two warpgroups, one per tile, were measured: no faster -- each waits for its own S -- and they
