@@ -18,9 +18,7 @@
 //                   MMA warp consumes tiles (K0, V0, K1, V1, ...); one warp issues the K tiles, a second one the V
 //                   tiles.  The HND pool makes every box one contiguous 2 KiB run of HBM/L2.
 //   MMA warp      : one elected lane issues, per KV tile, {PV_A(kt), S_A(kt+1)} when P_A(kt) is posted and then
-//                   {PV_B(kt), S_B(kt+1)} when P_B(kt) is; a one-tile item (MHA, odd groups) alternates between the
-//                   two S slots instead and issues S(kt+1) ahead of PV(kt).  All operands of the issue are
-//                   warp-uniform (common.cuh uni()).
+//                   {PV_B(kt), S_B(kt+1)} when P_B(kt) is; all operands of the issue are warp-uniform (common.cuh uni()).
 //   softmax WG    : 4 warps, thread r owns query row r (TMEM lane r) of BOTH query tiles: no shuffles.  It alternates
 //                   between the tiles, so the tensor pipe runs PV_A(kt), S_A(kt+1) while it exponentiates S_B(kt).
 //                   (Two warpgroups, one per tile, were measured: no faster -- each waits for its own S -- and they
@@ -184,24 +182,11 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
             }
         }
         const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
-        // ring order = the MMA warp's consumption order: two-tile items K0, V0, K1, V1, ...; one-tile items
-        // K0, K1, V0, K2, V1, ... (S(kt+1) is issued ahead of PV(kt) there, see prefill_mma): V lags K by `lag` steps
-        const int lag = it.nt == 1 ? 1 : 0;
-        for (int s = 0; s < it.n_kt + lag; ++s) {
-            // One-tile order: a ring slot is shared by both producers, so an entry of the OTHER producer is not just
-            // skipped, its slot's release is observed too -- a parity wait is only safe for a waiter at most one
-            // phase behind, and a producer that ran two uses of a slot ahead would see a stale phase as "free" and
-            // overwrite live tiles.  (Two-tile order: K tiles always use slot 0 and V tiles slot 1, one producer each.)
-            if (s < it.n_kt) {
-                if (KIND == 0) prefill_load_tile<D>(A, B, ring, it, pt, n_pages, s, tm_kv, cur, lane);
-                else if (lag) mbar_wait(&B->kv_empty[cur.slot], cur.phase ^ 1, 116);
-                cur.advance(C::KV_SLOTS);
-            }
-            if (s >= lag) {
-                if (KIND == 1) prefill_load_tile<D>(A, B, ring, it, pt, n_pages, s - lag, tm_kv, cur, lane);
-                else if (lag) mbar_wait(&B->kv_empty[cur.slot], cur.phase ^ 1, 117);
-                cur.advance(C::KV_SLOTS);
-            }
+        for (int kt = 0; kt < it.n_kt; ++kt) {  // ring entries 2 kt (K) and 2 kt + 1 (V)
+            if (KIND == 0) prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt, tm_kv, cur, lane);
+            cur.advance(C::KV_SLOTS);
+            if (KIND == 1) prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt, tm_kv, cur, lane);
+            cur.advance(C::KV_SLOTS);
         }
         ++item_it;
     }
@@ -222,11 +207,11 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
     constexpr uint32_t IDESC_S = make_idesc_bf16(128, 128, false);
     constexpr uint32_t IDESC_O = make_idesc_bf16(128, D, true);
     uint32_t item_it = 0;
-    uint32_t s0 = 0, s1 = 0;      // uses of S slot 0, 1 so far (phases of s_full / p_full)
-    uint32_t cnt0 = 0, cnt1 = 0;  // items that accumulated into O_A, O_B so far (o_empty phases)
+    uint32_t g0 = 0, g1 = 0;      // S / P / PV iterations of query tile A, B so far (barrier phases)
+    uint32_t cnt0 = 0, cnt1 = 0;  // items that carried tile A, B so far (o_empty phases)
     RingCursor cur = {0, 0};
 
-    auto issue_s = [&](int w, int sw, int slot) {  // S slot sw = Q_w K^T, K tile in ring slot `slot`
+    auto issue_s = [&](int w, int slot) {  // S_w = Q_w K^T, K tile in ring slot `slot`
         const uint32_t k_a = ring_a + slot * C::TILE_BYTES;
         const uint32_t qw_a = q_a + w * C::TILE_BYTES;
         if (elect_one()) {
@@ -235,43 +220,12 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
 #pragma unroll
                 for (int k4 = 0; k4 < 4; ++k4) {
                     const uint32_t o = cb * C::HALF_BYTES + k4 * 32;
-                    tc_mma_ss(tm + C::TM_S + sw * 128, make_smem_desc_sw128(qw_a + o, 0, 1024),
+                    tc_mma_ss(tm + C::TM_S + w * 128, make_smem_desc_sw128(qw_a + o, 0, 1024),
                               make_smem_desc_sw128(k_a + o, 0, 1024), IDESC_S, (cb | k4) != 0);
                 }
-            tc_commit(&B->s_full[sw]);
+            tc_commit(&B->s_full[w]);
         }
         __syncwarp();
-    };
-    // O_w += P(S slot sw) V, V tile at v_a; waits for the softmax warpgroup's P first
-    auto issue_pv = [&](int w, int sw, uint32_t v_a, int kt) {
-        if (kt == 0) mbar_wait(&B->o_empty[w], ((w ? cnt1 : cnt0) & 1) ^ 1, 108, item_it);  // previous epilogue has read O_w
-        mbar_wait(&B->p_full[sw], (sw ? s1 : s0) & 1, 109, item_it * 100000 + kt);
-        tc_fence_after();
-        if (elect_one()) {
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks)  // 16 keys per MMA
-                tc_mma_ts(tm + C::TM_O + w * 128, tm + C::TM_S + sw * 128 + ks * 8,
-                          make_smem_desc_sw128(v_a + ks * 2048, C::HALF_BYTES, 1024), IDESC_O, (kt | ks) != 0);
-            tc_commit(&B->pv_done[w]);
-        }
-        __syncwarp();
-        if (sw) ++s1; else ++s0;
-    };
-    auto wait_v = [&](const RingCursor& vcur, const PrefillItem& it, int kt) -> uint32_t {
-        mbar_wait(&B->kv_full[vcur.slot], vcur.phase, 107, item_it * 100000 + kt * 1000 + it.n_kt);
-        const uint32_t v_a = ring_a + vcur.slot * C::TILE_BYTES;
-        if (kt + 1 == it.n_kt) {  // zero V rows past the last visible key (stale or poisoned smem)
-            const int nvalid = it.l_tile - kt * kKvTile;
-            const int nz = (kKvTile - nvalid) * 8 * C::CB;
-            for (int idx = lane; idx < nz; idx += 32) {
-                const int r = nvalid + idx / (8 * C::CB), rem = idx % (8 * C::CB);
-                const uint32_t a = v_a + (rem >> 3) * C::HALF_BYTES + r * 128 + ((rem & 7) << 4);
-                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
-            }
-            fence_proxy_async();
-            __syncwarp();
-        }
-        return v_a;
     };
 
     for (;;) {
@@ -287,7 +241,7 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
         mbar_wait(&B->kv_full[cur.slot], cur.phase, 104, item_it);  // K(0)
         tc_fence_after();
 #pragma unroll 1
-        for (int w = 0; w < it.nt; ++w) issue_s(w, w, cur.slot);
+        for (int w = 0; w < it.nt; ++w) issue_s(w, cur.slot);
         if (elect_one()) {
             tc_commit(&B->kv_empty[cur.slot]);
             if (it.n_kt == 1) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
@@ -295,55 +249,56 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
         __syncwarp();
         cur.advance(C::KV_SLOTS);
 
-        if (it.nt == 1) {
-            // one query tile: the two S slots alternate per KV tile and S(kt+1) is issued AHEAD of PV(kt), so the
-            // tensor pipe computes the next scores while the softmax warpgroup works on the current ones
-            for (int kt = 0; kt < it.n_kt; ++kt) {
-                if (kt + 1 < it.n_kt) {
-                    mbar_wait(&B->kv_full[cur.slot], cur.phase, 104, item_it * 100000 + kt);  // K(kt+1)
-                    tc_fence_after();
-                    issue_s(0, (kt + 1) & 1, cur.slot);
-                    if (elect_one()) {
-                        tc_commit(&B->kv_empty[cur.slot]);
-                        if (kt + 2 == it.n_kt) tc_commit(&B->q_empty);
-                    }
-                    __syncwarp();
-                    cur.advance(C::KV_SLOTS);
+        for (int kt = 0; kt < it.n_kt; ++kt) {
+            const RingCursor vcur = cur;  // V(kt)
+            cur.advance(C::KV_SLOTS);
+            const RingCursor kcur = cur;  // K(kt+1)
+            const bool has_next = kt + 1 < it.n_kt;
+            if (has_next) cur.advance(C::KV_SLOTS);
+            mbar_wait(&B->kv_full[vcur.slot], vcur.phase, 107, item_it * 100000 + kt * 1000 + it.n_kt);
+            const uint32_t v_a = ring_a + vcur.slot * C::TILE_BYTES;
+            if (!has_next) {  // zero V rows past the last visible key (stale or poisoned smem)
+                const int nvalid = it.l_tile - kt * kKvTile;
+                const int nz = (kKvTile - nvalid) * 8 * C::CB;
+                for (int idx = lane; idx < nz; idx += 32) {
+                    const int r = nvalid + idx / (8 * C::CB), rem = idx % (8 * C::CB);
+                    const uint32_t a = v_a + (rem >> 3) * C::HALF_BYTES + r * 128 + ((rem & 7) << 4);
+                    asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
                 }
-                const uint32_t v_a = wait_v(cur, it, kt);
-                issue_pv(0, kt & 1, v_a, kt);
-                if (elect_one()) tc_commit(&B->kv_empty[cur.slot]);
+                fence_proxy_async();
                 __syncwarp();
-                cur.advance(C::KV_SLOTS);
             }
-        } else {
-            for (int kt = 0; kt < it.n_kt; ++kt) {
-                const RingCursor vcur = cur;  // V(kt)
-                cur.advance(C::KV_SLOTS);
-                const RingCursor kcur = cur;  // K(kt+1)
-                const bool has_next = kt + 1 < it.n_kt;
-                if (has_next) cur.advance(C::KV_SLOTS);
-                const uint32_t v_a = wait_v(vcur, it, kt);
 #pragma unroll 1
-                for (int w = 0; w < 2; ++w) {
-                    issue_pv(w, w, v_a, kt);
-                    if (has_next) {
-                        if (w == 0) {
-                            mbar_wait(&B->kv_full[kcur.slot], kcur.phase, 104, item_it * 100000 + kt);
-                            tc_fence_after();
-                        }
-                        issue_s(w, w, kcur.slot);
-                    }
-                }
+            for (int w = 0; w < it.nt; ++w) {
+                const uint32_t gw = w ? g1 : g0;
+                if (kt == 0) mbar_wait(&B->o_empty[w], ((w ? cnt1 : cnt0) & 1) ^ 1, 108, item_it);  // previous epilogue has read O_w
+                mbar_wait(&B->p_full[w], gw & 1, 109, item_it * 100000 + kt * 1000 + it.n_kt);
+                tc_fence_after();
                 if (elect_one()) {
-                    tc_commit(&B->kv_empty[vcur.slot]);
-                    if (has_next) {
-                        tc_commit(&B->kv_empty[kcur.slot]);
-                        if (kt + 2 == it.n_kt) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
-                    }
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks)  // 16 keys per MMA
+                        tc_mma_ts(tm + C::TM_O + w * 128, tm + C::TM_S + w * 128 + ks * 8,
+                                  make_smem_desc_sw128(v_a + ks * 2048, C::HALF_BYTES, 1024), IDESC_O, (kt | ks) != 0);
+                    tc_commit(&B->pv_done[w]);
                 }
                 __syncwarp();
+                if (has_next) {
+                    if (w == 0) {
+                        mbar_wait(&B->kv_full[kcur.slot], kcur.phase, 104, item_it * 100000 + kt);
+                        tc_fence_after();
+                    }
+                    issue_s(w, kcur.slot);
+                }
+                if (w) ++g1; else ++g0;
             }
+            if (elect_one()) {
+                tc_commit(&B->kv_empty[vcur.slot]);
+                if (has_next) {
+                    tc_commit(&B->kv_empty[kcur.slot]);
+                    if (kt + 2 == it.n_kt) tc_commit(&B->q_empty);  // every S MMA of this item has been issued
+                }
+            }
+            __syncwarp();
         }
         ++cnt0;
         if (it.nt > 1) ++cnt1;
@@ -365,8 +320,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
     const uint32_t tm = B->tmem_base + ((uint32_t)(wg_warp * 32) << 16);
     const float scale = A.scale_log2;
     uint32_t item_it = 0;
-    uint32_t cs0 = 0, cs1 = 0;  // uses of S slot 0, 1 so far (phases of s_full / p_full)
-    uint32_t gA = 0, gB = 0;    // PV iterations into O_A, O_B so far (phases of pv_done)
+    uint32_t gA = 0, gB = 0;  // S / P / PV iterations of query tile A, B so far (barrier phases)
 
     for (;;) {
         const int ms = item_it & 1;
@@ -385,12 +339,10 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
 #pragma unroll 1
           for (int w = 0; w < it.nt; ++w) {  // the warpgroup alternates between the two query tiles: while it works on
             // S_B(kt) the tensor pipe runs PV_A(kt) and S_A(kt+1)
-            // S slot: the tile's own for a two-tile item; alternating per KV tile for a one-tile item (prefill_mma)
-            const int sw = it.nt == 1 ? (kt & 1) : w;
-            const uint32_t s_col = tm + C::TM_S + sw * 128, o_col = tm + C::TM_O + w * 128;
+            const uint32_t s_col = tm + C::TM_S + w * 128, o_col = tm + C::TM_O + w * 128;
             float m_used = w ? mB : mA, l = w ? lB : lA;
             const uint32_t g = (w ? gB : gA) + kt;
-            mbar_wait(&B->s_full[sw], (sw ? cs1 : cs0) & 1, 111, item_it * 100000 + kt * 1000 + it.n_kt);
+            mbar_wait(&B->s_full[w], g & 1, 111, item_it * 100000 + kt * 1000 + it.n_kt);
             tc_fence_after();
             // ONE pass over the tile in 32-column chunks, the TMEM load of the next chunk in flight while the current
             // one is exponentiated (two register buffers).  P = exp2(s*scale - m_used) is written with the running
@@ -508,8 +460,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
             // and PV(last) in the epilogue.  Skipping phases let a short item's epilogue pass its wait on a
             // stale phase while the MMA warp was still waiting for that item's first V tile.
             if (kt > 0) mbar_wait(&B->pv_done[w], (g - 1) & 1, 114, item_it * 100000 + kt * 1000 + it.n_kt);
-            mbar_arrive(&B->p_full[sw]);
-            if (sw) ++cs1; else ++cs0;
+            mbar_arrive(&B->p_full[w]);
             if (w) { mB = m_used; lB = l; } else { mA = m_used; lA = l; }
           }
         }

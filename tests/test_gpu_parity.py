@@ -345,3 +345,14 @@ def test_step_is_cuda_graph_capturable_and_idempotent():
         assert np.array_equal(bits(dev.out), eager)
     assert np.array_equal(bits(dev.k_pool), kp) and np.array_equal(bits(dev.v_pool), vp)
     assert errors(dev.out_f64(), ref)[0] <= MAX_ABS_TOL
+
+
+def test_more_requests_than_plan_threads():
+    """1100 requests: the plan kernel's threads own two requests each and its ticket search falls back from the
+    shared-memory tables (1024 requests) to the workspace."""
+    rng = np.random.default_rng(77)
+    n = 1100
+    qs = [1] * n
+    qs[5], qs[700] = 33, 2
+    cs = rng.integers(0, 40, n).tolist()
+    _check_step(_step(78, 2, 2, 64, qs, cs))
