@@ -105,6 +105,15 @@ int tropical_mixed_attention(const tropical_kv_pool_t *pool, const tropical_batc
                              const void *q, void *out, float *lse, float sm_scale,
                              void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* Opt-in debug check of the DEVICE-resident contents of a batch, which the other calls cannot validate without a
+ * sync (out-of-range page ids there are undefined behaviour): q_lens / ctx_lens >= 0, q_offsets the exclusive prefix
+ * sum of q_lens with q_offsets[num_reqs] == total_q, ctx + q <= max_kv_len, ceil((ctx + q) / page_size) <=
+ * page_table_stride, every page id a request can touch in [0, num_pages).  Runs one small kernel and synchronises
+ * the stream.  Returns TROPICAL_OK, or TROPICAL_ERR_INVALID_ARG with *first_bad_request [host, nullable] = the lowest
+ * offending request index (num_reqs when only the final q_offsets entry is wrong). */
+int tropical_validate_batch(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
+                            int32_t *first_bad_request, void *cuda_stream);
+
 /* End-to-end step from HOST buffers (what bench.py's "e2e" times): copies this step's inputs
  * host->device into caller-provided device staging, runs append + attention, copies out back,
  * and synchronises the stream before returning.  The KV pool stays device resident (it is the

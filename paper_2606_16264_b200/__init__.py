@@ -28,6 +28,7 @@ from .binding import (  # noqa: F401
     sim_run,
     status_string,
     step_cost,
+    validate_batch,
     step_host,
     step_host_staging_bytes,
     version,

@@ -75,7 +75,7 @@ class SimSummary(ctypes.Structure):
 SIM_COLOCATED, SIM_DISAGGREGATED, SIM_MULTIPLEXED = 0, 1, 2
 
 EXPORTS = (
-    "tropical_kv_append", "tropical_kv_gather", "tropical_workspace_bytes", "tropical_mixed_attention",
+    "tropical_kv_append", "tropical_kv_gather", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
     "tropical_debug_attention_simt", "tropical_debug_set_mode", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile",
@@ -103,7 +103,7 @@ def lib():
     L.tropical_status_string.restype = ctypes.c_char_p
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
-    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_mixed_attention", "tropical_step_host",
+    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_validate_batch", "tropical_mixed_attention", "tropical_step_host",
                  "tropical_step_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
                  "tropical_debug_read_profile"):
         getattr(L, name).restype = ctypes.c_int
@@ -238,6 +238,17 @@ def kv_gather(pool: KVPool, batch: Batch, req: int, n_keys: int, stream=None):
     _check(lib().tropical_kv_gather(ctypes.byref(p), ctypes.byref(b), ctypes.c_int32(req), ctypes.c_int32(n_keys),
                                     _ptr(kd), _ptr(vd), _stream(stream)), "tropical_kv_gather")
     return kd, vd
+
+
+def validate_batch(pool: KVPool, batch: Batch, stream=None):
+    """Opt-in debug check of the batch's device arrays (syncs).  Returns None if valid, else the first bad request."""
+    bad = ctypes.c_int32(-1)
+    p, b = pool.c(), batch.c()
+    rc = lib().tropical_validate_batch(ctypes.byref(p), ctypes.byref(b), ctypes.byref(bad), _stream(stream))
+    if rc == 1 and bad.value >= 0:
+        return bad.value
+    _check(rc, "tropical_validate_batch")
+    return None
 
 
 def workspace_bytes(pool: KVPool, num_reqs: int, total_q: int, max_kv_len: int) -> int:

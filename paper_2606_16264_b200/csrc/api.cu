@@ -123,6 +123,33 @@ int tropical_kv_gather(const tropical_kv_pool_t* pool, const tropical_batch_t* b
     return TROPICAL_OK;
 }
 
+int tropical_validate_batch(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, int32_t* first_bad_request,
+                            void* cuda_stream) {
+    g_launches = 0;
+    int rc = check_pool(pool);
+    if (rc != TROPICAL_OK) return rc;
+    rc = check_batch(pool, batch);
+    if (rc != TROPICAL_OK) return rc;
+    if (batch->num_reqs > 0 && batch->q_offsets == nullptr) return TROPICAL_ERR_INVALID_ARG;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    int* d_bad = nullptr;  // the one call of this library that allocates: a debug aid, 4 bytes, freed before it returns
+    cudaError_t e = cudaMalloc((void**)&d_bad, sizeof(int));
+    if (e != cudaSuccess) return cuda_fail(e, "validate_batch alloc");
+    int bad = 0x7fffffff;
+    e = cudaMemcpyAsync(d_bad, &bad, sizeof bad, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess && batch->num_reqs >= 0) e = launch_validate_batch(to_pool(pool), to_batch(batch), d_bad, stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof bad, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    cudaFree(d_bad);
+    if (e != cudaSuccess) return cuda_fail(e, "validate_batch");
+    g_launches = 1;
+    if (bad != 0x7fffffff) {
+        if (first_bad_request != nullptr) *first_bad_request = bad;
+        return TROPICAL_ERR_INVALID_ARG;
+    }
+    return TROPICAL_OK;
+}
+
 size_t tropical_workspace_bytes(const tropical_kv_pool_t* pool, int32_t num_reqs, int32_t total_q,
                                 int32_t max_kv_len) {
     if (pool == nullptr || num_reqs < 0 || total_q < 0 || max_kv_len < 0) return 0;

@@ -12,6 +12,7 @@ cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const voi
                              cudaStream_t stream);
 cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, int n_keys, void* k_dense,
                              void* v_dense, cudaStream_t stream);
+cudaError_t launch_validate_batch(const PoolDesc& pool, const BatchDesc& b, int* first_bad_dev, cudaStream_t stream);
 cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
                                   float scale_log2, cudaStream_t stream, bool skip_decode = false);
 cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,

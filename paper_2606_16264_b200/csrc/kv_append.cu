@@ -64,6 +64,35 @@ __global__ void __launch_bounds__(256) kv_gather_kernel(PoolDesc pool, BatchDesc
     }
 }
 
+// debug check of a batch's device arrays (tropical_validate_batch): lowest offending request index via atomicMin
+__global__ void __launch_bounds__(256) validate_batch_kernel(BatchDesc b, int num_pages, int* first_bad) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= b.num_reqs; i += gridDim.x * blockDim.x) {
+        bool bad = false;
+        if (i == b.num_reqs) {
+            bad = b.q_offsets[i] != b.total_q;
+        } else {
+            const int q = b.q_lens[i], c = b.ctx_lens[i];
+            const long long L = (long long)q + c;
+            bad = q < 0 || c < 0 || b.q_offsets[i + 1] - b.q_offsets[i] != q || (i == 0 && b.q_offsets[0] != 0) ||
+                  L > b.max_kv_len || (L + kPageSize - 1) / kPageSize > b.stride;
+            if (!bad && q > 0) {
+                const int np = (int)((L + kPageSize - 1) / kPageSize);
+                for (int p = 0; p < np; ++p) {
+                    const int page = b.page_table[(size_t)i * b.stride + p];
+                    if (page < 0 || page >= num_pages) bad = true;
+                }
+            }
+        }
+        if (bad) atomicMin(first_bad, i);
+    }
+}
+
+cudaError_t launch_validate_batch(const PoolDesc& pool, const BatchDesc& b, int* first_bad_dev, cudaStream_t stream) {
+    const int grid = (b.num_reqs + 1 + 255) / 256;
+    validate_batch_kernel<<<grid < 1 ? 1 : grid, 256, 0, stream>>>(b, pool.num_pages, first_bad_dev);
+    return cudaGetLastError();
+}
+
 static int grid_for(long long total_threads, int block) {
     long long g = (total_threads + block - 1) / block;
     const long long cap = 148LL * 8;  // grid-stride beyond 8 CTAs per SM

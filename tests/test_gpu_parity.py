@@ -356,3 +356,20 @@ def test_more_requests_than_plan_threads():
     qs[5], qs[700] = 33, 2
     cs = rng.integers(0, 40, n).tolist()
     _check_step(_step(78, 2, 2, 64, qs, cs))
+
+
+def test_validate_batch_finds_the_first_bad_request():
+    s = _step(19, 4, 2, 64, [40, 1, 1, 0, 5], [3, 100, 17, 9, 0])
+    dev = DeviceStep(s)
+    assert tb.validate_batch(dev.pool, dev.batch) is None
+    pt = dev.batch.page_table.clone()
+    dev.batch.page_table[2, 1] = s.num_pages            # page id out of range, inside request 2's extent
+    assert tb.validate_batch(dev.pool, dev.batch) == 2
+    dev.batch.page_table.copy_(pt)
+    dev.batch.page_table[3, 5] = -7                     # beyond request 3's extent: ignored (reading S8)
+    assert tb.validate_batch(dev.pool, dev.batch) is None
+    dev.batch.q_offsets[2] += 1                         # prefix sums broken at request 1
+    assert tb.validate_batch(dev.pool, dev.batch) == 1
+    dev.batch.q_offsets[2] -= 1
+    dev.batch.ctx_lens[4] = -1
+    assert tb.validate_batch(dev.pool, dev.batch) == 4
