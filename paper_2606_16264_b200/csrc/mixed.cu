@@ -269,7 +269,7 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     // serialization it overlaps the tail of a preceding tropical_kv_append (whose kernel triggers early); after any
     // other kernel it starts in normal stream order.
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(1);
+    cfg.gridDim = dim3(b.num_reqs <= kPlanStagedReqs ? 8 : 1);  // see plan_kernel: several blocks share the work lists
     cfg.blockDim = dim3(kPlanThreads);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = stream;

@@ -87,7 +87,8 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     int my_pages = 0;
     for (int i = i0; i < i1; ++i)
         if (b.q_lens[i] == 1) my_pages += (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
-    if (my_pages) atomicAdd(&s_pages, my_pages);
+    my_pages = __reduce_add_sync(0xffffffffu, my_pages);
+    if ((tid & 31) == 0 && my_pages) atomicAdd(&s_pages, my_pages);
     __syncthreads();
     const long long page_heads = (long long)s_pages * Hkv * HB;
     int split = (int)((page_heads + kTargetUnits - 1) / kTargetUnits);
@@ -130,9 +131,16 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
             info.x = 2;
             ibase += ((q + kQTile - 1) / kQTile) * ipt;
         }
-        P.req_info[i] = info;
+        if (blockIdx.x == 0) P.req_info[i] = info;
+        if (n <= kPlanStagedReqs) {  // every block keeps its own copy of the directory for the ticket search below
+            s_ub[i] = info.y;
+            s_ib[i] = info.w;
+            s_ns[i] = info.z;
+            // decode request: pages of its context; prefill request: its 128-row query tiles
+            s_pg[i] = info.x == 1 ? (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize : (q + kQTile - 1) / kQTile;
+        }
     }
-    if (tid == 0) {
+    if (tid == 0 && blockIdx.x == 0) {
         P.hdr[HDR_N_ITEMS] = n_items;
         P.hdr[HDR_N_UNITS] = n_units;
         P.hdr[HDR_SPLIT_PAGES] = split;
@@ -145,19 +153,9 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     __syncthreads();  // req_info visible to the whole block (same-block global writes + barrier)
 
     // ticket -> request: binary search over the per-request bases, staged in shared memory when they fit (the
-    // dependent global loads of the search made this kernel ~20 us for a few hundred requests)
+    // dependent global loads of the search made this kernel ~20 us for a few hundred requests); then the blocks of
+    // the grid (several only in the staged case, each with its own copy of the directory) share the two work lists
     const bool staged = n <= kPlanStagedReqs;
-    if (staged) {
-        for (int i = tid; i < n; i += kPlanThreads) {
-            const int4 v = P.req_info[i];
-            s_ub[i] = v.y;
-            s_ib[i] = v.w;
-            s_ns[i] = v.z;
-            // decode request: pages of its context; prefill request: its 128-row query tiles
-            s_pg[i] = v.x == 1 ? (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize : (b.q_lens[i] + kQTile - 1) / kQTile;
-        }
-        __syncthreads();
-    }
     auto owner = [&](const int* base_s, int field, int e) {
         if (!staged) return field == 1 ? find_owner<1>(P.req_info, n, e) : find_owner<3>(P.req_info, n, e);
         int lo = 0, hi = n;
@@ -167,7 +165,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         }
         return lo;
     };
-    for (int e = tid; e < n_units; e += kPlanThreads) {
+    for (int e = blockIdx.x * kPlanThreads + tid; e < n_units; e += gridDim.x * kPlanThreads) {
         const int i = owner(s_ub, 1, e);
         int ubase, nsplit, pages;
         if (staged) {
@@ -185,7 +183,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         P.units[e] = make_int4(i, kvh | (hb << 16), p0, min(split, pages - p0));
         P.group_cnt[e] = 0;
     }
-    for (int e = tid; e < n_items; e += kPlanThreads) {
+    for (int e = blockIdx.x * kPlanThreads + tid; e < n_items; e += gridDim.x * kPlanThreads) {
         const int i = owner(s_ib, 3, e);
         const int local = e - (staged ? s_ib[i] : P.req_info[i].w);
         const int ntile = staged ? s_pg[i] : (b.q_lens[i] + kQTile - 1) / kQTile;
