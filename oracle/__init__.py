@@ -5,6 +5,9 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 ``paper_2606_16264_b200`` and shares no code with it.  The arithmetic is in
 ``tropical_oracle.c`` (plain C, fp64); this file only marshals numpy arrays through ctypes.
 
+``sim_oracle.py`` (same rules: test infrastructure only) is the plain-Python oracle of the scheduler simulation
+(include/tropical_sim.h).
+
 Citations: PAPER.md:143, :159 (the multiplexed iteration), BASELINE.json north_star (the
 attention definition and tolerances), SURVEY.md section 8(c) (readings S1-S28).
 """
