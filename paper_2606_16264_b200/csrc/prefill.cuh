@@ -309,7 +309,10 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
 // ------------------------------------------------------------------------------------------------
 // softmax warpgroup (4 warps, 128 threads: thread r <-> query row r <-> TMEM lane r, for both query tiles)
 __device__ __forceinline__ float max4(float a, float b, float c, float d) { return fmaxf(fmaxf(a, b), fmaxf(c, d)); }
-constexpr int kPolyEvery = 4;  // every 4th pair of a chunk takes exp2_poly_x2 instead of MUFU.EX2
+// Every kPolyEvery-th pair of a chunk takes exp2_poly_x2 (FMA pipe) instead of MUFU.EX2; 0 = never.  A quarter of the
+// exponentials on the FMA pipe makes a prefill-only step 2.5 % faster at full clocks, but the mixed C5 step, which runs
+// against the board's power limit, 1 % slower (more instructions per exponential): off (profiles/r1c_c5.md section 6).
+constexpr int kPolyEvery = 0;
 
 template <int D>
 __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBars* B, int wg_warp) {
@@ -402,7 +405,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
                     float x0, x1;
                     f32x2_unpack(f32x2_fma(f32x2_pack(__uint_as_float(s[j]), __uint_as_float(s[j + 1])), sc2, nm2), x0, x1);
                     float p0, p1;
-                    if ((j >> 1) % kPolyEvery == kPolyEvery - 1) {  // a quarter of the exponentials on the FMA pipe
+                    if (kPolyEvery > 0 && (j >> 1) % (kPolyEvery > 0 ? kPolyEvery : 1) == kPolyEvery - 1) {  // optional: on the FMA pipe
                         exp2_poly_x2(x0, x1, p0, p1);
                     } else {
                         p0 = fast_exp2(x0);
