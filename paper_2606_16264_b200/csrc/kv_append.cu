@@ -1,9 +1,9 @@
 // kv_append.cu -- SURVEY.md 8(a) rows A1 (KV append) and A2 (page gather), bit-exact copies.
 //
 // A1: for t < q_i, pos = c_i + t: pool[page_table[i][pos/P]][h][pos%P][:] = new[q_off_i+t][h][:].
-// HBM-bound and tiny: T*Hkv rows of 2*d bytes each for K and V.  One thread moves one 16-byte
-// chunk; the d/8 threads of a row read and write 2*d contiguous bytes (fully coalesced on both
-// sides -- a (page, head, slot) row of the HND pool is contiguous).
+// HBM-bound and tiny: T*Hkv rows of 2*d bytes each for K and V.  One thread moves the 16-byte chunk
+// `chunk` of every kv head of one (token, K|V); the d/8 threads of a row read and write 2*d contiguous
+// bytes (fully coalesced on both sides -- a (page, head, slot) row of the HND pool is contiguous).
 #include "common.cuh"
 #include "kernels.h"
 
@@ -18,26 +18,32 @@ __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc
     // which reads only q_lens / ctx_lens) may start while this one is still copying; every other kernel keeps
     // normal stream order.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const long long total = (long long)b.total_q * pool.Hkv * CH * 2;
+    // One thread per (token, K|V, 16-byte chunk): the request lookup and the (page, slot) of the token are done once
+    // and reused for all kv heads, whose rows are copied with several independent loads in flight.
+    const long long total = (long long)b.total_q * CH * 2;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
         const int chunk = (int)(idx % CH);
         long long r = idx / CH;
         const int which = (int)(r & 1);  // 0 = K, 1 = V
-        r >>= 1;
-        const int h = (int)(r % pool.Hkv);
-        const int tok = (int)(r / pool.Hkv);
+        const int tok = (int)(r >> 1);
         const int req = find_request(b.q_offsets, b.num_reqs, tok);
         const int t = tok - __ldg(b.q_offsets + req);
         const int pos = __ldg(b.ctx_lens + req) + t;
         const int page = __ldg(b.page_table + (size_t)req * b.stride + pos / kPageSize);
         const int slot = pos % kPageSize;
-        const size_t dst = (((size_t)page * pool.Hkv + h) * kPageSize + slot) * CH + chunk;
-        const size_t src = ((size_t)tok * pool.Hkv + h) * CH + chunk;
-        if (which == 0)
-            reinterpret_cast<uint4*>(const_cast<uint16_t*>(pool.k_pool))[dst] = __ldg(k_new + src);
-        else
-            reinterpret_cast<uint4*>(const_cast<uint16_t*>(pool.v_pool))[dst] = __ldg(v_new + src);
+        const uint4* src = (which == 0 ? k_new : v_new) + (size_t)tok * pool.Hkv * CH + chunk;
+        uint4* dst = reinterpret_cast<uint4*>(const_cast<uint16_t*>(which == 0 ? pool.k_pool : pool.v_pool)) +
+                     ((size_t)page * pool.Hkv * kPageSize + slot) * CH + chunk;
+        int h = 0;
+        for (; h + 4 <= pool.Hkv; h += 4) {
+            uint4 v[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) v[k] = __ldg(src + (size_t)(h + k) * CH);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) dst[(size_t)(h + k) * kPageSize * CH] = v[k];
+        }
+        for (; h < pool.Hkv; ++h) dst[(size_t)h * kPageSize * CH] = __ldg(src + (size_t)h * CH);
     }
 }
 
@@ -104,7 +110,7 @@ static int grid_for(long long total_threads, int block) {
 cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const void* k_new, const void* v_new,
                              cudaStream_t stream) {
     if (b.total_q == 0) return cudaSuccess;
-    const long long total = (long long)b.total_q * pool.Hkv * (pool.D / 8) * 2;
+    const long long total = (long long)b.total_q * (pool.D / 8) * 2;  // threads: (token, K|V, chunk); heads looped
     const int grid = grid_for(total, 256);
     if (pool.D == 128)
         kv_append_kernel<128><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new);
