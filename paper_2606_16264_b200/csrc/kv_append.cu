@@ -12,21 +12,25 @@ namespace tropical {
 template <int D>
 __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc b,
                                                         const uint4* __restrict__ k_new,
-                                                        const uint4* __restrict__ v_new) {
+                                                        const uint4* __restrict__ v_new, int hg) {
     constexpr int CH = D / 8;  // 16-byte chunks per row
     // Programmatic dependent launch: a following kernel that opted in (the plan kernel of tropical_mixed_attention,
     // which reads only q_lens / ctx_lens) may start while this one is still copying; every other kernel keeps
     // normal stream order.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    // One thread per (token, K|V, 16-byte chunk): the request lookup and the (page, slot) of the token are done once
-    // and reused for all kv heads, whose rows are copied with several independent loads in flight.
-    const long long total = (long long)b.total_q * CH * 2;
+    // One thread per (token, group of hg kv heads, K|V, 16-byte chunk): the request lookup and the (page, slot) of the
+    // token are done once per thread and reused for its heads, whose rows are copied with several independent loads
+    // in flight.  hg is chosen by the launcher: all heads for big steps, fewer when a step has few tokens.
+    const int ngroups = (pool.Hkv + hg - 1) / hg;
+    const long long total = (long long)b.total_q * ngroups * CH * 2;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
         const int chunk = (int)(idx % CH);
         long long r = idx / CH;
         const int which = (int)(r & 1);  // 0 = K, 1 = V
-        const int tok = (int)(r >> 1);
+        r >>= 1;
+        const int h_lo = (int)(r % ngroups) * hg, h_hi = min(pool.Hkv, h_lo + hg);
+        const int tok = (int)(r / ngroups);
         const int req = find_request(b.q_offsets, b.num_reqs, tok);
         const int t = tok - __ldg(b.q_offsets + req);
         const int pos = __ldg(b.ctx_lens + req) + t;
@@ -35,15 +39,15 @@ __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc
         const uint4* src = (which == 0 ? k_new : v_new) + (size_t)tok * pool.Hkv * CH + chunk;
         uint4* dst = reinterpret_cast<uint4*>(const_cast<uint16_t*>(which == 0 ? pool.k_pool : pool.v_pool)) +
                      ((size_t)page * pool.Hkv * kPageSize + slot) * CH + chunk;
-        int h = 0;
-        for (; h + 4 <= pool.Hkv; h += 4) {
+        int h = h_lo;
+        for (; h + 4 <= h_hi; h += 4) {
             uint4 v[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) v[k] = __ldg(src + (size_t)(h + k) * CH);
 #pragma unroll
             for (int k = 0; k < 4; ++k) dst[(size_t)(h + k) * kPageSize * CH] = v[k];
         }
-        for (; h < pool.Hkv; ++h) dst[(size_t)h * kPageSize * CH] = __ldg(src + (size_t)h * CH);
+        for (; h < h_hi; ++h) dst[(size_t)h * kPageSize * CH] = __ldg(src + (size_t)h * CH);
     }
 }
 
@@ -110,12 +114,17 @@ static int grid_for(long long total_threads, int block) {
 cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const void* k_new, const void* v_new,
                              cudaStream_t stream) {
     if (b.total_q == 0) return cudaSuccess;
-    const long long total = (long long)b.total_q * (pool.D / 8) * 2;  // threads: (token, K|V, chunk); heads looped
+    // heads per thread: as many as keep >= 64K threads in flight (all of them for steps with many new tokens)
+    const long long chunks = (long long)b.total_q * pool.Hkv * (pool.D / 8) * 2;
+    long long hg = chunks / 65536;
+    if (hg < 1) hg = 1;
+    if (hg > pool.Hkv) hg = pool.Hkv;
+    const long long total = (long long)b.total_q * ((pool.Hkv + hg - 1) / hg) * (pool.D / 8) * 2;
     const int grid = grid_for(total, 256);
     if (pool.D == 128)
-        kv_append_kernel<128><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new);
+        kv_append_kernel<128><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new, (int)hg);
     else
-        kv_append_kernel<64><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new);
+        kv_append_kernel<64><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new, (int)hg);
     return cudaGetLastError();
 }
 
