@@ -179,7 +179,6 @@ def run_ours(args, rank, world):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl")
-    tb.debug_set_mode({"fused": 0, "split": 1}[args.mode])
     s, gen_s = make_workload(args.config, rank)
     cnt = step_counts((s.num_q_heads, s.num_kv_heads, s.head_dim, s.page_size, s.q_lens, s.ctx_lens))
     peaks = load_peaks()
@@ -240,7 +239,7 @@ def run_ours(args, rank, world):
         torch.cuda.synchronize()
     sampler.stop_flag = True
     sampler.join()
-    roles = tb.debug_read_profile(dev.workspace) if args.mode != "split" else None
+    roles = tb.debug_read_profile(dev.workspace)
     total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms / args.steps
     us = ms_per_step * 1e3
@@ -284,7 +283,7 @@ def run_ours(args, rank, world):
         "config": {"workload": f"{args.config} ({describe(args.config)})", "replicas": world,
                    "l2": "step touches %.2f GB >> 126 MB L2, no flush needed" % (cnt["step_bytes"] / 1e9)
                    if not flush else "L2 flushed (512 MB rewritten, untimed) between timed steps; per-step event times summed",
-                   "new_tokens_per_step": int(cnt["new_tokens"]), "mode": args.mode},
+                   "new_tokens_per_step": int(cnt["new_tokens"])},
         "tokens_per_s": round(whole_job_tokens_per_s(cnt["new_tokens"], world, us), 1),
         "step_roofline": {"t_bytes_us": round(t_bytes_us, 2), "t_flops_us": round(t_flops_us, 2),
                           "t_roof_us": round(t_roof, 2), "frac": round(t_roof / us, 4),
@@ -343,9 +342,6 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", default="C5", choices=synth.CONFIG_NAMES)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="fused", choices=["fused", "split"],
-                    help="fused = the product path (one persistent step kernel); split = separate prefill/decode "
-                         "launches of the same tile code, for A/B timing only")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))

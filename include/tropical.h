@@ -19,8 +19,10 @@
  *   - All pointers marked [device] are CUDA device pointers, [host] are host pointers.
  *   - bf16 tensors are raw 16-bit patterns (void*), row-major in the stated shape.
  *   - The library owns nothing: it allocates no device memory, frees nothing and keeps no
- *     pointer after a call returns.  Process-global state: cached device attributes,
- *     one-time cudaFuncSetAttribute, the resolved cuTensorMapEncodeTiled entry point.
+ *     pointer after a call returns.  Process-global state: per-device cached attributes
+ *     (SM count, one-time cudaFuncSetAttribute), the resolved cuTensorMapEncodeTiled entry
+ *     point.  Any number of devices per process; calls act on the current device.
+ *   - Test and measurement hooks live in tropical_debug.h, not here.
  *   - Device work is enqueued on the caller's stream (void* = cudaStream_t, NULL = legacy
  *     default stream).  No host synchronisation, no H2D/D2H inside the device-pointer calls;
  *     they are CUDA-graph capturable.  tropical_step_host is the exception (see there).
@@ -100,7 +102,12 @@ size_t tropical_workspace_bytes(const tropical_kv_pool_t *pool, int32_t num_reqs
  *   sm_scale <= 0 selects 1/sqrt(d)
  *   workspace [device] 256-byte aligned, >= tropical_workspace_bytes(...); contents are scratch.
  * Never writes the pool.  Unused slots of a request's last page may hold any bits (NaN
- * included); the result does not depend on them.  Run-to-run deterministic. */
+ * included); the result does not depend on them.  Run-to-run deterministic.
+ * Stream ordering: the first of its two launches (the tile directory) opts into programmatic dependent launch so that
+ * it overlaps a preceding tropical_kv_append; it waits for that kernel's completion before the step kernel starts.
+ * A caller kernel placed right before this call that itself triggers dependents early
+ * (griddepcontrol.launch_dependents / cudaTriggerProgrammaticLaunchCompletion) must have finished writing q_lens,
+ * ctx_lens, q_offsets and page_table before it triggers. */
 int tropical_mixed_attention(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
                              const void *q, void *out, float *lse, float sm_scale,
                              void *workspace, size_t workspace_bytes, void *cuda_stream);
@@ -109,10 +116,12 @@ int tropical_mixed_attention(const tropical_kv_pool_t *pool, const tropical_batc
  * sync (out-of-range page ids there are undefined behaviour): q_lens / ctx_lens >= 0, q_offsets the exclusive prefix
  * sum of q_lens with q_offsets[num_reqs] == total_q, ctx + q <= max_kv_len, ceil((ctx + q) / page_size) <=
  * page_table_stride, every page id a request can touch in [0, num_pages).  Runs one small kernel and synchronises
- * the stream.  Returns TROPICAL_OK, or TROPICAL_ERR_INVALID_ARG with *first_bad_request [host, nullable] = the lowest
- * offending request index (num_reqs when only the final q_offsets entry is wrong). */
+ * the stream (so it is not graph-capturable).  scratch: [device] >= 4 bytes, 4-byte aligned, caller-owned (the first
+ * bytes of the attention workspace will do); its contents are overwritten.  Returns TROPICAL_OK, or
+ * TROPICAL_ERR_INVALID_ARG with *first_bad_request [host, nullable] = the lowest offending request index (num_reqs
+ * when only the final q_offsets entry is wrong). */
 int tropical_validate_batch(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
-                            int32_t *first_bad_request, void *cuda_stream);
+                            int32_t *first_bad_request, void *scratch, void *cuda_stream);
 
 /* End-to-end step from HOST buffers (what bench.py's "e2e" times): copies this step's inputs
  * host->device into caller-provided device staging, runs append + attention, copies out back,
@@ -163,42 +172,6 @@ int tropical_step_cost(const tropical_cost_model_t *model, int32_t num_q_heads,
 /* Number of kernel launches the last tropical_kv_append / tropical_mixed_attention /
  * tropical_step_host call on this thread enqueued (bench.py's gpu_launches). */
 int tropical_last_launch_count(void);
-
-/* Test hook: the plain CUDA-core (no tensor core, no split-K) attention kernel, same arguments
- * and semantics as tropical_mixed_attention without a workspace.  Used by tests to cross-check
- * the tile kernels on the device; not a product path. */
-int tropical_debug_attention_simt(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
-                                  const void *q, void *out, float *lse, float sm_scale,
-                                  void *cuda_stream);
-
-/* Test / measurement hook: 0 (default) = the fused step kernel, prefill tiles and decode tiles in one
- * persistent launch; 1 = the same tile code as separate prefill and decode launches, kept
- * only to time the two phases apart (A/B evidence under profiles/).  Process-global. */
-void tropical_debug_set_mode(int mode);
-
-/* Test hook: cap the number of CTAs of the persistent step kernel (0 = one per SM, the default), so that small
- * test batches put MANY tiles through each CTA's queues (multi-item sequencing of every role).  Process-global. */
-void tropical_debug_set_grid(int num_ctas);
-
-/* Test hook: force the decode split size in pages (multiple of 8; 0 = automatic, from the step's page count), so
- * that small test batches exercise multi-block decode units.  Process-global. */
-void tropical_debug_set_split_pages(int pages);
-
-/* Measurement / debugging hook, only in special builds (else TROPICAL_ERR_UNSUPPORTED).  Synchronises the device.
- *  -DTROPICAL_WAIT_PROF: cycles spent in and calls of every mbarrier wait of the step kernel, summed over warps,
- *    indexed by the wait's tag (the numbers next to the mbar_wait calls in csrc/); reset != 0 zeroes the counters.
- *  -DTROPICAL_DEBUG_WAIT: instead of trapping after ~2 s, a wait that is stuck for ~0.2 s raises an abort flag that
- *    lets every wait fall through (the step finishes with garbage); cycles[0] = that flag and, for warp w of CTA 0,
- *    cycles[16 + 3 w .. + 2] = tag, parity and aux value of the wait it was stuck in.  The record lives in
- *    host-mapped memory, so it can be read even when the kernel faulted afterwards.
- * cycles / calls are [host] arrays of n <= 512 entries. */
-int tropical_debug_wait_profile(uint64_t *cycles, uint64_t *calls, int32_t n, int32_t reset);
-
-/* Measurement hook: role timestamps of the LAST fused step kernel that ran with this workspace
- * (globaltimer nanoseconds): out_ns[0] kernel start (earliest CTA), [1] prefill queue drained (latest
- * softmax warp), [2] latest dedicated decode warp done, [3] latest late-joining decode warp done.
- * Copies 32 bytes device->host and synchronises the stream.  out_ns is [host]. */
-int tropical_debug_read_profile(const void *workspace, uint64_t *out_ns, void *cuda_stream);
 
 const char *tropical_status_string(int status);
 const char *tropical_last_cuda_error(void); /* thread-local text of the last CUDA failure */

@@ -238,7 +238,8 @@ def simulate(cfg: Config, requests: List[tuple]):
             if target < 0:  # Path 1, or the no-starvation rule once the TTFT slack is gone
                 best = min(range(np_), key=lambda w: (pred_queue(w), w))
                 slack_ttft = cfg.ttft_slo_us - waited
-                if slack_ttft <= 0 or pred_exec(r) + pred_queue(best) < slack_ttft:
+                slack_gone = now >= R[r].arrival + cfg.ttft_slo_us  # the expression the wake-up event is scheduled with
+                if slack_gone or pred_exec(r) + pred_queue(best) < slack_ttft:
                     target = best
             if target >= 0:
                 toggle_q.remove(r)
@@ -285,8 +286,10 @@ def simulate(cfg: Config, requests: List[tuple]):
 
     results = []
     for x in R:
-        assert x.finish >= 0, "request never finished"
-        results.append(dict(ttft_us=x.first_token - x.arrival, tpot_us=(x.finish - x.first_token) / max(1, x.output - 1),
+        # a request the run never served violates both SLOs (guard; the model's rules serve every request)
+        ttft = INF if x.first_token < 0 else x.first_token - x.arrival
+        tpot = INF if x.finish < 0 else (x.finish - x.first_token) / max(1, x.output - 1)
+        results.append(dict(ttft_us=ttft, tpot_us=tpot,
                             first_token_us=x.first_token, finish_us=x.finish, prefill_worker=x.prefill_worker,
                             decode_worker=x.decode_worker, multiplexed=x.multiplexed))
     return results, summarize(cfg, results, iterations)

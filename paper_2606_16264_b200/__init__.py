@@ -16,7 +16,6 @@ from .binding import (  # noqa: F401
     TropicalError,
     debug_attention_simt,
     debug_read_profile,
-    debug_set_mode,
     debug_set_grid,
     debug_set_split_pages,
     debug_wait_profile,

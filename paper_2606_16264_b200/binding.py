@@ -78,7 +78,7 @@ EXPORTS = (
     "tropical_kv_append", "tropical_kv_gather", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
-    "tropical_debug_attention_simt", "tropical_debug_set_mode", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile",
+    "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile",
     "tropical_sim_run",
 )
 
@@ -117,11 +117,6 @@ def status_string(status: int) -> str:
 
 def version() -> str:
     return lib().tropical_version().decode()
-
-
-def debug_set_mode(mode: int) -> None:
-    """0 = fused step kernel (default, the product path); 1 = separate prefill / decode launches (timing A/B)."""
-    lib().tropical_debug_set_mode(ctypes.c_int(int(mode)))
 
 
 def debug_set_grid(num_ctas: int) -> None:
@@ -240,11 +235,15 @@ def kv_gather(pool: KVPool, batch: Batch, req: int, n_keys: int, stream=None):
     return kd, vd
 
 
-def validate_batch(pool: KVPool, batch: Batch, stream=None):
-    """Opt-in debug check of the batch's device arrays (syncs).  Returns None if valid, else the first bad request."""
+def validate_batch(pool: KVPool, batch: Batch, scratch: Optional[torch.Tensor] = None, stream=None):
+    """Opt-in debug check of the batch's device arrays (syncs).  Returns None if valid, else the first bad request.
+    scratch: any CUDA tensor of >= 4 bytes (e.g. the attention workspace); allocated here when omitted."""
     bad = ctypes.c_int32(-1)
     p, b = pool.c(), batch.c()
-    rc = lib().tropical_validate_batch(ctypes.byref(p), ctypes.byref(b), ctypes.byref(bad), _stream(stream))
+    if scratch is None:
+        scratch = torch.empty(1, dtype=torch.int32, device=batch.q_lens.device)
+    rc = lib().tropical_validate_batch(ctypes.byref(p), ctypes.byref(b), ctypes.byref(bad), _ptr(scratch),
+                                       _stream(stream))
     if rc == 1 and bad.value >= 0:
         return bad.value
     _check(rc, "tropical_validate_batch")

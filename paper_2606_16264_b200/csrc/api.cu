@@ -6,6 +6,7 @@
 #include <string.h>
 
 #include "../../include/tropical.h"
+#include "../../include/tropical_debug.h"
 #include "kernels.h"
 
 using namespace tropical;
@@ -124,23 +125,20 @@ int tropical_kv_gather(const tropical_kv_pool_t* pool, const tropical_batch_t* b
 }
 
 int tropical_validate_batch(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, int32_t* first_bad_request,
-                            void* cuda_stream) {
+                            void* scratch, void* cuda_stream) {
     g_launches = 0;
     int rc = check_pool(pool);
     if (rc != TROPICAL_OK) return rc;
     rc = check_batch(pool, batch);
     if (rc != TROPICAL_OK) return rc;
-    if (batch->num_reqs > 0 && batch->q_offsets == nullptr) return TROPICAL_ERR_INVALID_ARG;
+    if (scratch == nullptr || ((uintptr_t)scratch & 3)) return TROPICAL_ERR_WORKSPACE;
     cudaStream_t stream = (cudaStream_t)cuda_stream;
-    int* d_bad = nullptr;  // the one call of this library that allocates: a debug aid, 4 bytes, freed before it returns
-    cudaError_t e = cudaMalloc((void**)&d_bad, sizeof(int));
-    if (e != cudaSuccess) return cuda_fail(e, "validate_batch alloc");
+    int* d_bad = (int*)scratch;  // caller-owned: the library allocates nothing
     int bad = 0x7fffffff;
-    e = cudaMemcpyAsync(d_bad, &bad, sizeof bad, cudaMemcpyHostToDevice, stream);
-    if (e == cudaSuccess && batch->num_reqs >= 0) e = launch_validate_batch(to_pool(pool), to_batch(batch), d_bad, stream);
+    cudaError_t e = cudaMemcpyAsync(d_bad, &bad, sizeof bad, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = launch_validate_batch(to_pool(pool), to_batch(batch), d_bad, stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, d_bad, sizeof bad, cudaMemcpyDeviceToHost, stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
-    cudaFree(d_bad);
     if (e != cudaSuccess) return cuda_fail(e, "validate_batch");
     g_launches = 1;
     if (bad != 0x7fffffff) {
@@ -291,8 +289,6 @@ int tropical_debug_read_profile(const void* workspace, uint64_t* out_ns, void* c
     if (e != cudaSuccess) return cuda_fail(e, "read_profile");
     return TROPICAL_OK;
 }
-
-void tropical_debug_set_mode(int mode) { set_debug_mode(mode == 1 ? 1 : 0); }
 
 void tropical_debug_set_grid(int num_ctas) { set_debug_grid(num_ctas); }
 

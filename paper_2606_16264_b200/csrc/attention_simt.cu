@@ -1,8 +1,8 @@
 // attention_simt.cu -- the plain CUDA-core attention kernel: one warp per (new token, q head) row,
 // online softmax over 32-key chunks, keys spread over lanes for QK^T and head-dim spread over
 // lanes for PV.  It is the first correct CUDA path and stays as the in-library cross-check for
-// the tensor-core tile kernels (tests call it through tropical_debug_attention_simt); the
-// product entry point only routes here for shapes the tile kernels do not cover.
+// the tensor-core tile kernels: tests call it through tropical_debug_attention_simt
+// (include/tropical_debug.h).  No product entry point ever routes here.
 //
 // Definition followed: SURVEY.md 8(c) phase 2 -- row (i, t, hq): keys j <= c_i + t of kv head
 // hq / (Hq/Hkv), s_j = scale * q.k_j, out = softmax(s) V, lse = m + ln Z.
@@ -17,7 +17,7 @@ template <int D>
 __global__ void __launch_bounds__(kSimtWarps * 32) attention_simt_kernel(PoolDesc pool, BatchDesc b,
                                                                          const uint16_t* __restrict__ q,
                                                                          uint16_t* __restrict__ out,
-                                                                         float* __restrict__ lse, float scale_log2, int skip_decode) {
+                                                                         float* __restrict__ lse, float scale_log2) {
     constexpr int EPL = D / 32;  // output elements per lane (4 at d=128, 2 at d=64)
     __shared__ float q_s[kSimtWarps][D];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -28,7 +28,6 @@ __global__ void __launch_bounds__(kSimtWarps * 32) attention_simt_kernel(PoolDes
          row += (long long)gridDim.x * kSimtWarps) {
         const int tok = (int)(row / pool.Hq), hq = (int)(row % pool.Hq), hk = hq / g;
         const int req = find_request(b.q_offsets, b.num_reqs, tok);
-        if (skip_decode && __ldg(b.q_lens + req) == 1) continue;  // decode rows belong to the decode tiles
         const int t = tok - __ldg(b.q_offsets + req);
         const int n = __ldg(b.ctx_lens + req) + t + 1;  // visible keys
         const int* pt = b.page_table + (size_t)req * b.stride;
@@ -112,17 +111,17 @@ __global__ void __launch_bounds__(kSimtWarps * 32) attention_simt_kernel(PoolDes
 }
 
 cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
-                                  float scale_log2, cudaStream_t stream, bool skip_decode) {
+                                  float scale_log2, cudaStream_t stream) {
     const long long n_rows = (long long)b.total_q * pool.Hq;
     if (n_rows == 0) return cudaSuccess;
     long long grid = (n_rows + kSimtWarps - 1) / kSimtWarps;
     if (grid > 148LL * 64) grid = 148LL * 64;
     if (pool.D == 128)
         attention_simt_kernel<128><<<(int)grid, kSimtWarps * 32, 0, stream>>>(pool, b, (const uint16_t*)q,
-                                                                              (uint16_t*)out, lse, scale_log2, skip_decode ? 1 : 0);
+                                                                              (uint16_t*)out, lse, scale_log2);
     else
         attention_simt_kernel<64><<<(int)grid, kSimtWarps * 32, 0, stream>>>(pool, b, (const uint16_t*)q,
-                                                                             (uint16_t*)out, lse, scale_log2, skip_decode ? 1 : 0);
+                                                                             (uint16_t*)out, lse, scale_log2);
     return cudaGetLastError();
 }
 

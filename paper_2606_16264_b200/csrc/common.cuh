@@ -61,26 +61,6 @@ __device__ __forceinline__ uint64_t f32x2_add(uint64_t a, uint64_t b) {
     return r;
 }
 
-// 2^x for a pair on the FMA pipe instead of MUFU.EX2 (the softmax inner loop is MUFU-bound: 16 ex2 / clk / SM):
-// round-to-nearest split x = i + f with the 1.5 * 2^23 trick, cubic for 2^f on [-0.5, 0.5] (relative error
-// < 7e-4, well under the bf16 rounding of P; exactly 1 at f = 0), exponent added with an integer shift.
-// Inputs are clamped to >= -126; inputs above ~120 (only ever seen on the speculative path whose result is
-// discarded) give garbage.
-__device__ __forceinline__ void exp2_poly_x2(float x0, float x1, float& p0, float& p1) {
-    const uint64_t magic = f32x2_pack(12582912.f, 12582912.f), nmagic = f32x2_pack(-12582912.f, -12582912.f);
-    const uint64_t x2 = f32x2_pack(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
-    const uint64_t r2 = f32x2_add(x2, magic);
-    const uint64_t f2 = f32x2_fma(f32x2_add(r2, nmagic), f32x2_pack(-1.f, -1.f), x2);
-    uint64_t q2 = f32x2_fma(f2, f32x2_pack(0.0555041f, 0.0555041f), f32x2_pack(0.2402265f, 0.2402265f));
-    q2 = f32x2_fma(q2, f2, f32x2_pack(0.6931472f, 0.6931472f));
-    q2 = f32x2_fma(q2, f2, f32x2_pack(1.f, 1.f));
-    float r0, r1, q0, q1;
-    f32x2_unpack(r2, r0, r1);
-    f32x2_unpack(q2, q0, q1);
-    p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(r0) << 23));
-    p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(r1) << 23));
-}
-
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
@@ -135,7 +115,7 @@ static __device__ int g_wait_abort_info[8];
 static __device__ int* g_wait_stuck;  // host-mapped [16][3] (readable after a fault): per warp of block 0, the wait it was in (tag, parity, aux)
 #endif
 
-// Bounded wait: a protocol bug traps (launch failure) instead of hanging the GPU box.
+// Bounded wait: a protocol bug traps (launch failure, TROPICAL_ERR_CUDA at the next call) instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0, int aux = 0) {
 #ifdef TROPICAL_WAIT_PROF
     const long long tp = clock64();
@@ -172,7 +152,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int ta
                 break;
             }
 #else
-            if (clock64() - t0 > 4000000000LL) __trap();  // ~2 s at 1.9 GHz
+#ifndef TROPICAL_NO_WAIT_TRAP
+            // ~20 s at 1.9 GHz: far beyond any legitimate wait even under time-slicing or MPS (a step takes < 1 ms);
+            // build with -DTROPICAL_NO_WAIT_TRAP to wait forever (debugger sessions)
+            if (clock64() - t0 > 40000000000LL) __trap();
+#endif
 #endif
         }
     }
@@ -336,41 +320,10 @@ __device__ __forceinline__ void tmem_st_32x32_x16(uint32_t taddr, const uint32_t
         : "memory");
 }
 
-// 32 lanes x 8 consecutive 32-bit columns (decode tiles: one thread per key / per d row, 8 heads)
-__device__ __forceinline__ void tmem_ld_32x32_x8(uint32_t taddr, uint32_t (&r)[8]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr)
-                 : "memory");
-}
-__device__ __forceinline__ void tmem_st_32x32_x8(uint32_t taddr, const uint32_t (&r)[8]) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
-                 : "memory");
-}
-
-// ---------------------------------------------------------------- warpgroup-scope helpers (decode softmax)
-__device__ __forceinline__ float warp_max_f32(float v) {  // one CREDUX on sm_100a
-    float m;
-    asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(m) : "f"(v));
-    return m;
-}
+// ---------------------------------------------------------------- named barriers
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("barrier.cta.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
-// OR of a predicate over the `nthreads` threads that meet at named barrier `id`
-__device__ __forceinline__ bool named_bar_or(int id, int nthreads, bool pred) {
-    uint32_t r;
-    asm volatile(
-        "{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %3, 0;\n\t"
-        "barrier.cta.red.or.pred q, %1, %2, p;\n\t"
-        "selp.u32 %0, 1, 0, q;\n\t}"
-        : "=r"(r)
-        : "r"(id), "r"(nthreads), "r"((uint32_t)pred)
-        : "memory");
-    return r != 0;
-}
-
 // K-major / MN-major SWIZZLE_128B shared-memory matrix descriptor (sm_100 format, version 1).
 //   bits [0,14) start>>4, [16,30) LBO>>4, [32,46) SBO>>4, [46,48) version=1, [61,64) layout (2 = SW128)
 __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {

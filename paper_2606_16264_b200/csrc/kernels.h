@@ -14,10 +14,9 @@ cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, 
                              void* v_dense, cudaStream_t stream);
 cudaError_t launch_validate_batch(const PoolDesc& pool, const BatchDesc& b, int* first_bad_dev, cudaStream_t stream);
 cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
-                                  float scale_log2, cudaStream_t stream, bool skip_decode = false);
+                                  float scale_log2, cudaStream_t stream);
 cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
                                    float scale_log2, void* workspace, cudaStream_t stream, int* launches);
-void set_debug_mode(int mode);
 void set_debug_grid(int num_ctas);
 void set_debug_split_pages(int pages);
 int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset);

@@ -1,6 +1,8 @@
-// mixed.cu -- kernels of tropical_mixed_attention: plan (A0), decode tiles (A4), combine (A5),
-// prefill tiles (A3) and their launchers.
+// mixed.cu -- tropical_mixed_attention: the plan launch (A0) and the fused persistent step kernel that runs the prefill
+// tiles (A3), the decode tiles (A4) and the combine (A5) side by side.
 #include <cuda.h>
+
+#include <atomic>
 
 #include "common.cuh"
 #include "decode.cuh"
@@ -10,9 +12,6 @@
 #include "tma_host.h"
 
 namespace tropical {
-
-constexpr int kDecodeWarps = 4;
-constexpr int kDecodeRingBytes = 24576;  // per decode warp: 6 page-head stages at d = 128
 
 __device__ __forceinline__ DecodeRing make_ring(uint8_t* base, uint64_t* bars, int nst) {
     DecodeRing R;
@@ -34,62 +33,6 @@ __device__ __forceinline__ unsigned long long global_ns() {
 __device__ __forceinline__ void prof_mark(const int* hdr, int which, bool is_min) {
     unsigned long long* p = reinterpret_cast<unsigned long long*>(const_cast<int*>(hdr) + HDR_PROF) + which;
     if (is_min) atomicMin(p, global_ns()); else atomicMax(p, global_ns());
-}
-
-template <int D>
-__global__ void __launch_bounds__(kDecodeWarps * 32, 2)
-decode_kernel(DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
-    using C = DecodeCfg<D>;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kDecodeWarps * kDecodeRingBytes);
-    constexpr int NST = kDecodeRingBytes / C::PAGE_BYTES;
-    static_assert(NST <= kMaxDecodeStages, "stage barriers");
-    const int warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) {
-        tma_prefetch_desc(&tm_k);
-        tma_prefetch_desc(&tm_v);
-        for (int i = 0; i < kDecodeWarps * NST; ++i) mbar_init(bars + i, 1);
-        fence_mbar_init();
-    }
-    __syncthreads();
-    DecodeRing R = make_ring(smem + warp * kDecodeRingBytes, bars + warp * NST, NST);
-    decode_warp_worker<D>(A, &tm_k, &tm_v, R);
-}
-
-
-constexpr int kPrefillThreads = 224;  // warps 0-3 softmax, 4 K producer, 5 MMA issuer, 6 V producer
-
-template <int D>
-__global__ void __launch_bounds__(kPrefillThreads, 1)
-prefill_kernel(PrefillArgs A, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-               const __grid_constant__ CUtensorMap tm_v) {
-    using C = PrefillCfg<D>;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    PrefillBars* B = reinterpret_cast<PrefillBars*>(tiles + C::SMEM_TILES);
-    const int warp = uni((int)(threadIdx.x >> 5));
-    if (threadIdx.x == 0) {
-        tma_prefetch_desc(&tm_q);
-        tma_prefetch_desc(&tm_k);
-        tma_prefetch_desc(&tm_v);
-        prefill_init_bars(B);
-        fence_mbar_init();
-    }
-    if (warp == 0) {
-        tmem_alloc(&B->tmem_base, C::TM_COLS);
-        tmem_relinquish();
-    }
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    if (warp < 4) prefill_softmax<D>(A, B, warp);
-    else if (warp == 4) prefill_producer<D, 0>(A, B, tiles, &tm_q, &tm_k);
-    else if (warp == 5) prefill_mma<D>(A, B, tiles);
-    else prefill_producer<D, 1>(A, B, tiles, &tm_q, &tm_v);
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 0) tmem_dealloc(B->tmem_base, C::TM_COLS);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -175,15 +118,29 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
     if (warp == 0) tmem_dealloc(PB->tmem_base, C::TM_COLS);
 }
 
-static int g_num_sms = 0;
-static int num_sms() {
-    if (g_num_sms == 0) {
+// Per-device one-time state (cudaFuncSetAttribute and the SM count are properties of a device, not of the process).
+constexpr int kMaxDevices = 64;
+struct DeviceState {
+    std::atomic<int> num_sms{0};
+    std::atomic<int> smem_attr_set{0};  // bit 0: mixed_kernel<128>, bit 1: mixed_kernel<64>
+};
+static DeviceState g_dev[kMaxDevices];
+
+static DeviceState& device_state() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return g_dev[(dev >= 0 && dev < kMaxDevices) ? dev : 0];
+}
+
+static int num_sms(DeviceState& ds) {
+    int n = ds.num_sms.load(std::memory_order_relaxed);
+    if (n == 0) {
         int dev = 0;
         cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-        if (g_num_sms <= 0) g_num_sms = 148;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        ds.num_sms.store(n, std::memory_order_relaxed);
     }
-    return g_num_sms;
+    return n;
 }
 
 size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q) {
@@ -192,9 +149,7 @@ size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q) 
 
 size_t profile_offset_bytes() { return make_layout(1, 1, 64, 1, 1).hdr + HDR_PROF * sizeof(int); }
 
-static int g_mode = 0;  // 0: fused step kernel (product path); 1: separate prefill / decode launches (A/B timing only)
-void set_debug_mode(int mode) { g_mode = mode; }
-static int g_grid_cap = 0;  // test hook: 0 = one CTA per SM
+static std::atomic<int> g_grid_cap{0};     // test hook (include/tropical_debug.h): 0 = one CTA per SM
 #ifdef TROPICAL_DEBUG_WAIT
 static volatile int* g_stuck_host = nullptr;
 static void debug_wait_setup() {
@@ -250,9 +205,9 @@ int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int
 #endif
 }
 
-static int g_split_pages = 0;  // test hook: 0 = automatic
-void set_debug_split_pages(int pages) { g_split_pages = pages > 0 ? (pages + 7) / 8 * 8 : 0; }
-void set_debug_grid(int num_ctas) { g_grid_cap = num_ctas > 0 ? num_ctas : 0; }
+static std::atomic<int> g_split_pages{0};  // test hook: 0 = automatic
+void set_debug_split_pages(int pages) { g_split_pages.store(pages > 0 ? (pages + 7) / 8 * 8 : 0); }
+void set_debug_grid(int num_ctas) { g_grid_cap.store(num_ctas > 0 ? num_ctas : 0); }
 
 template <int D>
 static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
@@ -266,8 +221,11 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     P.units = (int4*)(ws + w.units);
     P.group_cnt = (int*)(ws + w.group_cnt);
     // The plan reads only the step's metadata and writes only the workspace: launched with programmatic stream
-    // serialization it overlaps the tail of a preceding tropical_kv_append (whose kernel triggers early); after any
-    // other kernel it starts in normal stream order.
+    // serialization it overlaps a preceding tropical_kv_append (whose kernel triggers at once), and its last
+    // statement is griddepcontrol.wait, so the step kernel behind it -- a normal launch -- starts only after the
+    // append has completed.  After a kernel that never triggers it starts in normal stream order.  Contract for
+    // callers (include/tropical.h): a preceding kernel that triggers early must not still be writing q_lens /
+    // ctx_lens / q_offsets / page_table.
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(b.num_reqs <= kPlanStagedReqs ? 8 : 1);  // see plan_kernel: several blocks share the work lists
     cfg.blockDim = dim3(kPlanThreads);
@@ -278,7 +236,7 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, plan_kernel, b, pool.Hq, pool.Hkv, P, g_split_pages);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, plan_kernel, b, pool.Hq, pool.Hkv, P, g_split_pages.load(std::memory_order_relaxed));
     if (e != cudaSuccess) return e;
     ++*launches;
 
@@ -316,50 +274,20 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
 #ifdef TROPICAL_DEBUG_WAIT
     debug_wait_setup();
 #endif
-    if (g_mode == 0) {
-        // A3 + A4 in one persistent launch: the product path
-        const size_t smem = MixedCfg<D>::SMEM;
-        static bool attr_m = false;
-        if (!attr_m) {
-            e = cudaFuncSetAttribute(mixed_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            attr_m = true;
-        }
-        mixed_kernel<D><<<(g_grid_cap > 0 && g_grid_cap < num_sms()) ? g_grid_cap : num_sms(), kMixedThreads, smem, stream>>>(
-            PA, A, tm_q, tm_k, tm_v);
-        e = cudaGetLastError();
+    // A3 + A4 + A5 in one persistent launch
+    DeviceState& ds = device_state();
+    const size_t smem = MixedCfg<D>::SMEM;
+    const int attr_bit = D == 128 ? 1 : 2;
+    if (!(ds.smem_attr_set.load(std::memory_order_acquire) & attr_bit)) {
+        e = cudaFuncSetAttribute(mixed_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        ++*launches;
-    } else {
-        // A3: prefill tiles (q_i >= 2) on tcgen05
-        const size_t smem_p = (size_t)PrefillCfg<D>::SMEM_TILES + sizeof(PrefillBars) + 1024;
-        static bool attr_p = false;
-        if (!attr_p) {
-            e = cudaFuncSetAttribute(prefill_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p);
-            if (e != cudaSuccess) return e;
-            attr_p = true;
-        }
-        int grid_p = (b.total_q / 2) * pool.Hq;  // upper bound of items worth a CTA; every q_i >= 2 row pair
-        if (grid_p > num_sms()) grid_p = num_sms();
-        if (grid_p > 0) {
-            prefill_kernel<D><<<grid_p, kPrefillThreads, smem_p, stream>>>(PA, tm_q, tm_k, tm_v);
-            e = cudaGetLastError();
-            if (e != cudaSuccess) return e;
-            ++*launches;
-        }
-        // A4: decode tiles
-        const size_t smem = (size_t)kDecodeWarps * kDecodeRingBytes + 1024 + 1024;
-        static bool attr_done = false;
-        if (!attr_done) {
-            e = cudaFuncSetAttribute(decode_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            attr_done = true;
-        }
-        decode_kernel<D><<<2 * num_sms(), kDecodeWarps * 32, smem, stream>>>(A, tm_k, tm_v);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        ++*launches;
+        ds.smem_attr_set.fetch_or(attr_bit, std::memory_order_release);
     }
+    const int cap = g_grid_cap.load(std::memory_order_relaxed), sms = num_sms(ds);
+    mixed_kernel<D><<<(cap > 0 && cap < sms) ? cap : sms, kMixedThreads, smem, stream>>>(PA, A, tm_q, tm_k, tm_v);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    ++*launches;
 
     return cudaSuccess;
 }

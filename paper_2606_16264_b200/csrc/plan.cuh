@@ -14,7 +14,7 @@ constexpr int kTargetUnits = 9472;   // ~8 decode units per resident decode warp
 constexpr int kMinSplitPages = 8;    // never split finer than 128 tokens
 
 enum { HDR_N_ITEMS = 0, HDR_N_UNITS = 1, HDR_SPLIT_PAGES = 2, HDR_TICKET_PREFILL = 3, HDR_TICKET_DECODE = 4,
-       HDR_N_COMBINE = 5, HDR_PROF = 16 /* 4 x u64: kernel start (min), prefill end, WG1 decode end, WG0 decode end (max) */,
+       HDR_PROF = 16 /* 4 x u64: kernel start (min), prefill end, WG1 decode end, WG0 decode end (max) */,
        HDR_INTS = 64 };
 
 // req_info[i] = {kind, unit_base, nsplit, item_base}; kind 0 skip, 1 decode, 2 prefill
@@ -94,7 +94,8 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     int split = (int)((page_heads + kTargetUnits - 1) / kTargetUnits);
     if (split < kMinSplitPages) split = kMinSplitPages;
     split = (split + 7) / 8 * 8;  // whole 128-key blocks: only a request's last unit is ragged
-    if (forced_split > 0) split = forced_split;  // test hook (workspace sizing assumes split >= 8)
+    // test hook: coarser splits only -- make_layout's max_units bound holds for split >= the automatic value
+    if (forced_split > split) split = forced_split;
 
     int my_units = 0, my_items = 0;
     for (int i = i0; i < i1; ++i) {
@@ -190,6 +191,12 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         const int qt = ntile - 1 - local / ipt;  // heaviest (most KV tiles) first
         P.items[e] = make_int2(i, (qt << 16) | (pair << 15) | ((local % ipt) << pair));
     }
+    // Programmatic dependent launch: this kernel may have started while the kernel before it on the stream (the
+    // append, which triggers at its first instruction) was still running.  The step kernel is launched in normal
+    // stream order behind this one and reads what the append wrote, so completion of the plan must imply completion
+    // and visibility of the append: griddepcontrol.wait returns once every prerequisite grid has completed and its
+    // memory is flushed (PTX ISA, griddepcontrol); it is a no-op when there is no programmatic dependency.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 }  // namespace tropical

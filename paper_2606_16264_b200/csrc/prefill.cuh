@@ -309,11 +309,6 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
 // ------------------------------------------------------------------------------------------------
 // softmax warpgroup (4 warps, 128 threads: thread r <-> query row r <-> TMEM lane r, for both query tiles)
 __device__ __forceinline__ float max4(float a, float b, float c, float d) { return fmaxf(fmaxf(a, b), fmaxf(c, d)); }
-// Every kPolyEvery-th pair of a chunk takes exp2_poly_x2 (FMA pipe) instead of MUFU.EX2; 0 = never.  A quarter of the
-// exponentials on the FMA pipe makes a prefill-only step 2.5 % faster at full clocks, but the mixed C5 step, which runs
-// against the board's power limit, 1 % slower (more instructions per exponential): off (profiles/r1c_c5.md section 6).
-constexpr int kPolyEvery = 0;
-
 template <int D>
 __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBars* B, int wg_warp) {
     using C = PrefillCfg<D>;
@@ -404,13 +399,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
                 for (int j = 0; j < 32; j += 2) {
                     float x0, x1;
                     f32x2_unpack(f32x2_fma(f32x2_pack(__uint_as_float(s[j]), __uint_as_float(s[j + 1])), sc2, nm2), x0, x1);
-                    float p0, p1;
-                    if (kPolyEvery > 0 && (j >> 1) % (kPolyEvery > 0 ? kPolyEvery : 1) == kPolyEvery - 1) {  // optional: on the FMA pipe
-                        exp2_poly_x2(x0, x1, p0, p1);
-                    } else {
-                        p0 = fast_exp2(x0);
-                        p1 = fast_exp2(x1);
-                    }
+                    const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
                     cs2 = f32x2_add(cs2, f32x2_pack(p0, p1));
                     pk[j >> 1] = pack_bf16x2(p0, p1);
                 }

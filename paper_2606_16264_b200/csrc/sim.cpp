@@ -214,7 +214,10 @@ struct Sim {
             if (target < 0) {  // Path 1, or the no-starvation rule once the TTFT slack is gone
                 const int best = least_queue_prefill_worker();
                 const double slack_ttft = cfg.ttft_slo_us - waited;
-                if (slack_ttft <= 0 || pred_exec(r) + pred_queue(best) < slack_ttft) target = best;
+                // the no-starvation rule fires on the very expression the wake-up below is scheduled with: testing
+                // `slack_ttft <= 0` instead can miss it by one rounding of (now - arrival)
+                const bool slack_gone = now >= R[r].arrival + cfg.ttft_slo_us;
+                if (slack_gone || pred_exec(r) + pred_queue(best) < slack_ttft) target = best;
             }
             if (target >= 0) {
                 toggle_q.erase(std::find(toggle_q.begin(), toggle_q.end(), r));
@@ -291,8 +294,9 @@ extern "C" int tropical_sim_run(const tropical_sim_config_t* cfg, int32_t n, con
     int64_t ok = 0, mux = 0;
     for (int i = 0; i < n; ++i) {
         const Req& x = S.R[i];
-        ttft[i] = x.first_token - x.arrival;
-        tpot[i] = (x.finish - x.first_token) / (double)std::max(1, x.output - 1);
+        // a request the run never served (cannot happen under the model's rules; kept as a guard) violates both SLOs
+        ttft[i] = x.first_token < 0 ? kInf : x.first_token - x.arrival;
+        tpot[i] = x.finish < 0 ? kInf : (x.finish - x.first_token) / (double)std::max(1, x.output - 1);
         if (ttft[i] <= cfg->ttft_slo_us && tpot[i] <= cfg->tpot_slo_us) ++ok;  // eq. (1)-(3)
         mux += x.multiplexed;
         makespan = std::max(makespan, x.finish);

@@ -1,5 +1,5 @@
 """CPU-side checks of the C-ABI library: it loads without a GPU, exports every symbol
-include/tropical.h declares, validates host-visible arguments before touching CUDA, and its
+include/*.h declares, validates host-visible arguments before touching CUDA, and its
 step-cost feature arithmetic matches hand-derived counts (tests/golden/step_cost_features.txt)."""
 import ctypes
 import os
@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared_functions():
-    text = open(os.path.join(ROOT, "include", "tropical.h")).read() + open(os.path.join(ROOT, "include", "tropical_sim.h")).read()
+    text = "".join(open(os.path.join(ROOT, "include", h)).read() for h in sorted(os.listdir(os.path.join(ROOT, "include"))) if h.endswith(".h"))
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(tropical_[a-z_0-9]+)\s*\(", text)))
 

@@ -222,41 +222,17 @@ def test_product_path_matches_simt_cross_check():
     assert np.abs(a - b).max() <= 2e-2 and np.abs(la - lb).max() <= 2e-3
 
 
-def test_split_launch_mode_matches_fused():
-    """The A/B timing mode (separate prefill / decode launches) runs the same tile code: same bits."""
-    s = _step(16, 16, 2, 128, [300, 1, 1, 1, 40], [0, 777, 4097, 15, 130])
-    dev = DeviceStep(s)
-    dev.step()
-    a = bits(dev.out).copy()
-    for mode in (1,):
-        tb.debug_set_mode(mode)
-        try:
-            dev.out.zero_()
-            dev.attention()
-            torch.cuda.synchronize()
-            b = bits(dev.out).copy()
-        finally:
-            tb.debug_set_mode(0)
-        if mode == 1:
-            assert np.array_equal(a, b)
-        assert np.array_equal(a[:300], b[:300]) and np.array_equal(a[303:], b[303:])
-        fa, fb = synth.bf16_bits_to_f32(a).astype(np.float64), synth.bf16_bits_to_f32(b).astype(np.float64)
-        assert np.abs(fa - fb).max() <= 2e-2
-
-
 # ------------------------------------------------------------------ queue sequencing: many tiles per CTA
-@pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("split", [0, 16, 24, 64])
 @pytest.mark.parametrize("grid", [1, 2, 5])
 @pytest.mark.parametrize("shape", [(8, 1, 128), (16, 2, 128), (4, 4, 64)])
-def test_few_ctas_many_tiles_per_queue(grid, shape, split, mode):
+def test_few_ctas_many_tiles_per_queue(grid, shape, split):
     """With the step kernel capped to a few CTAs every role walks long sequences of prefill items and decode
     units (ring wrap-around, mailbox and barrier phases, TMEM slot reuse, both decode pipelines of a CTA)."""
     Hq, Hkv, d = shape
     qs = [300, 1, 1, 1, 1, 40, 1, 1, 1, 1, 1, 1]
     cs = [0, 777, 4097, 15, 130, 100, 2000, 128, 127, 1, 513, 3000]
     s = _step(20 + grid, Hq, Hkv, d, qs, cs)
-    tb.debug_set_mode(mode)  # 0 = product kernel; 1 = separate prefill / decode launches (grid cap applies to 0 only)
     tb.debug_set_grid(grid)
     tb.debug_set_split_pages(split)  # 0 = automatic (one 128-key block per unit at these sizes); else multi-block units
     try:
@@ -265,7 +241,6 @@ def test_few_ctas_many_tiles_per_queue(grid, shape, split, mode):
         s2 = _step(30 + grid, Hq, Hkv, d, [1] * 9, [5000, 3000, 17, 900, 256, 255, 4096, 64, 2500])
         _check_step(s2)
     finally:
-        tb.debug_set_mode(0)
         tb.debug_set_grid(0)
         tb.debug_set_split_pages(0)
 
