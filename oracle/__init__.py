@@ -90,6 +90,20 @@ def kv_gather(k_pool, v_pool, page_table, req: int, n_keys: int) -> Tuple[np.nda
     return kd, vd
 
 
+def kv_migrate(k_src, v_src, k_dst, v_dst, kv_lens, src_page_table, dst_page_table) -> None:
+    """In-place migration of the first kv_lens[m] tokens of every request m from the source pools (through
+    src_page_table) into the destination pools (under dst_page_table): tropical_oracle.c: oracle_kv_migrate."""
+    k_src, v_src, k_dst, v_dst = _u16(k_src), _u16(v_src), _u16(k_dst), _u16(v_dst)
+    assert k_dst.flags.writeable and v_dst.flags.writeable
+    _, Hkv, P, d = k_src.shape
+    assert k_dst.shape[1:] == (Hkv, P, d)
+    kv_lens, src_page_table, dst_page_table = _i32(kv_lens), _i32(src_page_table), _i32(dst_page_table)
+    _load().oracle_kv_migrate(
+        ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(P), ctypes.c_int(kv_lens.shape[0]), _p(kv_lens),
+        _p(src_page_table), ctypes.c_int(src_page_table.shape[1]), _p(dst_page_table),
+        ctypes.c_int(dst_page_table.shape[1]), _p(k_src), _p(v_src), _p(k_dst), _p(v_dst))
+
+
 def attention_rows(k_pool, v_pool, q, q_lens, ctx_lens, q_offsets, page_table,
                    rows: Sequence[Tuple[int, int]], sm_scale: float = 0.0, want_wsum: bool = False):
     """fp64 attention for chosen (request, new-token index) rows; all q heads of each row.

@@ -18,7 +18,8 @@
  *
  * Pins (tests/test_oracle_pins.py): brute-force dense attention, torch fp64 SDPA, closed
  * forms, row-sum-to-one, page-size and page-permutation invariance, chunk/decode
- * consistency, needle selection.  Step-cost model: not in this file (parity unpinned, see
+ * consistency, needle selection; kv_migrate: gather(dst) == gather(src) by fancy indexing, changed-row
+ * count, attention unchanged by the move.  Step-cost model: not in this file (parity unpinned, see
  * DESIGN.md).
  *
  * Layouts (host pointers, bf16 carried as uint16 bit patterns):
@@ -92,6 +93,35 @@ void oracle_kv_gather(int Hkv, int d, int P, const int32_t *page_table, int stri
             for (int c = 0; c < d; ++c) {
                 k_dense[dst + c] = k_pool[src + c];
                 v_dense[dst + c] = v_pool[src + c];
+            }
+        }
+    }
+}
+
+/* KV migration (PAPER.md:155 Path 1: after its prefill on a prefill worker a request
+ * re-enters through the decode queue and its KV cache moves to the multiplexing worker that will decode it;
+ * PAPER.md:58, :101 "migration of KVCache"; :171 P2P between GPUs).  The paper fixes nothing below "the cache
+ * moves"; the reading is token-granular and page-table to page-table:
+ *   for request m, j < kv_lens[m], h < Hkv:
+ *     dst_pool[dst_pt[m][j / P]][h][j % P][:] = src_pool[src_pt[m][j / P]][h][j % P][:]      (K and V)
+ * Raw 16-bit copies.  Slots j >= kv_lens[m] of a destination page and every other destination page keep
+ * their bits; the source pools are read-only. */
+void oracle_kv_migrate(int Hkv, int d, int P, int num_reqs, const int32_t *kv_lens,
+                       const int32_t *src_pt, int src_stride, const int32_t *dst_pt, int dst_stride,
+                       const uint16_t *k_src, const uint16_t *v_src, uint16_t *k_dst, uint16_t *v_dst)
+{
+    for (int m = 0; m < num_reqs; ++m) {
+        for (int64_t j = 0; j < kv_lens[m]; ++j) {
+            int64_t sp = src_pt[(int64_t)m * src_stride + j / P];
+            int64_t dp = dst_pt[(int64_t)m * dst_stride + j / P];
+            int64_t slot = j % P;
+            for (int h = 0; h < Hkv; ++h) {
+                int64_t so = ((sp * Hkv + h) * P + slot) * d;
+                int64_t dof = ((dp * Hkv + h) * P + slot) * d;
+                for (int c = 0; c < d; ++c) {
+                    k_dst[dof + c] = k_src[so + c];
+                    v_dst[dof + c] = v_src[so + c];
+                }
             }
         }
     }

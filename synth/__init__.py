@@ -17,6 +17,7 @@ from .workloads import (  # noqa: F401
     config_lengths,
     f32_to_bf16_bits,
     make_config,
+    make_migration_target,
     make_step,
     needed_pages,
 )

@@ -237,3 +237,27 @@ def make_config(name: str, *, poison: bool = True, values: str = "normal") -> St
     num_pages = 64 if name == "C1" else None
     return make_step(rng, Hq, Hkv, d, P, q_lens, ctx_lens, num_pages=num_pages, poison=poison,
                      values=values, name=name, seed=seed)
+
+
+# ----------------------------------------------------------------------------- KV migration
+def make_migration_target(rng, kv_lens: Sequence[int], page_size: int, *, num_pages: Optional[int] = None,
+                          shuffle_pages: bool = True):
+    """Destination side of a KV migration (PAPER.md:155 Path 1: the cache of a prefilled request moves to the
+    worker that will decode it): a page table into a second pool for requests holding kv_lens[m] tokens.
+    Returns (dst_page_table int32 [n, stride] with -1 past ceil(len/P), num_dst_pages).  Placement only."""
+    kv_lens = np.asarray(kv_lens, np.int64)
+    pages_per_req = (kv_lens + page_size - 1) // page_size
+    need = int(pages_per_req.sum())
+    if num_pages is None:
+        num_pages = 64 * max(1, math.ceil(1.25 * need / 64))
+    assert num_pages >= need, "destination pool too small"
+    perm = rng.permutation(num_pages) if shuffle_pages else np.arange(num_pages)
+    n = int(kv_lens.shape[0])
+    stride = max(1, int(pages_per_req.max()) if n else 1)
+    table = np.full((n, stride), -1, np.int32)
+    used = 0
+    for m in range(n):
+        k = int(pages_per_req[m])
+        table[m, :k] = perm[used:used + k]
+        used += k
+    return table, int(num_pages)

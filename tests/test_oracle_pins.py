@@ -9,6 +9,7 @@ O6 closed forms                                                       pin O6
 O7 chunk / decode / GQA consistency                                   pin O7
 O8 needle: the softmax selects exactly one key                        pin O8
 +  append vs python loops, gather vs fancy indexing, whole-pool stray-write check.
++  kv_migrate (NEXT-3): destination gathers equal source gathers, changed-row count, identity, attention invariance.
 """
 import math
 
@@ -73,6 +74,59 @@ def test_gather_matches_fancy_indexing():
         assert np.array_equal(vd, gather_dense(vp, s.page_table[i], n))
         # the tail of the gathered K is exactly this step's new rows
         assert np.array_equal(kd[int(s.ctx_lens[i]):], s.k_new[s.q_offsets[i]:s.q_offsets[i + 1]])
+
+
+# ------------------------------------------------------------------ KV migration (NEXT-3; PAPER.md:155 Path 1, :58)
+def _migration_case(seed, Hkv, d, kv_lens, P=16):
+    """A source step whose pools already hold kv_lens[m] tokens per request (contexts only), a poisoned destination
+    pool of a different size and a fresh random destination page table."""
+    rng = np.random.default_rng(seed)
+    s = synth.make_step(rng, Hkv, Hkv, d, P, [0] * len(kv_lens), kv_lens)
+    dst_pt, n_dst = synth.make_migration_target(rng, kv_lens, P)
+    kd = np.full((n_dst, Hkv, P, d), synth.POISON_BF16, np.uint16)
+    return s, dst_pt, kd, kd.copy()
+
+
+def test_migrate_gather_of_destination_equals_gather_of_source():
+    kv_lens = [1, 15, 16, 17, 100, 0, 255]
+    s, dst_pt, kd, vd = _migration_case(21, 3, 64, kv_lens)
+    k_src, v_src = s.copy_pools()
+    oracle.kv_migrate(s.k_pool, s.v_pool, kd, vd, kv_lens, s.page_table, dst_pt)
+    assert np.array_equal(s.k_pool, k_src) and np.array_equal(s.v_pool, v_src)      # the source is read-only
+    for m, n in enumerate(kv_lens):                                                  # numpy fancy indexing, not the oracle's gather
+        assert np.array_equal(gather_dense(kd, dst_pt[m], n), gather_dense(s.k_pool, s.page_table[m], n))
+        assert np.array_equal(gather_dense(vd, dst_pt[m], n), gather_dense(s.v_pool, s.page_table[m], n))
+    # exactly sum(kv_lens) * Hkv destination rows changed (every other slot still holds the poison pattern): token-granular,
+    # nothing past a request's last token, no stray page
+    assert ((kd != synth.POISON_BF16).any(axis=-1)).sum() == sum(kv_lens) * 3
+    assert ((vd != synth.POISON_BF16).any(axis=-1)).sum() == sum(kv_lens) * 3
+    # K went to K and V to V (the generator draws them differently)
+    assert not np.array_equal(gather_dense(kd, dst_pt[4], 100), gather_dense(s.v_pool, s.page_table[4], 100))
+
+
+def test_migrate_is_the_identity_when_both_tables_name_the_same_pages():
+    kv_lens = [40, 7]
+    s, _, _, _ = _migration_case(22, 2, 64, kv_lens)
+    kd, vd = np.full_like(s.k_pool, synth.POISON_BF16), np.full_like(s.v_pool, synth.POISON_BF16)
+    oracle.kv_migrate(s.k_pool, s.v_pool, kd, vd, kv_lens, s.page_table, s.page_table)
+    # the installed context rows are the only non-poison rows of the source as well
+    assert np.array_equal(kd, s.k_pool) and np.array_equal(vd, s.v_pool)
+
+
+def test_attention_is_unchanged_by_a_migration():
+    """Decoding on the destination worker sees the same cache: fp64 outputs bit-identical (same j order)."""
+    rng = np.random.default_rng(23)
+    s = synth.make_step(rng, 4, 2, 64, 16, [1, 1, 1], [33, 16, 250])
+    kp, vp = s.copy_pools()
+    oracle.kv_append(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new)
+    L = (s.q_lens + s.ctx_lens).tolist()
+    dst_pt, n_dst = synth.make_migration_target(rng, L, 16)
+    kd = np.full((n_dst, 2, 16, 64), synth.POISON_BF16, np.uint16)
+    vd = kd.copy()
+    oracle.kv_migrate(kp, vp, kd, vd, L, s.page_table, dst_pt)
+    a, la = oracle.mixed_attention(kp, vp, s.q, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table)
+    b, lb = oracle.mixed_attention(kd, vd, s.q, s.q_lens, s.ctx_lens, s.q_offsets, dst_pt)
+    assert np.array_equal(a, b) and np.array_equal(la, lb)
 
 
 # ------------------------------------------------------------------ O1 / O2
