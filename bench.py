@@ -1,16 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- one multiplexed-iteration step (KV append + mixed prefill/decode attention) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C5] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C5|C1..C4|MIG] [--impl ours|reference]
 
-Prints ONE JSON line (contract in the task prompt).  metric = BASELINE.json's "mixed prefill+decode
-attention step us"; `value` = device-timed us per step with inputs resident in HBM; `e2e` = the same
-step through tropical_step_host with pinned HOST buffers (H2D/D2H inside the timed region);
-`roofline` = the attention kernel against the measured HBM peak; `cpu_baseline` = the fp64 oracle
-timed on this box's host cores on a bounded sample of the same workload.
+Prints ONE JSON line (contract in the task prompt).  metric = BASELINE.json's "mixed prefill+decode attention step
+us"; `value` = device-timed us per step over EXACTLY K back-to-back steps with inputs resident in HBM; `e2e` = the
+same step through tropical_step_host with pinned HOST buffers (H2D/D2H inside the timed region); `roofline` = the
+attention launches against the measured HBM peak; `cpu_baseline` = the fp64 oracle timed on this box's host cores.
 
-N > 1 (torchrun): the path shards by request with no collective; each rank
-runs its own replica of the workload (weak scaling), timing = max over ranks.
+Beyond the contract the line carries: `us_per_step` (median / min / max of per-step event times from a second,
+instrumented pass over the same steps), `sustained` (the same step in a >= 2 s back-to-back loop: C5 runs against
+the board's power limit and the clocks it holds after ~100 ms are lower than in a short burst), fractions against
+the nominal peaks, and -- on the default run -- `extra.C4` (the other "mixed config" of the 70 % bar) and
+`extra.MIG` (KV migration).  `--config MIG` makes the migration the line's own workload.
+
+N > 1 (torchrun): the path shards by request with no collective; each rank runs its own
+replica of the workload (weak scaling), timing = max over ranks.
 """
 from __future__ import annotations
 
@@ -30,11 +35,16 @@ import synth  # noqa: E402
 
 METRIC = "mixed prefill+decode attention step time"
 UNIT = "us"
+NOMINAL = dict(hbm_gbs=8000.0, bf16_tflops=2250.0)  # B200 data sheet, dense
 
 
 # ----------------------------------------------------------------------------- roofline arithmetic
 def step_counts(s_or_lengths):
-    """FLOPs / algorithmic bytes of a step; attention-kernel bytes separately."""
+    """FLOPs / algorithmic bytes of a step; the attention call's share separately.
+
+    step_bytes: prior K+V read once, new K/V rows read and written once, Q read, O written, page table.
+    attn_bytes: what of that belongs to tropical_mixed_attention: prior K+V, Q, O, page table.  The re-read of this
+    step's new rows from the pool (4 Hkv d T) is an implementation cost, not algorithmic (reading S21)."""
     Hq, Hkv, d, P, q, c = s_or_lengths
     q = q.astype(np.float64)
     c = c.astype(np.float64)
@@ -42,8 +52,8 @@ def step_counts(s_or_lengths):
     L = q + c
     pages = np.ceil(L[q > 0] / P).sum()
     flops = 4.0 * d * Hq * (q * c + q * (q + 1) / 2).sum()
-    step_bytes = 4.0 * Hkv * d * c.sum() + 2 * (4.0 * Hkv * d * T) + 2 * (2.0 * Hq * d * T) + 4.0 * pages
-    attn_bytes = 4.0 * Hkv * d * L[q > 0].sum() + 2 * (2.0 * Hq * d * T) + 4.0 * pages
+    step_bytes = 4.0 * Hkv * d * c[q > 0].sum() + 2 * (4.0 * Hkv * d * T) + 2 * (2.0 * Hq * d * T) + 4.0 * pages
+    attn_bytes = 4.0 * Hkv * d * c[q > 0].sum() + 2 * (2.0 * Hq * d * T) + 4.0 * pages
     return dict(flops=flops, step_bytes=step_bytes, attn_bytes=attn_bytes, new_tokens=T)
 
 
@@ -57,7 +67,7 @@ def load_peaks():
 
 
 def ncu_traffic(config: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the step kernel, one launch, from the committed ncu capture
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one launch, from the committed ncu capture
     of this config (profiles/ncu_traffic.csv; the .md beside it names the command); None when there is none."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(path):
@@ -67,6 +77,13 @@ def ncu_traffic(config: str):
         if f and f[0] == config:
             return float(f[1])
     return None
+
+
+def roofline_times(cnt, peaks):
+    t_bytes = cnt["step_bytes"] / (peaks["hbm_gbs"] * 1e3)
+    t_flops = cnt["flops"] / (peaks["bf16_tflops_sustained"] * 1e6)
+    t_nom = max(cnt["step_bytes"] / (NOMINAL["hbm_gbs"] * 1e3), cnt["flops"] / (NOMINAL["bf16_tflops"] * 1e6))
+    return t_bytes, t_flops, max(t_bytes, t_flops), t_nom
 
 
 # ----------------------------------------------------------------------------- clocks sampler
@@ -103,6 +120,11 @@ class ClockSampler(threading.Thread):
             except Exception:
                 pass
             time.sleep(self.period)
+
+    def finish(self):
+        self.stop_flag = True
+        self.join()
+        return self.summary()
 
     def summary(self):
         if not self.samples:
@@ -157,7 +179,6 @@ def whole_job_tokens_per_s(new_tokens_per_replica: float, world: int, us_per_ste
     return new_tokens_per_replica * world / (us_per_step * 1e-6)
 
 
-# ----------------------------------------------------------------------------- main legs
 def make_workload(name: str, rank: int):
     t0 = time.perf_counter()
     if rank == 0:
@@ -169,82 +190,115 @@ def make_workload(name: str, rank: int):
     return s, time.perf_counter() - t0
 
 
-def run_ours(args, rank, world):
-    import torch
-    import torch.distributed as dist
-    import paper_2606_16264_b200 as tb
-    from paper_2606_16264_b200.harness import DeviceStep
+def describe(name):
+    return {"C1": "tiny mixed 4/4/64", "C2": "decode-only 32/32/128 x64", "C3": "prefill-only 32/32/128 x4",
+            "C4": "mixed 13B-like 40/40/128: 2048 chunk + 128 decodes",
+            "C5": "mixed GQA 64/8/128: 4096+1024 chunks + 256 decodes",
+            "MIG": "KV migration of the C5 cache (258 requests, 64/8/128) pool -> pool under a new page table"}[name]
 
-    local = int(os.environ.get("LOCAL_RANK", 0))
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl")
-    s, gen_s = make_workload(args.config, rank)
-    cnt = step_counts((s.num_q_heads, s.num_kv_heads, s.head_dim, s.page_size, s.q_lens, s.ctx_lens))
-    peaks = load_peaks()
-    dev = DeviceStep(s)
-    stream = torch.cuda.current_stream()
 
-    def one_step(ev=None):
+# ----------------------------------------------------------------------------- timing of the attention step
+class StepTimer:
+    """The step of one config on the current device: append + attention through the C-ABI binding."""
+
+    def __init__(self, s, tb, torch):
+        from paper_2606_16264_b200.harness import DeviceStep
+        self.s, self.tb, self.torch = s, tb, torch
+        self.cnt = step_counts((s.num_q_heads, s.num_kv_heads, s.head_dim, s.page_size, s.q_lens, s.ctx_lens))
+        self.dev = DeviceStep(s)
+        self.stream = torch.cuda.current_stream()
+        # A step whose working set fits the 126 MB L2 is timed cold: a 512 MB buffer is rewritten between timed steps
+        # (untimed) and the per-step event times are summed.  The big configs (> 0.5 GB per step) need no flush.
+        self.flush = self.cnt["step_bytes"] < 5e8
+        self.flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda") if self.flush else None
+        self.launches_per_step = 0
+
+    def one_step(self, ev=None):
+        tb, dev = self.tb, self.dev
+        if ev is not None:
+            ev[0].record(self.stream)
         tb.kv_append(dev.pool, dev.batch, dev.k_new, dev.v_new)
         n = tb.last_launch_count()
         if ev is not None:
-            ev[0].record(stream)
+            ev[1].record(self.stream)
         tb.mixed_attention(dev.pool, dev.batch, dev.q, out=dev.out, workspace=dev.workspace)
         n += tb.last_launch_count()
         if ev is not None:
-            ev[1].record(stream)
+            ev[2].record(self.stream)
+        self.launches_per_step = n
         return n
 
-    for _ in range(max(args.warmup, 3)):
-        launches_per_step = one_step()
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    # A step whose working set fits the 126 MB L2 is timed cold: a 512 MB buffer is rewritten between timed steps
-    # (untimed) and the per-step event times are summed.  The big configs (> 0.5 GB per step) need no flush.
-    flush = cnt["step_bytes"] < 5e8
-    flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda") if flush else None
-    sampler = ClockSampler(local)
-    sampler.start()
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    st_evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record(stream)
-    for k in range(args.steps):  # the timed region: exactly K steps, nothing but the two library calls per step
-        if flush:
-            flush_buf.fill_(k & 0xff)
-            st_evs[k][0].record(stream)
-        one_step()
-        if flush:
-            st_evs[k][1].record(stream)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    total_ms = sum(a.elapsed_time(b) for a, b in st_evs) if flush else e0.elapsed_time(e1)
-    # second pass, same steps: an event between the append and the attention call isolates the attention launches
-    # for the per-kernel roofline (kept out of the timed region: the event breaks the plan kernel's overlap with
-    # the append)
-    n_k = min(args.steps, 50)
-    for k in range(n_k):
-        if flush:
-            flush_buf.fill_(k & 0xff)
-        one_step(evs[k])
-    torch.cuda.synchronize()
-    attn_ms = sum(a.elapsed_time(b) for a, b in evs[:n_k]) / n_k
-    if total_ms < 400:  # keep the GPU busy long enough for the clock sampler to see it under load
-        t_end = time.perf_counter() + 0.4
-        while time.perf_counter() < t_end:
-            one_step()
-        torch.cuda.synchronize()
-    sampler.stop_flag = True
-    sampler.join()
-    roles = tb.debug_read_profile(dev.workspace)
-    total_ms = max_over_ranks(total_ms, world, "cuda")
-    ms_per_step = total_ms / args.steps
-    us = ms_per_step * 1e3
+    def warm(self, n):
+        for _ in range(max(n, 3)):
+            self.one_step()
+        self.torch.cuda.synchronize()
 
-    # ---- e2e through tropical_step_host (pinned host buffers, H2D + D2H inside the timed region)
+    def timed(self, steps):
+        """EXACTLY `steps` steps between two events (per-step events summed when the L2 is flushed in between)."""
+        torch = self.torch
+        ev = lambda: torch.cuda.Event(enable_timing=True)
+        st = [(ev(), ev()) for _ in range(steps)] if self.flush else None
+        e0, e1 = ev(), ev()
+        torch.cuda.synchronize()
+        e0.record(self.stream)
+        for k in range(steps):
+            if self.flush:
+                self.flush_buf.fill_(k & 0xff)
+                st[k][0].record(self.stream)
+            self.one_step()
+            if self.flush:
+                st[k][1].record(self.stream)
+        e1.record(self.stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in st) if self.flush else e0.elapsed_time(e1)
+
+    def instrumented(self, steps):
+        """Second pass over the same steps with events around every step and between its two calls: per-step times
+        (median / min / max) and the attention launches' share.  Kept out of the timed region: the event between the
+        append and the attention breaks the tile directory's overlap with the append."""
+        torch = self.torch
+        ev = lambda: torch.cuda.Event(enable_timing=True)
+        evs = [(ev(), ev(), ev()) for _ in range(steps)]
+        for k in range(steps):
+            if self.flush:
+                self.flush_buf.fill_(k & 0xff)
+            self.one_step(evs[k])
+        torch.cuda.synchronize()
+        step_us = np.array([a.elapsed_time(c) for a, _, c in evs]) * 1e3
+        attn_us = np.array([b.elapsed_time(c) for _, b, c in evs]) * 1e3
+        return step_us, attn_us
+
+    def sustained(self, seconds, local):
+        """The step back to back for >= `seconds`: what a long-running worker sees once the power management has
+        settled (C5 runs against the 1000 W board limit; a 50 ms burst holds higher clocks)."""
+        torch = self.torch
+        if self.flush:
+            return None
+        sampler = ClockSampler(local)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n, t_end = 0, time.perf_counter() + seconds
+        torch.cuda.synchronize()
+        # settle first (untimed), then time the second half
+        while time.perf_counter() < t_end - seconds / 2:
+            for _ in range(20):
+                self.one_step()
+            torch.cuda.synchronize()
+        e0.record(self.stream)
+        while time.perf_counter() < t_end:
+            for _ in range(20):
+                self.one_step()
+            n += 20
+            torch.cuda.synchronize()
+        e1.record(self.stream)
+        torch.cuda.synchronize()
+        clk = sampler.finish()
+        return dict(us=e0.elapsed_time(e1) * 1e3 / n, steps=n, seconds=seconds, clocks=clk)
+
+
+def e2e_host_step(st: StepTimer, steps, world):
+    """The step through tropical_step_host: pinned host buffers, H2D + D2H inside the timed region."""
+    torch, tb, s, dev = st.torch, st.tb, st.s, st.dev
     pin = lambda a: torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).pin_memory()
     h = dict(ql=pin(s.q_lens), cl=pin(s.ctx_lens), qo=pin(s.q_offsets), pt=pin(s.page_table), q=pin(s.q),
              k=pin(s.k_new), v=pin(s.v_new))
@@ -256,58 +310,269 @@ def run_ours(args, rank, world):
     for _ in range(3):
         host_step()
     torch.cuda.synchronize()
-    e2e_steps = max(3, min(args.steps, 50))
+    n = max(3, min(steps, 50))
     t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+    for _ in range(n):
         host_step()
-    e2e_us = (time.perf_counter() - t0) / e2e_steps * 1e6
-    e2e_us = max_over_ranks(e2e_us, world, "cuda")
+    us = (time.perf_counter() - t0) / n * 1e6
+    us = max_over_ranks(us, world, "cuda")
     h2d = sum(int(h[k].numel() * h[k].element_size()) for k in h)
-    d2h = int(h_out.numel() * 2)
+    return us, h2d, int(h_out.numel() * 2)
 
+
+# ----------------------------------------------------------------------------- KV migration (NEXT-3)
+class MigrationTimer:
+    """The cache of every request of a step after its append (L_i tokens each) moves from the step's pool into a second
+    pool under a fresh random page table: tropical_kv_migrate."""
+
+    def __init__(self, s, tb, torch, dst_device=None, src_pools=None):
+        from paper_2606_16264_b200.harness import to_dev
+        self.s, self.tb, self.torch = s, tb, torch
+        self.L = (s.q_lens.astype(np.int64) + s.ctx_lens).astype(np.int32)
+        self.dst_pt, n_dst = synth.make_migration_target(np.random.default_rng(77), self.L, s.page_size)
+        self.k_src, self.v_src = src_pools if src_pools is not None else (to_dev(s.k_pool), to_dev(s.v_pool))
+        self.src = tb.KVPool(self.k_src, self.v_src, s.num_q_heads)
+        shape = (n_dst, s.num_kv_heads, s.page_size, s.head_dim)
+        dd = dst_device if dst_device is not None else torch.cuda.current_device()
+        self.k_dst = torch.zeros(shape, dtype=torch.int16, device=f"cuda:{dd}")
+        self.v_dst = torch.zeros(shape, dtype=torch.int16, device=f"cuda:{dd}")
+        self.dst = tb.KVPool(self.k_dst, self.v_dst, s.num_q_heads)
+        self.lens_d, self.spt, self.dpt = to_dev(self.L), to_dev(s.page_table), to_dev(self.dst_pt)
+        self.max_len = int(self.L.max())
+        self.tokens = int(self.L.sum())
+        # K + V, read once from the source pool and written once to the destination pool, + the two page tables
+        self.bytes = 2.0 * (4.0 * s.num_kv_heads * s.head_dim * self.tokens) + 8.0 * float(np.ceil(self.L / s.page_size).sum())
+        self.stream = torch.cuda.current_stream()
+
+    def call(self):
+        self.tb.kv_migrate(self.src, self.dst, self.lens_d, self.spt, self.dpt, self.max_len)
+        return self.tb.last_launch_count()
+
+    def timed(self, steps, warmup):
+        torch = self.torch
+        n = 0
+        for _ in range(max(3, warmup)):
+            n = self.call()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(self.stream)
+        for _ in range(steps):
+            self.call()
+        e1.record(self.stream)
+        torch.cuda.synchronize()
+        total_ms = e0.elapsed_time(e1)
+        for a, b in evs:
+            a.record(self.stream)
+            self.call()
+            b.record(self.stream)
+        torch.cuda.synchronize()
+        per = np.array([a.elapsed_time(b) for a, b in evs]) * 1e3
+        return total_ms, per, n
+
+
+def migration_report(s, tb, torch, steps, warmup, peaks, local, world, src_pools=None):
+    mt = MigrationTimer(s, tb, torch, src_pools=src_pools)
+    sampler = ClockSampler(local)
+    sampler.start()
+    total_ms, per, launches = mt.timed(steps, warmup)
+    clk = sampler.finish()
+    us = max_over_ranks(total_ms * 1e3 / steps, world, "cuda")
+    rep = dict(us=us, per=per, launches=launches, clocks=clk, bytes=mt.bytes, tokens=mt.tokens,
+               gbs=mt.bytes / (us * 1e3), frac=mt.bytes / (us * 1e3) / peaks["hbm_gbs"])
+    # the peer path: the same call with the destination pool on a second GPU, pushed over NVLink (P:171)
+    if world == 1 and torch.cuda.device_count() >= 2:
+        peer = torch.cuda.current_device() ^ 1
+        if tb.enable_peer_access(peer):
+            mp = MigrationTimer(s, tb, torch, dst_device=peer, src_pools=(mt.k_src, mt.v_src))
+            k = max(3, steps // 4)
+            p_ms, _, _ = mp.timed(k, 3)
+            p_us = p_ms * 1e3 / k
+            rep["peer"] = {"us": round(p_us, 1), "link_gbs_one_direction": round(mt.bytes / 2 / (p_us * 1e3), 1),
+                           "dst_device": peer}
+        else:
+            rep["peer"] = "not measured: no peer path between the visible GPUs"
+    else:
+        rep["peer"] = ("not measured: one GPU visible to this process (same kernel; the destination pointers would be "
+                       "peer-mapped memory)")
+    return mt, rep
+
+
+# ----------------------------------------------------------------------------- main legs
+def run_ours(args, rank, world):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_16264_b200 as tb
+
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    peaks = load_peaks()
+    if args.config == "MIG":
+        return run_migration(args, rank, world, local, tb, torch, dist, peaks)
+    s, gen_s = make_workload(args.config, rank)
+    st = StepTimer(s, tb, torch)
+    cnt = st.cnt
+    warm = max(args.warmup, 3)
+    st.warm(warm)
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    total_ms = st.timed(args.steps)                # the timed region: exactly K steps, nothing but the two library calls
+    n_k = min(args.steps, 100)
+    step_us, attn_us = st.instrumented(n_k)
+    roles = tb.debug_read_profile(st.dev.workspace)  # of the LAST launch of the instrumented pass
+    if total_ms < 400:  # keep the GPU busy long enough for the clock sampler to see it under load
+        t_end = time.perf_counter() + 0.4
+        while time.perf_counter() < t_end:
+            st.one_step()
+        torch.cuda.synchronize()
+    clocks = sampler.finish()
+    total_ms = max_over_ranks(total_ms, world, "cuda")
+    ms_per_step = total_ms / args.steps
+    us = ms_per_step * 1e3
+    sus = st.sustained(args.sustain_seconds, local) if args.sustain_seconds > 0 else None
+    e2e_us, h2d, d2h = e2e_host_step(st, args.steps, world)
+
+    extra = {}
+    if args.config == "C5" and not args.no_extra and world == 1:
+        extra = run_extras(args, tb, torch, peaks, local, st)
     if rank != 0:
         return
-    t_bytes_us = cnt["step_bytes"] / (peaks["hbm_gbs"] * 1e3)
-    t_flops_us = cnt["flops"] / (peaks["bf16_tflops_sustained"] * 1e6)
-    t_roof = max(t_bytes_us, t_flops_us)
-    attn_us = attn_ms * 1e3
-    achieved = cnt["attn_bytes"] / (attn_us * 1e3)  # GB/s
+    t_bytes_us, t_flops_us, t_roof, t_nom = roofline_times(cnt, peaks)
+    attn_med = float(np.median(attn_us))
+    achieved = cnt["attn_bytes"] / (attn_med * 1e3)  # GB/s
     if args.no_cpu:
         cpu_us, cpu_desc, cores = float("nan"), "skipped (--no-cpu)", 0
     else:
         cpu_us, cpu_desc, cores, _ = oracle_sample_us(s)
     line = {
         "metric": METRIC, "value": round(us, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 5), "higher_is_better": False,
+        "warmup": warm, "ms_per_step": round(ms_per_step, 5), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": f"{args.config} ({describe(args.config)})", "replicas": world,
                    "l2": "step touches %.2f GB >> 126 MB L2, no flush needed" % (cnt["step_bytes"] / 1e9)
-                   if not flush else "L2 flushed (512 MB rewritten, untimed) between timed steps; per-step event times summed",
+                   if not st.flush else "L2 flushed (512 MB rewritten, untimed) between timed steps; per-step event times summed",
                    "new_tokens_per_step": int(cnt["new_tokens"])},
         "tokens_per_s": round(whole_job_tokens_per_s(cnt["new_tokens"], world, us), 1),
+        "us_per_step": {"mean_timed_region": round(us, 2), "median": round(float(np.median(step_us)), 2),
+                        "min": round(float(step_us.min()), 2), "max": round(float(step_us.max()), 2),
+                        "of": f"{n_k} per-step event pairs, second pass (rank 0)"},
         "step_roofline": {"t_bytes_us": round(t_bytes_us, 2), "t_flops_us": round(t_flops_us, 2),
                           "t_roof_us": round(t_roof, 2), "frac": round(t_roof / us, 4),
+                          "frac_of_nominal_peaks": round(t_nom / us, 4), "t_roof_nominal_us": round(t_nom, 2),
                           "achieved_gbs": round(cnt["step_bytes"] / (us * 1e3), 1),
                           "achieved_tflops": round(cnt["flops"] / (us * 1e6), 1),
-                          "peaks": peaks},
-        "roofline": {"bound": "hbm", "kernel": "launches of tropical_mixed_attention: plan + persistent step kernel (>= 95 % of it)",
+                          "peaks": peaks, "nominal": NOMINAL},
+        "roofline": {"bound": "hbm",
+                     "kernel": "launches of tropical_mixed_attention: tile directory + persistent step kernel (>= 95 % of it)",
                      "achieved": round(achieved, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
                      "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": ncu_traffic(args.config),
-                     "kernel_us": round(attn_us, 2), "algorithmic_bytes": cnt["attn_bytes"], "of": peaks["source"]},
+                     "kernel_us": round(attn_med, 2), "kernel_us_min": round(float(attn_us.min()), 2),
+                     "kernel_share_of_step": round(float(np.median(attn_us / step_us)), 4),
+                     "algorithmic_bytes": cnt["attn_bytes"], "of": peaks["source"],
+                     "timing": f"median of {n_k} event pairs around the attention call, second pass"},
         "cpu_baseline": {"value": round(cpu_us, 1), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc},
         "e2e": {"value": round(e2e_us, 2), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": int(launches_per_step) * args.steps,
-        "clocks": sampler.summary(),
+        "gpu_launches": int(st.launches_per_step) * args.steps,
+        "clocks": clocks,
         "gen_seconds": round(gen_s, 1),
-        "role_finish_us": {k: round(v / 1e3, 1) for k, v in roles.items()} if roles else None,
+        "role_finish_us": dict({k: round(v / 1e3, 1) for k, v in roles.items()},
+                               launch="last step kernel of the second (instrumented) pass"),
     }
+    if sus is not None:
+        line["sustained"] = {"value": round(sus["us"], 2), "unit": UNIT, "frac": round(t_roof / sus["us"], 4),
+                             "steps": sus["steps"], "clocks": sus["clocks"],
+                             "how": f"back to back for {sus['seconds']:.1f} s, second half timed"}
+    if extra:
+        line["extra"] = extra
     print(json.dumps(line))
 
 
-def describe(name):
-    return {"C1": "tiny mixed 4/4/64", "C2": "decode-only 32/32/128 x64", "C3": "prefill-only 32/32/128 x4",
-            "C4": "mixed 13B-like 40/40/128: 2048 chunk + 128 decodes",
-            "C5": "mixed GQA 64/8/128: 4096+1024 chunks + 256 decodes"}[name]
+def run_extras(args, tb, torch, peaks, local, st_c5):
+    """On the default (C5) run: the other mixed config of the 70 % bar, and the KV migration of the C5 cache."""
+    extra = {}
+    steps = min(args.steps, 100)
+    try:  # NEXT-3 on the pools that are already resident (they hold the step's rows: the timed steps appended them)
+        _, rep = migration_report(st_c5.s, tb, torch, steps, 3, peaks, local, 1,
+                                  src_pools=(st_c5.dev.k_pool, st_c5.dev.v_pool))
+        extra["MIG"] = {"workload": describe("MIG"), "us": round(rep["us"], 1), "us_min": round(float(rep["per"].min()), 1),
+                        "gbs_read_plus_write": round(rep["gbs"], 1), "frac_of_hbm_peak": round(rep["frac"], 4),
+                        "bytes": rep["bytes"], "tokens": rep["tokens"],
+                        "us_per_token_per_layer": round(rep["us"] / rep["tokens"], 6), "peer": rep["peer"],
+                        "clocks": rep["clocks"]}
+    except Exception as exc:  # an extra must never cost the headline line
+        extra["MIG"] = {"error": repr(exc)}
+    try:
+        s4, _ = make_workload("C4", 0)
+        st = StepTimer(s4, tb, torch)
+        st.warm(3)
+        sampler = ClockSampler(local)
+        sampler.start()
+        us = st.timed(steps) * 1e3 / steps
+        step_us, attn_us = st.instrumented(min(steps, 50))
+        clk = sampler.finish()
+        _, _, t_roof, t_nom = roofline_times(st.cnt, peaks)
+        extra["C4"] = {"workload": f"C4 ({describe('C4')})", "value": round(us, 2), "unit": UNIT, "steps": steps,
+                       "frac": round(t_roof / us, 4), "frac_of_nominal_peaks": round(t_nom / us, 4),
+                       "t_roof_us": round(t_roof, 2), "median": round(float(np.median(step_us)), 2),
+                       "min": round(float(step_us.min()), 2), "kernel_us": round(float(np.median(attn_us)), 2),
+                       "clocks": clk}
+    except Exception as exc:
+        extra["C4"] = {"error": repr(exc)}
+    return extra
+
+
+def run_migration(args, rank, world, local, tb, torch, dist, peaks):
+    import oracle
+    s, gen_s = make_workload("C5", rank)
+    oracle.kv_append(s.k_pool, s.v_pool, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new)
+    if world > 1:
+        dist.barrier()
+    mt, rep = migration_report(s, tb, torch, args.steps, args.warmup, peaks, local, world)
+    # e2e: the migration's metadata (lengths and both page tables) from pinned host memory, then the call, then a sync
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h = [pin(mt.L), pin(s.page_table), pin(mt.dst_pt)]
+    d = [mt.lens_d, mt.spt, mt.dpt]
+    n = max(3, min(args.steps, 50))
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(n):
+        for a, b in zip(h, d):
+            b.copy_(a, non_blocking=True)
+        mt.call()
+        torch.cuda.synchronize()
+    e2e_us = max_over_ranks((time.perf_counter() - t0) / n * 1e6, world, "cuda")
+    if rank != 0:
+        return
+    if args.no_cpu:
+        cpu_us, cores, desc = float("nan"), 0, "skipped (--no-cpu)"
+    else:
+        kd, vd = np.zeros(tuple(mt.k_dst.shape), np.uint16), np.zeros(tuple(mt.k_dst.shape), np.uint16)
+        t0 = time.perf_counter()
+        oracle.kv_migrate(s.k_pool, s.v_pool, kd, vd, mt.L, s.page_table, mt.dst_pt)
+        cpu_us, cores = (time.perf_counter() - t0) * 1e6, 1
+        desc = "oracle.kv_migrate on the whole workload (single-threaded C loops)"
+    us = rep["us"]
+    print(json.dumps({
+        "metric": "KV migration time (SURVEY 8(f) NEXT-3)", "value": round(us, 2), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": round(us / 1e3, 5), "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u16", "data": "synthetic",
+        "config": {"workload": f"MIG ({describe('MIG')})", "replicas": world, "tokens": rep["tokens"],
+                   "l2": "5.1 GB moved per call >> 126 MB L2, no flush needed"},
+        "us_per_step": {"median": round(float(np.median(rep["per"])), 2), "min": round(float(rep["per"].min()), 2)},
+        "roofline": {"bound": "hbm", "kernel": "kv_migrate_kernel", "achieved": round(rep["gbs"], 1),
+                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": round(rep["frac"], 4), "traffic": ncu_traffic("MIG"),
+                     "algorithmic_bytes": rep["bytes"], "of": peaks["source"],
+                     "frac_of_nominal_peak": round(rep["gbs"] / NOMINAL["hbm_gbs"], 4)},
+        "cpu_baseline": {"value": round(cpu_us, 1), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": round(e2e_us, 2), "unit": UNIT, "h2d_bytes_per_step": int(sum(x.numel() * 4 for x in h)),
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": int(rep["launches"]) * args.steps, "clocks": rep["clocks"], "peer": rep["peer"],
+        "gen_seconds": round(gen_s, 1),
+    }))
 
 
 def run_reference(args, rank, world):
@@ -315,7 +580,8 @@ def run_reference(args, rank, world):
     that the whole --steps K --warmup W run ends within a few minutes."""
     if rank != 0:
         return
-    s, _ = make_workload(args.config, 0)
+    cfg = "C5" if args.config == "MIG" else args.config
+    s, _ = make_workload(cfg, 0)
     _, _, cores, dt0 = oracle_sample_us(s, budget_rows_flops=2e8, seed=12345)  # calibrate rows/s
     per_step_s = min(10.0, max(0.05, 90.0 / max(1, args.steps + args.warmup)))
     budget = max(2e7, 2e8 * per_step_s / max(dt0, 1e-3))
@@ -329,7 +595,7 @@ def run_reference(args, rank, world):
         "impl": "reference", "metric": METRIC, "value": round(us, 1), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(us / 1e3, 3), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{args.config} ({describe(args.config)})"},
+        "config": {"workload": f"{cfg} ({describe(cfg)})"},
         "cpu_baseline": {"value": round(us, 1), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": round(us, 1), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -340,9 +606,11 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", default="C5", choices=synth.CONFIG_NAMES)
+    ap.add_argument("--config", default="C5", choices=synth.CONFIG_NAMES + ("MIG",))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--no-extra", action="store_true", help="skip extra.C4 / extra.MIG on the default run")
+    ap.add_argument("--sustain-seconds", type=float, default=2.0, help="length of the sustained loop (0 = skip)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))

@@ -90,6 +90,39 @@ int tropical_kv_append(const tropical_kv_pool_t *pool, const tropical_batch_t *b
 int tropical_kv_gather(const tropical_kv_pool_t *pool, const tropical_batch_t *batch, int32_t req,
                        int32_t n_keys, void *k_dense, void *v_dense, void *cuda_stream);
 
+/* KV migration of Path 1 (a request prefilled on a prefill worker re-enters through
+ * the decode queue and its KV cache moves to the multiplexing worker that will decode it; "migration of
+ * KVCache"; P:171 P2P between GPUs).  For every request m of the list, token j < kv_lens[m], kv head h:
+ *   dst_pool[dst_page_table[m][j / P]][h][j % P][:] = src_pool[src_page_table[m][j / P]][h][j % P][:]   (K and V)
+ * Gather through the source table and scatter under the destination table fused in one kernel (bulk-async copies
+ * through shared memory; no dense staging buffer).  Bit copy.  Token-granular: slots >= kv_lens[m] of a destination
+ * page and every other destination page keep their bits; the source pools are only read.
+ *   src_pool, dst_pool: same num_kv_heads, head_dim, page_size (num_q_heads is ignored); num_pages may differ.
+ *     The call runs on the CURRENT device, which must own src_pool; dst_pool may live on a peer device whose memory
+ *     is mapped here (tropical_enable_peer_access, cudaDeviceEnablePeerAccess or a VMM mapping): the source GPU then
+ *     pushes over NVLink.  The two pools must not overlap in the pages the tables name.
+ *   Two requests of the list naming the same destination (page, slot) are undefined behaviour; page ids are not
+ *   validated (device data).  Up to 1024 requests per launch; longer lists are split into several launches.
+ * Returns INVALID_ARG for null pointers / negative sizes / strides smaller than ceil(max_kv_len / P) / mismatched pool
+ * shapes, UNSUPPORTED for head_dim not in {64, 128} or page_size != 16. */
+typedef struct {
+    int32_t num_reqs;               /* >= 0 */
+    int32_t max_kv_len;             /* >= max_m kv_lens[m]: grid sizing and stride validation */
+    int32_t src_page_table_stride;  /* >= ceil(max_kv_len / P) */
+    int32_t dst_page_table_stride;  /* >= ceil(max_kv_len / P) */
+    const int32_t *kv_lens;         /* [device] [num_reqs] tokens to move per request */
+    const int32_t *src_page_table;  /* [device] [num_reqs][src_page_table_stride] */
+    const int32_t *dst_page_table;  /* [device] [num_reqs][dst_page_table_stride] */
+} tropical_migration_t;
+
+int tropical_kv_migrate(const tropical_kv_pool_t *src_pool, const tropical_kv_pool_t *dst_pool,
+                        const tropical_migration_t *migration, void *cuda_stream);
+
+/* Maps the memory of peer_device into the current device's address space (cudaDeviceEnablePeerAccess; "already
+ * enabled" counts as success) so that a pool allocated there can be the dst_pool of tropical_kv_migrate.
+ * TROPICAL_ERR_UNSUPPORTED when the two devices have no peer path. */
+int tropical_enable_peer_access(int32_t peer_device);
+
 /* Upper bound of the scratch tropical_mixed_attention needs for any batch with these host
  * scalars (work lists, split-K partials, tickets).  Returns 0 on invalid arguments. */
 size_t tropical_workspace_bytes(const tropical_kv_pool_t *pool, int32_t num_reqs, int32_t total_q,

@@ -21,6 +21,8 @@ from .binding import (  # noqa: F401
     debug_wait_profile,
     kv_append,
     kv_gather,
+    kv_migrate,
+    enable_peer_access,
     last_launch_count,
     lib,
     mixed_attention,

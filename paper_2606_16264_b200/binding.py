@@ -75,7 +75,7 @@ class SimSummary(ctypes.Structure):
 SIM_COLOCATED, SIM_DISAGGREGATED, SIM_MULTIPLEXED = 0, 1, 2
 
 EXPORTS = (
-    "tropical_kv_append", "tropical_kv_gather", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention",
+    "tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
     "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile",
@@ -103,7 +103,7 @@ def lib():
     L.tropical_status_string.restype = ctypes.c_char_p
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
-    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_validate_batch", "tropical_mixed_attention", "tropical_step_host",
+    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_step_host",
                  "tropical_step_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
                  "tropical_debug_read_profile"):
         getattr(L, name).restype = ctypes.c_int
@@ -233,6 +233,37 @@ def kv_gather(pool: KVPool, batch: Batch, req: int, n_keys: int, stream=None):
     _check(lib().tropical_kv_gather(ctypes.byref(p), ctypes.byref(b), ctypes.c_int32(req), ctypes.c_int32(n_keys),
                                     _ptr(kd), _ptr(vd), _stream(stream)), "tropical_kv_gather")
     return kd, vd
+
+
+class _Migration(ctypes.Structure):
+    _fields_ = [("num_reqs", ctypes.c_int32), ("max_kv_len", ctypes.c_int32), ("src_page_table_stride", ctypes.c_int32),
+                ("dst_page_table_stride", ctypes.c_int32), ("kv_lens", ctypes.c_void_p),
+                ("src_page_table", ctypes.c_void_p), ("dst_page_table", ctypes.c_void_p)]
+
+
+def kv_migrate(src_pool: KVPool, dst_pool: KVPool, kv_lens: torch.Tensor, src_page_table: torch.Tensor,
+               dst_page_table: torch.Tensor, max_kv_len: int, stream=None) -> None:
+    """KV migration (include/tropical.h: tropical_kv_migrate).  kv_lens int32 [n], page tables int32 [n, stride], all on
+    the CURRENT device (the owner of src_pool); dst_pool may be on a peer device (enable_peer_access first)."""
+    for t in (kv_lens, src_page_table, dst_page_table):
+        if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+            raise ValueError("migration arrays must be contiguous int32 CUDA tensors")
+    sp, dp = src_pool.c(), dst_pool.c()
+    n = kv_lens.numel()
+    m = _Migration(n, int(max_kv_len), src_page_table.shape[1] if src_page_table.dim() == 2 else 0,
+                   dst_page_table.shape[1] if dst_page_table.dim() == 2 else 0, kv_lens.data_ptr(),
+                   src_page_table.data_ptr(), dst_page_table.data_ptr())
+    _check(lib().tropical_kv_migrate(ctypes.byref(sp), ctypes.byref(dp), ctypes.byref(m), _stream(stream)),
+           "tropical_kv_migrate")
+
+
+def enable_peer_access(peer_device: int) -> bool:
+    """True when peer_device's memory is (now) mapped into the current device; False when there is no peer path."""
+    rc = lib().tropical_enable_peer_access(ctypes.c_int32(int(peer_device)))
+    if rc == 2:
+        return False
+    _check(rc, "tropical_enable_peer_access")
+    return True
 
 
 def validate_batch(pool: KVPool, batch: Batch, scratch: Optional[torch.Tensor] = None, stream=None):

@@ -124,6 +124,60 @@ int tropical_kv_gather(const tropical_kv_pool_t* pool, const tropical_batch_t* b
     return TROPICAL_OK;
 }
 
+int tropical_kv_migrate(const tropical_kv_pool_t* src, const tropical_kv_pool_t* dst, const tropical_migration_t* mig,
+                        void* cuda_stream) {
+    g_launches = 0;
+    int rc = check_pool(src);
+    if (rc != TROPICAL_OK) return rc;
+    rc = check_pool(dst);
+    if (rc != TROPICAL_OK) return rc;
+    if (src->num_kv_heads != dst->num_kv_heads || src->head_dim != dst->head_dim || src->page_size != dst->page_size)
+        return TROPICAL_ERR_INVALID_ARG;
+    if (mig == nullptr || mig->num_reqs < 0 || mig->max_kv_len < 0 || mig->src_page_table_stride < 0 ||
+        mig->dst_page_table_stride < 0)
+        return TROPICAL_ERR_INVALID_ARG;
+    const long long need_pages = ((long long)mig->max_kv_len + kPageSize - 1) / kPageSize;
+    if (mig->src_page_table_stride < need_pages || mig->dst_page_table_stride < need_pages) return TROPICAL_ERR_INVALID_ARG;
+    if (mig->num_reqs == 0 || mig->max_kv_len == 0) return TROPICAL_OK;
+    if (mig->kv_lens == nullptr || mig->src_page_table == nullptr || mig->dst_page_table == nullptr)
+        return TROPICAL_ERR_INVALID_ARG;
+    MigrateArgs a;
+    a.Hkv = src->num_kv_heads;
+    a.D = src->head_dim;
+    a.num_reqs = mig->num_reqs;
+    a.src_stride = mig->src_page_table_stride;
+    a.dst_stride = mig->dst_page_table_stride;
+    a.kv_lens = mig->kv_lens;
+    a.src_pt = mig->src_page_table;
+    a.dst_pt = mig->dst_page_table;
+    a.k_src = (const uint16_t*)src->k_pool;
+    a.v_src = (const uint16_t*)src->v_pool;
+    a.k_dst = (uint16_t*)dst->k_pool;
+    a.v_dst = (uint16_t*)dst->v_pool;
+    int launches = 0;
+    cudaError_t e = launch_kv_migrate(a, mig->max_kv_len, (cudaStream_t)cuda_stream, &launches);
+    if (e != cudaSuccess) return cuda_fail(e, "kv_migrate");
+    g_launches = launches;
+    return TROPICAL_OK;
+}
+
+int tropical_enable_peer_access(int32_t peer_device) {
+    int dev = 0, can = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "enable_peer_access");
+    if (peer_device == dev) return TROPICAL_OK;
+    e = cudaDeviceCanAccessPeer(&can, dev, peer_device);
+    if (e != cudaSuccess) return cuda_fail(e, "enable_peer_access");
+    if (!can) return TROPICAL_ERR_UNSUPPORTED;
+    e = cudaDeviceEnablePeerAccess(peer_device, 0);
+    if (e == cudaErrorPeerAccessAlreadyEnabled) {
+        cudaGetLastError();  // clear the sticky-less error
+        return TROPICAL_OK;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "enable_peer_access");
+    return TROPICAL_OK;
+}
+
 int tropical_validate_batch(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, int32_t* first_bad_request,
                             void* scratch, void* cuda_stream) {
     g_launches = 0;

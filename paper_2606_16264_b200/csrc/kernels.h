@@ -12,6 +12,18 @@ cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const voi
                              cudaStream_t stream);
 cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, int n_keys, void* k_dense,
                              void* v_dense, cudaStream_t stream);
+// NEXT-3 KV migration (csrc/kv_migrate.cu): source pool through src_pt -> destination pool under dst_pt
+struct MigrateArgs {
+    int Hkv, D, num_reqs, src_stride, dst_stride;
+    const int* kv_lens;
+    const int* src_pt;
+    const int* dst_pt;
+    const uint16_t* k_src;
+    const uint16_t* v_src;
+    uint16_t* k_dst;
+    uint16_t* v_dst;
+};
+cudaError_t launch_kv_migrate(const MigrateArgs& args, int max_kv_len, cudaStream_t stream, int* launches);
 cudaError_t launch_validate_batch(const PoolDesc& pool, const BatchDesc& b, int* first_bad_dev, cudaStream_t stream);
 cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
                                   float scale_log2, cudaStream_t stream);

@@ -1,13 +1,11 @@
-"""Parity at BASELINE.json's FULL sizes (configs[1..4] = C2..C5), in the launch configuration bench.py
-times (fused step kernel, same workspace sizing, `values="tiled"` pools with NaN-poisoned unused slots).
+"""Parity at BASELINE.json's FULL sizes (configs[1..4] = C2..C5), in the launch configuration bench.py times (fused
+step kernel, same workspace sizing, `values="tiled"` pools with NaN-poisoned unused slots), over ALL elements of `out`
+("over all elements of out per config"):
 
-The fp64 oracle cannot finish all of C4/C5 in seconds, so:
-  * KV append: the WHOLE pool is compared bit for bit with the oracle's pool (the oracle's append is cheap);
-  * attention: every decode row (one row per request, all q heads) plus a seeded sample of prefill rows that
-    always includes the rows around 128-row tile edges and the first / last row of every chunk are computed one
-    by one with oracle.attention_rows and compared within the BASELINE tolerance;
-  * every other output element is checked by a property that holds at any size: finite, and inside the convex
-    hull bound |out| <= max |V| of the whole pool (a softmax-weighted mean of V rows).
+  * KV append: the WHOLE pool is compared bit for bit with the oracle's pool;
+  * attention: oracle.mixed_attention on EVERY row of the step (C5: 5376 rows x 64 heads, a few seconds on the GPU
+    box's cores), max |d| <= 2e-2 and mean |d| <= 2e-3 over all T * Hq * d outputs, LSE within 2e-3;
+  * extra, not parity: every output inside the convex-hull bound |out| <= max |V| of the pool.
 """
 import numpy as np
 import pytest
@@ -19,28 +17,8 @@ from tests.gpu_harness import MAX_ABS_TOL, MEAN_ABS_TOL, DeviceStep, bits
 pytestmark = pytest.mark.gpu
 
 
-def _sample_rows(s, rng, n_prefill_random=48):
-    rows = []
-    for i in range(s.num_reqs):
-        q = int(s.q_lens[i])
-        if q == 1:
-            rows.append((i, 0))
-        elif q > 1:
-            edge = {0, 1, q - 1, q - 2}
-            for e in range(128, q, 128):
-                edge.update((e - 1, e, e + 1))
-            edge = sorted(t for t in edge if 0 <= t < q)
-            if len(edge) > 40:  # keep the oracle's work bounded: all edges of the first / last tiles, sampled middle
-                keep = set(edge[:8] + edge[-8:])
-                keep.update(rng.choice(edge, 24, replace=False).tolist())
-                edge = sorted(keep)
-            rows += [(i, t) for t in edge]
-            rows += [(i, int(t)) for t in rng.integers(0, q, n_prefill_random)]
-    return sorted(set(rows))
-
-
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
-def test_full_config_sampled_parity(name):
+def test_full_config_all_rows_parity(name):
     s = synth.make_config(name, poison=True, values="tiled")
     kp, vp = s.copy_pools()
     oracle.kv_append(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new)
@@ -51,15 +29,19 @@ def test_full_config_sampled_parity(name):
     assert np.array_equal(bits(dev.v_pool), vp), "V pool differs"
     del dev
 
-    rows = _sample_rows(s, np.random.default_rng(77))
-    ref, ref_lse = oracle.attention_rows(kp, vp, s.q, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, rows)
-    idx = np.array([int(s.q_offsets[i]) + t for i, t in rows])
-    err = np.abs(out[idx] - ref)
+    ref, ref_lse = oracle.mixed_attention(kp, vp, s.q, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table)
+    assert ref.shape == out.shape == (s.total_q, s.num_q_heads, s.head_dim)
+    err = np.abs(out - ref)
+    assert np.isfinite(out).all() and np.isfinite(lse).all()
     assert err.max() <= MAX_ABS_TOL and err.mean() <= MEAN_ABS_TOL, (name, err.max(), err.mean())
-    assert np.abs(lse[idx] - ref_lse).max() <= 2e-3
+    assert np.abs(lse - ref_lse).max() <= 2e-3
+    # per-request view of the same comparison: no request hides behind the others' mean
+    for i in range(s.num_reqs):
+        a, b = int(s.q_offsets[i]), int(s.q_offsets[i + 1])
+        if b > a:
+            assert err[a:b].mean() <= MEAN_ABS_TOL, (name, i, err[a:b].mean())
 
-    # properties over ALL rows
-    assert np.isfinite(out).all()
+    # extra (a property, not parity): a softmax-weighted mean of V rows cannot leave their hull
     mag = 0  # largest finite |V| in the pool after the append, by bit pattern (|bf16| is monotone in bits & 0x7FFF)
     for p0 in range(0, vp.shape[0], 4096):
         b = vp[p0:p0 + 4096] & np.uint16(0x7FFF)
@@ -67,4 +49,3 @@ def test_full_config_sampled_parity(name):
         mag = max(mag, int(b.max()))
     vmax = float(synth.bf16_bits_to_f32(np.array([mag], np.uint16))[0])
     assert np.abs(out).max() <= vmax * 1.01 + 1e-6
-    assert np.isfinite(lse).all()

@@ -64,14 +64,13 @@ EDGE_C = [0, 1, 15, 16, 17, 127, 128, 129, 255, 256, 257, 511, 512, 513, 4095, 4
 @pytest.mark.parametrize("d", [64, 128])
 @pytest.mark.parametrize("g", [1, 4, 8])
 def test_edge_matrix_q_by_c(d, g):
-    """Every q in EDGE_Q paired with several c in EDGE_C, batched so the whole matrix is covered."""
-    Hkv = 2
+    """The full product EDGE_Q x EDGE_C (13 x 17 = 221 (q, c) pairs) for every (d, g): one step per q whose 17 requests
+    carry all the c values, so every pairing of a chunk length with a prior-context length is compared with the oracle
+    over all of its outputs."""
+    Hkv = 2 if g < 8 else 1
     rng = np.random.default_rng(100 + d + g)
-    for k, q in enumerate(EDGE_Q):
-        cs = [EDGE_C[(k * 5 + r * 3) % len(EDGE_C)] for r in range(4)]
-        if q == 1000:
-            cs = cs[:2]
-        s = synth.make_step(rng, Hkv * g, Hkv, d, 16, [q] * len(cs), cs)
+    for q in EDGE_Q:
+        s = synth.make_step(rng, Hkv * g, Hkv, d, 16, [q] * len(EDGE_C), EDGE_C)
         _check_step(s)
 
 
@@ -131,7 +130,7 @@ def test_chunked_equals_unchunked_and_decode_equals_last_row():
 
 
 # ------------------------------------------------------------------ O8 needle (bit-exact gather through attention)
-def _needle_step(d, c, ql, targets_fn, Hq=2, Hkv=1, seed=0):
+def _needle_step(d, c, ql, targets_fn, Hq=2, Hkv=1, seed=0, values="normal"):
     rng = np.random.default_rng(seed)
     L = c + ql
 
@@ -144,7 +143,7 @@ def _needle_step(d, c, ql, targets_fn, Hq=2, Hkv=1, seed=0):
     V = rng.standard_normal((L, Hkv, d)).astype(np.float32)
     targets = [targets_fn(t) for t in range(ql)]
     Q = np.stack([code(j) for j in targets])[:, None, :].repeat(Hq, 1)
-    s = synth.make_step(rng, Hq, Hkv, d, 16, [ql], [c])
+    s = synth.make_step(rng, Hq, Hkv, d, 16, [ql], [c], values=values)
     Kb, Vb = f32_to_bf16_bits(K), f32_to_bf16_bits(V)
     # install prior context rows [0,c) directly, new rows via the append under test
     for j in range(c):
@@ -188,6 +187,71 @@ def test_negative_needle_future_key_not_selected():
     assert errors(out, ref)[0] <= MAX_ABS_TOL
     got = bits(dev.out)
     assert not np.array_equal(got[3, 0], Vb[c + 3 + 1, 0])
+
+
+def test_append_then_attention_ordering_stress():
+    """Stream ordering of the step's three launches (append -> tile directory, which overlaps the append by programmatic
+    dependent launch -> step kernel): a C4-sized append (2048 tokens x 40 kv heads, ~45 MB of scattered rows) directly
+    followed by the attention that reads those rows, 200 times.  Before every repetition the target slots are
+    overwritten with NaN patterns and V alternates between two draws, so a step kernel that started before the append
+    had landed would return NaN or the other draw's rows.  Needle queries select the just-appended row: bit-exact."""
+    d, ql, H = 128, 2048, 40
+    s, targets, Vb = _needle_step(d, 0, ql, lambda t: t, Hq=H, Hkv=H, seed=5, values="tiled")
+    assert targets == list(range(ql))
+    dev = DeviceStep(s)
+    rng = np.random.default_rng(6)
+    v_alt = f32_to_bf16_bits(rng.standard_normal((ql, 1, d)).astype(np.float32))
+    v_sets = [s.v_new.copy(), np.ascontiguousarray(np.broadcast_to(v_alt, (ql, H, d)))]
+    v_dev = [torch.from_numpy(v.view(np.int16)).cuda() for v in v_sets]
+    pages = dev.batch.page_table[0, : ql // 16].long()
+    for rep in range(200):
+        dev.k_pool[pages] = synth.POISON_BF16
+        dev.v_pool[pages] = synth.POISON_BF16
+        dev.out.zero_()
+        tb.kv_append(dev.pool, dev.batch, dev.k_new, v_dev[rep & 1])
+        tb.mixed_attention(dev.pool, dev.batch, dev.q, out=dev.out, workspace=dev.workspace)
+        if rep % 20 == 19 or rep < 4:
+            torch.cuda.synchronize()
+            got = bits(dev.out)
+            assert np.array_equal(got, v_sets[rep & 1][:, :, :]), f"repetition {rep}: stale or poisoned rows were read"
+    torch.cuda.synchronize()
+
+
+def test_head_sharded_step_equals_unsharded_bit_for_bit():
+    """SURVEY 8(e) / P:184 (tensor parallelism 2 inside a worker): the path shards by kv head with no collective.  Two
+    pools holding kv heads [0, Hkv/2) and [Hkv/2, Hkv) of the same step, each run with Hq/2 and Hkv/2: the concatenated
+    outputs equal the unsharded run bit for bit (the decode split boundaries are pinned equal with the test hook,
+    since the automatic split size depends on the head count), and the oracle within tolerance."""
+    Hq, Hkv, d = 64, 8, 128
+    rng = np.random.default_rng(31)
+    ctx = np.clip(np.rint(np.exp(np.log(1500) + 1.0 * rng.standard_normal(24))), 64, 8192).astype(int).tolist()
+    s = synth.make_step(rng, Hq, Hkv, d, 16, [700, 130] + [1] * 24, [0, 300] + ctx)
+    ref, ref_lse, kp, vp = oracle.step(s)
+    tb.debug_set_split_pages(32)
+    try:
+        dev = DeviceStep(s)
+        out, lse = dev.step()
+        whole = bits(dev.out).copy()
+        assert errors(out, ref)[0] <= MAX_ABS_TOL and errors(out, ref)[1] <= MEAN_ABS_TOL
+        g = Hq // Hkv
+        parts, lses = [], []
+        for r in range(2):
+            hk = slice(r * Hkv // 2, (r + 1) * Hkv // 2)
+            hq = slice(r * Hq // 2, (r + 1) * Hq // 2)
+            sh = synth.StepInputs(f"shard{r}", -1, Hq // 2, Hkv // 2, d, 16, s.num_pages, s.q_lens, s.ctx_lens,
+                                  s.q_offsets, s.page_table, np.ascontiguousarray(s.k_pool[:, hk]),
+                                  np.ascontiguousarray(s.v_pool[:, hk]), np.ascontiguousarray(s.q[:, hq]),
+                                  np.ascontiguousarray(s.k_new[:, hk]), np.ascontiguousarray(s.v_new[:, hk]))
+            dsh = DeviceStep(sh)
+            _, l_sh = dsh.step()
+            parts.append(bits(dsh.out).copy())
+            lses.append(l_sh)
+            assert np.array_equal(bits(dsh.k_pool), kp[:, hk]) and np.array_equal(bits(dsh.v_pool), vp[:, hk])
+        assert g == 8
+        assert np.array_equal(np.concatenate(parts, axis=1), whole)
+        assert np.array_equal(np.concatenate(lses, axis=1), lse)
+    finally:
+        tb.debug_set_split_pages(0)
 
 
 # ------------------------------------------------------------------ O9 poison + stray writes, determinism

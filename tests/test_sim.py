@@ -121,6 +121,93 @@ def test_disaggregated_adds_migration_and_keeps_decode_off_prefill_workers():
     assert res[0]["tpot_us"] == pytest.approx((50.0 + 2 * 10.1) / 2)   # TPOT contains the migration
 
 
+def test_step_cost_closed_form_on_the_golden_batches():
+    """The oracle's restatement of the step-cost form, and the library's, against values worked by hand from the feature
+    counts of tests/golden/step_cost_features.txt (derived there without code) and a model with round coefficients:
+    t0 = 5, a = 1e-6 us/FLOP, b = 1e-5 us/B, kappa = 0.5, e_p = 2, e_d = 3, n_sm = 4.
+      A (Hq 4, Hkv 2, d 64; q = [130, 1], c = [0, 17]): F = 8737792, B = 277036, N_p = 12 iterations, N_d = 4 units:
+        aF = 8.737792 >= bB = 2.77036 -> 5 + 8.737792 + 0.5 * 2.77036 + 2 * 12 / 4 + 3 * 4 / 4 = 24.122972
+      B (8/8/128; q = [256], c = [300]): F = 449314816, B = 4374668, N_p = 72, N_d = 0:
+        5 + 449.314816 + 0.5 * 43.74668 + 2 * 72 / 4 = 512.188156
+      A with a = 1e-8 (the byte term leads): 5 + 2.77036 + 0.5 * 0.08737792 + 6 + 3 = 16.81404896"""
+    cm = (5.0, 1e-6, 1e-5, 0.5, 2.0, 3.0, 4.0)
+    cases = [((4, 2, 64), [130, 1], [0, 17], cm, 24.122972),
+             ((8, 8, 128), [256], [300], cm, 512.188156),
+             ((4, 2, 64), [130, 1], [0, 17], (5.0, 1e-8, 1e-5, 0.5, 2.0, 3.0, 4.0), 16.81404896)]
+    for (Hq, Hkv, d), q, c, model, want in cases:
+        cfg = _ocfg(so.COLOCATED, cm=model, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d)
+        assert so.step_cost_us(cfg, q, c) == pytest.approx(want, rel=1e-12)
+        got, _ = tb.step_cost(Hq, Hkv, d, 16, q, c, model=tb.CostModel(*model))
+        assert got == pytest.approx(want, rel=1e-12)
+        # an iteration = layers * step + linear * new tokens + overhead (tropical_sim.h "Worker iteration")
+        cfg3 = _ocfg(so.COLOCATED, cm=model, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d, num_layers=3)
+        assert so.iter_time_us(cfg3, q, c) == pytest.approx(3 * want + 0.1 * sum(q) + 10.0, rel=1e-12)
+
+
+def test_least_unfinished_tokens_dispatch_by_hand():
+    """P:186 with several non-empty candidates.  Two colocated workers, flat cost (iteration = 10 + 0.1 * tokens).
+      t=0  r0 (prompt 100, 50 outputs): both empty, tie -> worker 0.           unfinished: w0 = 100 + 49 = 149
+      t=1  r1 (50, 2):   w0 149, w1 0 -> worker 1.                              w1 = 50 + 1 = 51
+      t=2  r2 (10, 2):   w0 149, w1 51 -> worker 1 (busier queue, fewer tokens). w1 = 51 + 10 + 1 = 62
+      t=3  r3 (200, 30): w0 149, w1 62 -> worker 1.                             w1 = 62 + 200 + 29 = 291
+      t=4  r4 (5, 1):    w0 149, w1 291 -> worker 0.
+    Worker 1: prefill r1 1..16; then {prefill r2 (10 tokens), decode r1} = 10 + 0.1 * 11 = 11.1 -> r2's first token at
+    27.1 (TTFT 25.1), r1 finished at 27.1 (TPOT 11.1)."""
+    reqs = [(0.0, 100, 50), (1.0, 50, 2), (2.0, 10, 2), (3.0, 200, 30), (4.0, 5, 1)]
+    cfg = _ocfg(so.COLOCATED, num_workers=2)
+    res, _ = so.simulate(cfg, reqs)
+    assert [r["prefill_worker"] for r in res] == [0, 1, 1, 1, 0]
+    assert res[2]["ttft_us"] == pytest.approx(25.1) and res[1]["tpot_us"] == pytest.approx(11.1)
+    cres, _ = tb.sim_run(_ccfg(cfg), reqs)
+    assert [r.prefill_worker for r in cres] == [0, 1, 1, 1, 0] and cres[2].ttft_us == pytest.approx(25.1)
+
+
+def test_path1_counts_the_iteration_in_flight_as_queueing_time():
+    """P:157 "predicted queuing time in the workers" with a BUSY prefill worker.  Worker 0 prefill worker, worker 1
+    multiplexing worker closed by its HBM watermark (capacity 100 tokens).  Flat cost, TTFT SLO 150.
+      t=0   r0 (1000, 1): exec 110 + queue 0 < 150 -> worker 0, busy until 110.
+      t=10  r1 (500, 1):  exec 60 + queue (110 - 10 = 100, the iteration in flight) = 160 >= slack 150: NOT sent.
+      t=110 worker 0 idle: exec 60 + 0 >= slack 150 - 100 = 50: still not sent.
+      t=160 = arrival + SLO: slack gone, sent anyway; prefill 160..220 -> TTFT 210.
+    (Ignoring the iteration in flight would have sent r1 at t = 10: TTFT 160.)
+      r1' (300, 1) instead: exec 40 + 100 = 140 < 150 -> sent at t = 10, runs 110..150 -> TTFT 140."""
+    cfg = _ocfg(so.MULTIPLEXED, ttft_slo_us=150.0, kv_capacity_tokens=100)
+    for sim in (lambda c, r: [x["ttft_us"] for x in so.simulate(c, r)[0]],
+                lambda c, r: [x.ttft_us for x in tb.sim_run(_ccfg(c), r)[0]]):
+        assert sim(cfg, [(0.0, 1000, 1), (10.0, 500, 1)]) == pytest.approx([110.0, 210.0])
+        assert sim(cfg, [(0.0, 1000, 1), (10.0, 300, 1)]) == pytest.approx([110.0, 140.0])
+
+
+def test_p90_index_by_hand():
+    """P:173 "P90 latency": value at index ceil(0.9 n) - 1 of the sorted list -- the 9th smallest of 10, the 10th of 11.
+    Ten requests far apart on one worker: TTFT = 10 + 0.1 * prompt = 11, 12, ..., 20 -> p90 = 19; TPOT = 10.1 each."""
+    results = [dict(ttft_us=float(v), tpot_us=float(21 - v), first_token_us=0.0, finish_us=float(v), multiplexed=0)
+               for v in (7, 3, 10, 1, 9, 2, 8, 4, 6, 5)]
+    summ = so.summarize(_ocfg(so.COLOCATED), results, 0)
+    assert summ["ttft_p90_us"] == 9.0 and summ["tpot_p90_us"] == 19.0 and summ["ttft_mean_us"] == pytest.approx(5.5)
+    results.append(dict(ttft_us=11.0, tpot_us=9.0, first_token_us=0.0, finish_us=11.0, multiplexed=0))
+    assert so.summarize(_ocfg(so.COLOCATED), results, 0)["ttft_p90_us"] == 10.0
+    reqs = [(1000.0 * i, 10 * (i + 1), 2) for i in range(10)]
+    _, csum = tb.sim_run(_ccfg(_ocfg(so.COLOCATED, num_workers=1)), reqs)
+    assert csum.ttft_p90_us == pytest.approx(19.0) and csum.tpot_p90_us == pytest.approx(10.1)
+    assert csum.ttft_mean_us == pytest.approx(15.5)
+
+
+def test_no_starvation_wake_up_fires_despite_rounding():
+    """with arrival 2724338.6555860057 and SLO 60.37494846539122 the residual slo - (now - arrival) at the
+    wake-up time arrival + slo is +1e-10, not <= 0; the rule must fire on the expression the wake-up was scheduled
+    with.  Multiplexing worker closed (capacity 500 < prompt), prefill worker too slow for the SLO: the request is sent
+    at arrival + SLO and finishes; nobody is scored as served without being served."""
+    a, slo = 2724338.6555860057, 60.37494846539122
+    cfg = _ocfg(so.MULTIPLEXED, ttft_slo_us=slo, kv_capacity_tokens=500)
+    ores, osum = so.simulate(cfg, [(a, 1000, 3)])
+    cres, csum = tb.sim_run(_ccfg(cfg), [(a, 1000, 3)])
+    want_first = (a + slo) + 110.0
+    assert ores[0]["first_token_us"] == pytest.approx(want_first, rel=1e-12)
+    assert cres[0].first_token_us == pytest.approx(want_first, rel=1e-12) and cres[0].finish_us > cres[0].first_token_us
+    assert osum["attainment"] == 0.0 and csum.attainment == 0.0      # TTFT = slo + 110 > slo
+
+
 def _trace(seed, n, mean_gap_us):
     rng = random.Random(seed)
     t, out = 0.0, []
