@@ -268,6 +268,23 @@ class StepTimer:
         attn_us = np.array([b.elapsed_time(c) for _, b, c in evs]) * 1e3
         return step_us, attn_us
 
+    def timeline(self, reps=8):
+        """Measurement builds only (-DTROPICAL_TIMELINE): when each of the step's three kernels starts and ends, median
+        over `reps` steps (L2 flushed before each so that the chain of cold metadata loads is visible)."""
+        tb, torch = self.tb, self.torch
+        if tb.debug_timeline(reset=True) is None:
+            return None
+        buf = self.flush_buf if self.flush_buf is not None else torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+        rows = []
+        for k in range(reps):
+            tb.debug_timeline(reset=True)   # synchronises: re-arm first, then keep the GPU busy with the flush so that
+            buf.fill_(k & 0xff)             # the step's launches are queued behind it (no host launch latency inside)
+            self.one_step()
+            t = tb.debug_timeline()
+            rows.append([t[f] / 1e3 for f in tb.TIMELINE_FIELDS])
+        med = np.median(np.array(rows), axis=0)
+        return {f: round(float(v), 1) for f, v in zip(tb.TIMELINE_FIELDS, med)}
+
     def sustained(self, seconds, local):
         """The step back to back for >= `seconds`: what a long-running worker sees once the power management has
         settled (C5 runs against the 1000 W board limit; a 50 ms burst holds higher clocks)."""
@@ -435,6 +452,7 @@ def run_ours(args, rank, world):
     us = ms_per_step * 1e3
     sus = st.sustained(args.sustain_seconds, local) if args.sustain_seconds > 0 else None
     e2e_us, h2d, d2h = e2e_host_step(st, args.steps, world)
+    tl = st.timeline()
 
     extra = {}
     if args.config == "C5" and not args.no_extra and world == 1:
@@ -486,6 +504,8 @@ def run_ours(args, rank, world):
         line["sustained"] = {"value": round(sus["us"], 2), "unit": UNIT, "frac": round(t_roof / sus["us"], 4),
                              "steps": sus["steps"], "clocks": sus["clocks"],
                              "how": f"back to back for {sus['seconds']:.1f} s, second half timed"}
+    if tl is not None:
+        line["timeline_us"] = dict(tl, note="-DTROPICAL_TIMELINE build: not a bench build; L2 flushed before each step")
     if extra:
         line["extra"] = extra
     print(json.dumps(line))

@@ -44,6 +44,14 @@ int tropical_debug_wait_profile(uint64_t *cycles, uint64_t *calls, int32_t n, in
  * [3] latest late-joining decode warp done.  Copies 32 bytes device->host and synchronises the stream. */
 int tropical_debug_read_profile(const void *workspace, uint64_t *out_ns, void *cuda_stream);
 
+/* Only in builds with -DTROPICAL_TIMELINE (else TROPICAL_ERR_UNSUPPORTED): global-timer stamps (ns) of the three
+ * kernels of the last step(s) since the last reset -- out_ns[0] append start, [1] append end, [2] tile directory start,
+ * [3] directory body end, [4] directory end (after its wait on the append), [5] step kernel start, [6] its prologue end
+ * (last CTA), [7] its first CTA past griddepcontrol.wait, [8] its end.  Starts are minima over blocks, ends maxima.
+ * out_ns [host, nullable] 9 entries; reset != 0 re-arms the stamps.  Synchronises the device.  This is how the overlap
+ * of the directory kernel and of the step kernel's prologue with the append was measured (profiles/). */
+int tropical_debug_timeline(uint64_t *out_ns, int32_t reset);
+
 #ifdef __cplusplus
 }
 #endif

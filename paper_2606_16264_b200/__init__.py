@@ -13,10 +13,12 @@ from .binding import (  # noqa: F401
     SIM_DISAGGREGATED,
     SIM_MULTIPLEXED,
     SimConfig,
+    TIMELINE_FIELDS,
     TropicalError,
     debug_attention_simt,
     debug_read_profile,
     debug_set_grid,
+    debug_timeline,
     debug_set_split_pages,
     debug_wait_profile,
     kv_append,

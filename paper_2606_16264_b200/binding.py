@@ -78,7 +78,7 @@ EXPORTS = (
     "tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
-    "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile",
+    "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile", "tropical_debug_timeline",
     "tropical_sim_run",
 )
 
@@ -148,6 +148,24 @@ def debug_read_profile(workspace: torch.Tensor, stream=None):
     t0 = int(out[0])
     rel = lambda v: int(v) - t0 if int(v) else 0
     return {"prefill_done": rel(out[1]), "decode_done": rel(out[2]), "late_decode_done": rel(out[3])}
+
+
+TIMELINE_FIELDS = ("append_start", "append_end", "plan_start", "plan_body_end", "plan_end", "step_start",
+                   "step_prologue_end", "step_main_start", "step_end")
+
+
+def debug_timeline(reset: bool = False):
+    """{field: ns relative to the append's start} of the step(s) since the last reset; None unless built with
+    -DTROPICAL_TIMELINE.  debug_timeline(reset=True) before a step, debug_timeline() after it."""
+    out = (ctypes.c_uint64 * 9)()
+    rc = lib().tropical_debug_timeline(None if reset else out, ctypes.c_int32(1 if reset else 0))
+    if rc == 2:
+        return None
+    _check(rc, "tropical_debug_timeline")
+    if reset:
+        return {}
+    t0 = int(out[0])
+    return {k: int(out[i]) - t0 for i, k in enumerate(TIMELINE_FIELDS)}
 
 
 def last_launch_count() -> int:

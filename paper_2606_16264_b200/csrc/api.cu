@@ -355,6 +355,16 @@ int tropical_debug_wait_profile(uint64_t* cycles, uint64_t* calls, int32_t n, in
     return got == 0 ? TROPICAL_ERR_UNSUPPORTED : TROPICAL_OK;
 }
 
+int tropical_debug_timeline(uint64_t* out_ns, int32_t reset) {
+    unsigned long long a[16] = {0}, m[16] = {0};
+    const int ra = read_timeline_append(out_ns ? a : nullptr, reset), rm = read_timeline_mixed(out_ns ? m : nullptr, reset);
+    if (ra < 0 || rm < 0) return cuda_fail(cudaGetLastError(), "timeline");
+    if (ra == 0 || rm == 0) return TROPICAL_ERR_UNSUPPORTED;
+    if (out_ns != nullptr)
+        for (int i = 0; i < 9; ++i) out_ns[i] = i < 2 ? a[i] : m[i];
+    return TROPICAL_OK;
+}
+
 const char* tropical_last_cuda_error(void) { return g_cuda_err; }
 
 const char* tropical_version(void) { return "tropical-b200 0.1 (sm_100a)"; }

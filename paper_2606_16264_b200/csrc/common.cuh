@@ -8,6 +8,32 @@
 
 namespace tropical {
 
+// Measurement build only (-DTROPICAL_TIMELINE): global-timer stamps of the three kernels of a step (min over the
+// blocks for a start, max for an end), one copy per translation unit, read back by tropical_debug_timeline:
+//   0 append start, 1 append end, 2 directory start, 3 directory body end, 4 directory end (after its wait on the
+//   append), 5 step kernel start, 6 its prologue end (last CTA), 7 its first CTA past griddepcontrol.wait, 8 its end.
+#ifdef TROPICAL_TIMELINE
+static __device__ unsigned long long g_tl[16];
+__device__ __forceinline__ void tl_mark(int i, bool mn) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    if (mn) atomicMin(&g_tl[i], t); else atomicMax(&g_tl[i], t);
+}
+static inline int timeline_read(unsigned long long* out16, int reset) {
+    if (cudaDeviceSynchronize() != cudaSuccess) return -1;
+    if (out16 && cudaMemcpyFromSymbol(out16, g_tl, 16 * sizeof(unsigned long long)) != cudaSuccess) return -1;
+    if (reset) {
+        unsigned long long init[16];
+        for (int i = 0; i < 16; ++i) init[i] = 0ull;
+        init[0] = init[2] = init[5] = init[7] = ~0ull;  // starts are minima
+        if (cudaMemcpyToSymbol(g_tl, init, sizeof init) != cudaSuccess) return -1;
+    }
+    return 16;
+}
+#else
+__device__ __forceinline__ void tl_mark(int, bool) {}
+#endif
+
 constexpr int kPageSize = 16;  // BASELINE.json: page size 16 in every config
 
 struct PoolDesc {

@@ -33,6 +33,8 @@ void set_debug_grid(int num_ctas);
 void set_debug_split_pages(int pages);
 int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset);
 size_t profile_offset_bytes();
+int read_timeline_append(unsigned long long* out16, int reset);  // 0 unless built with -DTROPICAL_TIMELINE
+int read_timeline_mixed(unsigned long long* out16, int reset);
 size_t mixed_workspace_bytes(int Hq, int Hkv, int D, int num_reqs, int total_q);
 
 }  // namespace tropical

@@ -4,20 +4,34 @@
 // HBM-bound and tiny: T*Hkv rows of 2*d bytes each for K and V.  One thread moves the 16-byte chunk
 // `chunk` of every kv head of one (token, K|V); the d/8 threads of a row read and write 2*d contiguous
 // bytes (fully coalesced on both sides -- a (page, head, slot) row of the HND pool is contiguous).
+#include <atomic>
+
 #include "common.cuh"
 #include "kernels.h"
 
 namespace tropical {
+
+constexpr int kAppendStagedReqs = 2048;  // q_offsets kept in shared memory for the token -> request search
 
 template <int D>
 __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc b,
                                                         const uint4* __restrict__ k_new,
                                                         const uint4* __restrict__ v_new, int hg) {
     constexpr int CH = D / 8;  // 16-byte chunks per row
-    // Programmatic dependent launch: a following kernel that opted in (the plan kernel of tropical_mixed_attention,
-    // which reads only q_lens / ctx_lens) may start while this one is still copying; every other kernel keeps
-    // normal stream order.
+    // Programmatic dependent launch: a following kernel that opted in (the tile-directory kernel of
+    // tropical_mixed_attention, which reads only q_lens / ctx_lens) may start while this one is still copying; every
+    // other kernel keeps normal stream order.  The launcher keeps the grid small enough for all of its blocks to be
+    // resident at once (so that all of them trigger at once) with room left on every SM for the directory's blocks.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (threadIdx.x == 0) tl_mark(0, true);
+    // token -> request: binary search over q_offsets, from shared memory when the batch fits (one coalesced load
+    // instead of log2(n) dependent global loads per thread)
+    __shared__ int s_off[kAppendStagedReqs + 1];
+    const bool staged = b.num_reqs <= kAppendStagedReqs;
+    if (staged) {
+        for (int i = threadIdx.x; i <= b.num_reqs; i += blockDim.x) s_off[i] = __ldg(b.q_offsets + i);
+        __syncthreads();
+    }
     // One thread per (token, group of hg kv heads, K|V, 16-byte chunk): the request lookup and the (page, slot) of the
     // token are done once per thread and reused for its heads, whose rows are copied with several independent loads
     // in flight.  hg is chosen by the launcher: all heads for big steps, fewer when a step has few tokens.
@@ -31,8 +45,19 @@ __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc
         r >>= 1;
         const int h_lo = (int)(r % ngroups) * hg, h_hi = min(pool.Hkv, h_lo + hg);
         const int tok = (int)(r / ngroups);
-        const int req = find_request(b.q_offsets, b.num_reqs, tok);
-        const int t = tok - __ldg(b.q_offsets + req);
+        int req, t;
+        if (staged) {
+            int lo = 0, hi = b.num_reqs;  // invariant: s_off[lo] <= tok < s_off[hi]
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (s_off[mid] <= tok) lo = mid; else hi = mid;
+            }
+            req = lo;
+            t = tok - s_off[lo];
+        } else {
+            req = find_request(b.q_offsets, b.num_reqs, tok);
+            t = tok - __ldg(b.q_offsets + req);
+        }
         const int pos = __ldg(b.ctx_lens + req) + t;
         const int page = __ldg(b.page_table + (size_t)req * b.stride + pos / kPageSize);
         const int slot = pos % kPageSize;
@@ -49,6 +74,7 @@ __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc
         }
         for (; h < h_hi; ++h) dst[(size_t)h * kPageSize * CH] = __ldg(src + (size_t)h * CH);
     }
+    if (threadIdx.x == 0) tl_mark(1, false);
 }
 
 template <int D>
@@ -103,9 +129,8 @@ cudaError_t launch_validate_batch(const PoolDesc& pool, const BatchDesc& b, int*
     return cudaGetLastError();
 }
 
-static int grid_for(long long total_threads, int block) {
-    long long g = (total_threads + block - 1) / block;
-    const long long cap = 148LL * 8;  // grid-stride beyond 8 CTAs per SM
+static int grid_for(long long total_threads, int block, long long cap = 148LL * 8) {
+    long long g = (total_threads + block - 1) / block;  // grid-stride beyond `cap` CTAs
     if (g > cap) g = cap;
     if (g < 1) g = 1;
     return (int)g;
@@ -120,7 +145,22 @@ cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const voi
     if (hg < 1) hg = 1;
     if (hg > pool.Hkv) hg = pool.Hkv;
     const long long total = (long long)b.total_q * ((pool.Hkv + hg - 1) / hg) * (pool.D / 8) * 2;
-    const int grid = grid_for(total, 256);
+    // at most 6 blocks per SM: all resident in one wave (they trigger their programmatic dependents together) and a
+    // quarter of every SM's threads and registers stays free for the tile-directory kernel that overlaps this one.
+    // Blocks of two kernels share an SM only when both run with the same shared-memory carve-out: every kernel of
+    // the step asks for the maximum one, which the step kernel needs anyway.
+    const int grid = grid_for(total, 256, 148LL * 6);
+    {
+        static std::atomic<int> carve[64];
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (dev < 0 || dev >= 64) dev = 0;
+        if (!carve[dev].load(std::memory_order_acquire)) {
+            cudaFuncSetAttribute(kv_append_kernel<128>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+            cudaFuncSetAttribute(kv_append_kernel<64>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+            carve[dev].store(1, std::memory_order_release);
+        }
+    }
     if (pool.D == 128)
         kv_append_kernel<128><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new, (int)hg);
     else
@@ -138,6 +178,16 @@ cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, 
     else
         kv_gather_kernel<64><<<grid, 256, 0, stream>>>(pool, b, req, n_keys, (uint4*)k_dense, (uint4*)v_dense);
     return cudaGetLastError();
+}
+
+// measurement builds (-DTROPICAL_TIMELINE): this translation unit's copy of the timestamps (slots 0, 1)
+int read_timeline_append(unsigned long long* out16, int reset) {
+#ifdef TROPICAL_TIMELINE
+    return timeline_read(out16, reset);
+#else
+    (void)out16; (void)reset;
+    return 0;
+#endif
 }
 
 }  // namespace tropical

@@ -75,6 +75,7 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
     PrefillBars* PB = reinterpret_cast<PrefillBars*>(rings + M::DEC_WARPS * M::DEC_RING);
     uint64_t* dec_full = reinterpret_cast<uint64_t*>(PB + 1);
     const int warp = uni((int)(threadIdx.x >> 5));
+    if (threadIdx.x == 0) tl_mark(5, true);
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -82,12 +83,19 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
         prefill_init_bars(PB);
         for (int i = 0; i < M::N_DEC_BARS; ++i) mbar_init(dec_full + i, 1);
         fence_mbar_init();
-        prof_mark(PA.hdr, 0, true);
     }
     if (warp == 0) {
         tmem_alloc(&PB->tmem_base, C::TM_COLS);
         tmem_relinquish();
     }
+    // Programmatic dependent launch: everything above (barriers, TMEM, descriptor prefetch) touches no global memory
+    // and overlaps the tile-directory kernel and the tail of the append.  From here on the workspace and the pool are
+    // read: wait until the directory kernel has completed -- which, by its own final griddepcontrol.wait, implies
+    // that the append before it has completed and is visible.
+    if (threadIdx.x == 0) tl_mark(6, false);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (threadIdx.x == 0) tl_mark(7, true);
+    if (threadIdx.x == 0) prof_mark(PA.hdr, 0, true);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -115,6 +123,7 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
     }
     tc_fence_before();
     __syncthreads();
+    if (threadIdx.x == 0) tl_mark(8, false);
     if (warp == 0) tmem_dealloc(PB->tmem_base, C::TM_COLS);
 }
 
@@ -122,7 +131,7 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
 constexpr int kMaxDevices = 64;
 struct DeviceState {
     std::atomic<int> num_sms{0};
-    std::atomic<int> smem_attr_set{0};  // bit 0: mixed_kernel<128>, bit 1: mixed_kernel<64>
+    std::atomic<int> smem_attr_set{0};  // bit 0: mixed_kernel<128>, bit 1: mixed_kernel<64>, bit 2: plan_kernel carve-out
 };
 static DeviceState g_dev[kMaxDevices];
 
@@ -222,12 +231,20 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     P.group_cnt = (int*)(ws + w.group_cnt);
     // The plan reads only the step's metadata and writes only the workspace: launched with programmatic stream
     // serialization it overlaps a preceding tropical_kv_append (whose kernel triggers at once), and its last
-    // statement is griddepcontrol.wait, so the step kernel behind it -- a normal launch -- starts only after the
-    // append has completed.  After a kernel that never triggers it starts in normal stream order.  Contract for
+    // statement is griddepcontrol.wait.  The step kernel behind it is a programmatic dependent of the directory kernel
+    // in turn: it sets up its barriers and tensor memory early and executes griddepcontrol.wait before its first read
+    // of the workspace or the pool, so it reads them only after the directory kernel -- hence the append -- has
+    // completed.  After a kernel that never triggers, each of the two starts in normal stream order.  Contract for
     // callers (include/tropical.h): a preceding kernel that triggers early must not still be writing q_lens /
     // ctx_lens / q_offsets / page_table.
+    DeviceState& ds = device_state();
+    if (!(ds.smem_attr_set.load(std::memory_order_acquire) & 4)) {
+        // same shared-memory carve-out as the append and the step kernel: its blocks can then share SMs with theirs
+        cudaFuncSetAttribute(plan_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        ds.smem_attr_set.fetch_or(4, std::memory_order_release);
+    }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(b.num_reqs <= kPlanStagedReqs ? 8 : 1);  // see plan_kernel: several blocks share the work lists
+    cfg.gridDim = dim3(kPlanBlocks);  // see plan_kernel: the blocks share the work lists
     cfg.blockDim = dim3(kPlanThreads);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = stream;
@@ -275,7 +292,6 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     debug_wait_setup();
 #endif
     // A3 + A4 + A5 in one persistent launch
-    DeviceState& ds = device_state();
     const size_t smem = MixedCfg<D>::SMEM;
     const int attr_bit = D == 128 ? 1 : 2;
     if (!(ds.smem_attr_set.load(std::memory_order_acquire) & attr_bit)) {
@@ -284,8 +300,14 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
         ds.smem_attr_set.fetch_or(attr_bit, std::memory_order_release);
     }
     const int cap = g_grid_cap.load(std::memory_order_relaxed), sms = num_sms(ds);
-    mixed_kernel<D><<<(cap > 0 && cap < sms) ? cap : sms, kMixedThreads, smem, stream>>>(PA, A, tm_q, tm_k, tm_v);
-    e = cudaGetLastError();
+    cudaLaunchConfig_t mcfg = {};
+    mcfg.gridDim = dim3((cap > 0 && cap < sms) ? cap : sms);
+    mcfg.blockDim = dim3(kMixedThreads);
+    mcfg.dynamicSmemBytes = smem;
+    mcfg.stream = stream;
+    mcfg.attrs = attr;  // programmatic stream serialization: its prologue overlaps the directory kernel (which triggers at once)
+    mcfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&mcfg, mixed_kernel<D>, PA, A, tm_q, tm_k, tm_v);
     if (e != cudaSuccess) return e;
     ++*launches;
 
@@ -296,6 +318,16 @@ cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, con
                                    float scale_log2, void* workspace, cudaStream_t stream, int* launches) {
     if (pool.D == 128) return launch_mixed_t<128>(pool, b, q, out, lse, scale_log2, workspace, stream, launches);
     return launch_mixed_t<64>(pool, b, q, out, lse, scale_log2, workspace, stream, launches);
+}
+
+// measurement builds (-DTROPICAL_TIMELINE): this translation unit's copy of the timestamps (slots 2 .. 8)
+int read_timeline_mixed(unsigned long long* out16, int reset) {
+#ifdef TROPICAL_TIMELINE
+    return timeline_read(out16, reset);
+#else
+    (void)out16; (void)reset;
+    return 0;
+#endif
 }
 
 }  // namespace tropical

@@ -64,12 +64,39 @@ __device__ __forceinline__ int find_owner(const int4* __restrict__ info, int n, 
     return lo;
 }
 
-constexpr int kPlanThreads = 1024;
+constexpr int kPlanThreads = 256;      // small blocks with few registers: they find room beside the append's blocks
+constexpr int kPlanBlocks = 16;        // each block rebuilds the (cheap) per-request directory and writes a share of the lists
 constexpr int kPlanStagedReqs = 1024;  // per-request bases kept in shared memory for the ticket -> request search
 
+// block-wide exclusive scan of one int per thread (256 threads): returns the exclusive prefix, *total = block sum
+__device__ __forceinline__ int plan_block_scan(int v, int* s_warp, int* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int incl = v;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += t;
+    }
+    __syncthreads();  // s_warp may still be read from a previous scan
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    int base = 0, sum = 0;
+#pragma unroll
+    for (int w = 0; w < kPlanThreads / 32; ++w) {
+        const int t = s_warp[w];
+        if (w < warp) base += t;
+        sum += t;
+    }
+    *total = sum;
+    return base + incl - v;
+}
+
 __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split) {
-    __shared__ int s_units[kPlanThreads], s_items[kPlanThreads];
-    __shared__ int s_pages;
+    // the step kernel (a programmatic dependent of this one) may start its prologue now; it waits for this kernel's
+    // completion before it reads the workspace
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (threadIdx.x == 0) tl_mark(2, true);
+    __shared__ int s_warp[kPlanThreads / 32];
     __shared__ int s_ub[kPlanStagedReqs], s_ib[kPlanStagedReqs], s_ns[kPlanStagedReqs], s_pg[kPlanStagedReqs];
     const int tid = threadIdx.x;
     const int g = Hq / Hkv;
@@ -79,18 +106,15 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     // (and its K/V tiles in shared memory); otherwise one head per item
     const int pair = (g % 2 == 0) ? 1 : 0;
     const int ipt = pair ? Hq / 2 : Hq;
-    const int chunk = (n + kPlanThreads - 1) / kPlanThreads;
+    const int chunk = (n + kPlanThreads - 1) / kPlanThreads;  // requests per thread (contiguous: prefix sums)
     const int i0 = tid * chunk, i1 = min(n, i0 + chunk);
 
-    if (tid == 0) s_pages = 0;
-    __syncthreads();
     int my_pages = 0;
     for (int i = i0; i < i1; ++i)
-        if (b.q_lens[i] == 1) my_pages += (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
-    my_pages = __reduce_add_sync(0xffffffffu, my_pages);
-    if ((tid & 31) == 0 && my_pages) atomicAdd(&s_pages, my_pages);
-    __syncthreads();
-    const long long page_heads = (long long)s_pages * Hkv * HB;
+        if (__ldg(b.q_lens + i) == 1) my_pages += (__ldg(b.ctx_lens + i) + 1 + kPageSize - 1) / kPageSize;
+    int total_pages;
+    plan_block_scan(my_pages, s_warp, &total_pages);
+    const long long page_heads = (long long)total_pages * Hkv * HB;
     int split = (int)((page_heads + kTargetUnits - 1) / kTargetUnits);
     if (split < kMinSplitPages) split = kMinSplitPages;
     split = (split + 7) / 8 * 8;  // whole 128-key blocks: only a request's last unit is ragged
@@ -99,32 +123,22 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
 
     int my_units = 0, my_items = 0;
     for (int i = i0; i < i1; ++i) {
-        const int q = b.q_lens[i];
+        const int q = __ldg(b.q_lens + i);
         if (q == 1) {
-            const int pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+            const int pages = (__ldg(b.ctx_lens + i) + 1 + kPageSize - 1) / kPageSize;
             my_units += ((pages + split - 1) / split) * Hkv * HB;
         } else if (q > 1) {
             my_items += ((q + kQTile - 1) / kQTile) * ipt;
         }
     }
-    s_units[tid] = my_units;
-    s_items[tid] = my_items;
-    __syncthreads();
-    for (int off = 1; off < kPlanThreads; off <<= 1) {  // inclusive Hillis-Steele scan
-        int u = 0, it = 0;
-        if (tid >= off) { u = s_units[tid - off]; it = s_items[tid - off]; }
-        __syncthreads();
-        s_units[tid] += u;
-        s_items[tid] += it;
-        __syncthreads();
-    }
-    int ubase = s_units[tid] - my_units, ibase = s_items[tid] - my_items;
-    const int n_units = s_units[kPlanThreads - 1], n_items = s_items[kPlanThreads - 1];
+    int n_units, n_items;
+    int ubase = plan_block_scan(my_units, s_warp, &n_units);
+    int ibase = plan_block_scan(my_items, s_warp, &n_items);
     for (int i = i0; i < i1; ++i) {
-        const int q = b.q_lens[i];
+        const int q = __ldg(b.q_lens + i);
         int4 info = make_int4(0, ubase, 0, ibase);
         if (q == 1) {
-            const int pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
+            const int pages = (__ldg(b.ctx_lens + i) + 1 + kPageSize - 1) / kPageSize;
             info.x = 1;
             info.z = (pages + split - 1) / split;
             ubase += info.z * Hkv * HB;
@@ -138,7 +152,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
             s_ib[i] = info.w;
             s_ns[i] = info.z;
             // decode request: pages of its context; prefill request: its 128-row query tiles
-            s_pg[i] = info.x == 1 ? (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize : (q + kQTile - 1) / kQTile;
+            s_pg[i] = info.x == 1 ? (__ldg(b.ctx_lens + i) + 1 + kPageSize - 1) / kPageSize : (q + kQTile - 1) / kQTile;
         }
     }
     if (tid == 0 && blockIdx.x == 0) {
@@ -151,12 +165,19 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         prof[0] = ~0ull;
         prof[1] = prof[2] = prof[3] = 0ull;
     }
-    __syncthreads();  // req_info visible to the whole block (same-block global writes + barrier)
-
-    // ticket -> request: binary search over the per-request bases, staged in shared memory when they fit (the
-    // dependent global loads of the search made this kernel ~20 us for a few hundred requests); then the blocks of
-    // the grid (several only in the staged case, each with its own copy of the directory) share the two work lists
     const bool staged = n <= kPlanStagedReqs;
+    if (!staged && gridDim.x > 1) {
+        // the un-staged search reads req_info from global memory, which only block 0 writes: one block does it all
+        if (blockIdx.x != 0) {
+            asm volatile("griddepcontrol.wait;" ::: "memory");
+            return;
+        }
+    }
+    __syncthreads();  // the directory (shared memory, or block 0's global writes) is visible to the whole block
+
+    // ticket -> request: binary search over the per-request bases, staged in shared memory when they fit; the blocks
+    // of the grid (each with its own copy of the directory) share the two work lists
+    const int nblk = staged ? gridDim.x : 1, blk = staged ? blockIdx.x : 0;
     auto owner = [&](const int* base_s, int field, int e) {
         if (!staged) return field == 1 ? find_owner<1>(P.req_info, n, e) : find_owner<3>(P.req_info, n, e);
         int lo = 0, hi = n;
@@ -166,17 +187,17 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         }
         return lo;
     };
-    for (int e = blockIdx.x * kPlanThreads + tid; e < n_units; e += gridDim.x * kPlanThreads) {
+    for (int e = blk * kPlanThreads + tid; e < n_units; e += nblk * kPlanThreads) {
         const int i = owner(s_ub, 1, e);
-        int ubase, nsplit, pages;
+        int ub, nsplit, pages;
         if (staged) {
-            ubase = s_ub[i]; nsplit = s_ns[i]; pages = s_pg[i];
+            ub = s_ub[i]; nsplit = s_ns[i]; pages = s_pg[i];
         } else {
             const int4 info = P.req_info[i];
-            ubase = info.y; nsplit = info.z;
+            ub = info.y; nsplit = info.z;
             pages = (b.ctx_lens[i] + 1 + kPageSize - 1) / kPageSize;
         }
-        const int u = e - ubase;
+        const int u = e - ub;
         const int hb = u % HB;
         const int s = (u / HB) % nsplit;
         const int kvh = u / (HB * nsplit);
@@ -184,7 +205,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         P.units[e] = make_int4(i, kvh | (hb << 16), p0, min(split, pages - p0));
         P.group_cnt[e] = 0;
     }
-    for (int e = blockIdx.x * kPlanThreads + tid; e < n_items; e += gridDim.x * kPlanThreads) {
+    for (int e = blk * kPlanThreads + tid; e < n_items; e += nblk * kPlanThreads) {
         const int i = owner(s_ib, 3, e);
         const int local = e - (staged ? s_ib[i] : P.req_info[i].w);
         const int ntile = staged ? s_pg[i] : (b.q_lens[i] + kQTile - 1) / kQTile;
@@ -192,11 +213,13 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         P.items[e] = make_int2(i, (qt << 16) | (pair << 15) | ((local % ipt) << pair));
     }
     // Programmatic dependent launch: this kernel may have started while the kernel before it on the stream (the
-    // append, which triggers at its first instruction) was still running.  The step kernel is launched in normal
-    // stream order behind this one and reads what the append wrote, so completion of the plan must imply completion
-    // and visibility of the append: griddepcontrol.wait returns once every prerequisite grid has completed and its
-    // memory is flushed (PTX ISA, griddepcontrol); it is a no-op when there is no programmatic dependency.
+    // append, which triggers at its first instruction) was still running.  The step kernel behind this one reads what
+    // the append wrote, so completion of this kernel must imply completion and visibility of the append:
+    // griddepcontrol.wait returns once every prerequisite grid has completed and its memory is flushed (PTX ISA,
+    // griddepcontrol); it is a no-op when there is no programmatic dependency.
+    if (threadIdx.x == 0) tl_mark(3, false);
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (threadIdx.x == 0) tl_mark(4, false);
 }
 
 }  // namespace tropical
