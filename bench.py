@@ -179,12 +179,16 @@ def whole_job_tokens_per_s(new_tokens_per_replica: float, world: int, us_per_ste
     return new_tokens_per_replica * world / (us_per_step * 1e-6)
 
 
-def make_workload(name: str, rank: int):
+def make_workload(name: str, rank: int, part: str = "all"):
+    """part = "prefill" / "decode": only those requests of the config (analysis runs: what each role costs alone)."""
     t0 = time.perf_counter()
-    if rank == 0:
+    if rank == 0 and part == "all":
         s = synth.make_config(name, poison=False, values="tiled")
     else:  # replica with the same lengths, different page placement / values
         seed, Hq, Hkv, d, P, q, c, _ = synth.config_lengths(name)
+        if part != "all":
+            keep = (q > 1) if part == "prefill" else (q == 1)
+            q, c = q[keep], c[keep]
         s = synth.make_step(np.random.default_rng(1000 + rank), Hq, Hkv, d, P, q, c, poison=False, values="tiled",
                             name=name, seed=seed)
     return s, time.perf_counter() - t0
@@ -428,7 +432,7 @@ def run_ours(args, rank, world):
     peaks = load_peaks()
     if args.config == "MIG":
         return run_migration(args, rank, world, local, tb, torch, dist, peaks)
-    s, gen_s = make_workload(args.config, rank)
+    s, gen_s = make_workload(args.config, rank, args.part)
     st = StepTimer(s, tb, torch)
     cnt = st.cnt
     warm = max(args.warmup, 3)
@@ -455,7 +459,7 @@ def run_ours(args, rank, world):
     tl = st.timeline()
 
     extra = {}
-    if args.config == "C5" and not args.no_extra and world == 1:
+    if args.config == "C5" and args.part == "all" and not args.no_extra and world == 1:
         extra = run_extras(args, tb, torch, peaks, local, st)
     if rank != 0:
         return
@@ -470,7 +474,8 @@ def run_ours(args, rank, world):
         "metric": METRIC, "value": round(us, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": warm, "ms_per_step": round(ms_per_step, 5), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{args.config} ({describe(args.config)})", "replicas": world,
+        "config": {"workload": f"{args.config} ({describe(args.config)})" +
+                               ("" if args.part == "all" else f", its {args.part} requests only (analysis run)"), "replicas": world,
                    "l2": "step touches %.2f GB >> 126 MB L2, no flush needed" % (cnt["step_bytes"] / 1e9)
                    if not st.flush else "L2 flushed (512 MB rewritten, untimed) between timed steps; per-step event times summed",
                    "new_tokens_per_step": int(cnt["new_tokens"])},
@@ -508,6 +513,8 @@ def run_ours(args, rank, world):
         line["timeline_us"] = dict(tl, note="-DTROPICAL_TIMELINE build: not a bench build; L2 flushed before each step")
     if extra:
         line["extra"] = extra
+    if "WHATIF" in tb.version():
+        line["invalid"] = tb.version()   # a what-if measurement build computes wrong results: never a bench value
     print(json.dumps(line))
 
 
@@ -628,6 +635,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", default="C5", choices=synth.CONFIG_NAMES + ("MIG",))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--part", default="all", choices=["all", "prefill", "decode"],
+                    help="analysis runs: only the prefill (q > 1) or only the decode (q = 1) requests of the config")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-extra", action="store_true", help="skip extra.C4 / extra.MIG on the default run")
     ap.add_argument("--sustain-seconds", type=float, default=2.0, help="length of the sustained loop (0 = skip)")

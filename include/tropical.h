@@ -202,6 +202,56 @@ int tropical_step_cost(const tropical_cost_model_t *model, int32_t num_q_heads,
                        const int32_t *q_lens_host, const int32_t *ctx_lens_host, double *out_us,
                        tropical_cost_breakdown_t *breakdown /* nullable */);
 
+/* predicted microseconds of a WHOLE model iteration on one GPU of a worker (the toggle
+ * predicts "the execution time of a prefill request" and of the decoding batch with offline profiling; TP = 2
+ * inside a worker).  Pure host code, reentrant.  Per layer, on one GPU of a tp-way tensor-parallel group:
+ *   attention + KV append : tropical_step_cost on this GPU's head shard (Hq/tp, Hkv/tp, d) -- the path shards by kv head
+ *                           with no collective;
+ *   linear layers         : QKV [d_model x (Hq+2Hkv)d/tp], O [Hq d/tp x d_model], (gate and) up [d_model x (1 or 2)
+ *                           d_ffn/tp], down [d_ffn/tp x d_model] as bf16 GEMMs over the T new tokens of the batch:
+ *                             W = sum_j K_j N_j,  F = 2 T W,  B = 2 W + 2 T sum_j (K_j + N_j)
+ *                             t_lin = g0 + max(f F, w B) + kappa min(f F, w B)
+ *                           (weights streamed once per layer, activations in and out; same overlap form as the step);
+ *   all-reduce (tp > 1)   : two per layer over T d_model bf16 values: 2 (ar0 + ar_b * 2 T d_model).
+ *   total = num_layers * (attention + linear + all-reduce).
+ * linear == NULL selects the built-in fit of `python -m paper_2606_16264_b200.cost_fit measure-gemm | fit` (library
+ * GEMMs on a B200; its all-reduce coefficients are 0: one GPU is all that could be measured).
+ * attn == NULL selects the built-in step model of the SHARD shape, else TROPICAL_ERR_UNCALIBRATED.  No norms, RoPE,
+ * sampling or embedding: the form is this build's (parity unpinned, like row A6).
+ * INVALID_ARG: null shape, non-positive sizes, tp not dividing num_kv_heads / d_ffn, and whatever tropical_step_cost
+ * rejects. */
+typedef struct {
+    int32_t d_model;     /* hidden size */
+    int32_t d_ffn;       /* FFN inner size */
+    int32_t gated_mlp;   /* 1: gate, up and down projections; 0: up and down */
+    int32_t num_layers;  /* >= 1 */
+    int32_t tp;          /* tensor-parallel degree >= 1: heads and FFN columns split tp ways */
+} tropical_layer_shape_t;
+
+typedef struct {
+    double g0_us;           /* fixed cost of a layer's four GEMM launches */
+    double f_us_per_flop;   /* library-GEMM tensor throughput */
+    double w_us_per_byte;   /* streaming of weights and activations */
+    double kappa;           /* how imperfectly the two overlap, in [0, 1] */
+    double ar0_us;          /* per all-reduce: latency */
+    double ar_us_per_byte;  /* per all-reduce: per byte of the reduced tensor */
+} tropical_linear_model_t;
+
+typedef struct {
+    double attn_us;       /* one layer: append + attention of this GPU's head shard */
+    double linear_us;     /* one layer: the four GEMMs of this GPU's shard */
+    double allreduce_us;  /* one layer: its two all-reduces (0 when tp == 1) */
+    double gemm_flops;    /* F above */
+    double gemm_bytes;    /* B above */
+    double total_us;      /* num_layers * (attn_us + linear_us + allreduce_us) */
+} tropical_iter_breakdown_t;
+
+int tropical_iter_cost(const tropical_cost_model_t *attn /* nullable */, const tropical_linear_model_t *linear /* nullable */,
+                       const tropical_layer_shape_t *shape, int32_t num_q_heads, int32_t num_kv_heads,
+                       int32_t head_dim, int32_t page_size, int32_t num_reqs, const int32_t *q_lens_host,
+                       const int32_t *ctx_lens_host, double *out_us /* nullable */,
+                       tropical_iter_breakdown_t *breakdown /* nullable */);
+
 /* Number of kernel launches the last tropical_kv_append / tropical_mixed_attention /
  * tropical_step_host call on this thread enqueued (bench.py's gpu_launches). */
 int tropical_last_launch_count(void);

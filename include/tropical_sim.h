@@ -42,7 +42,19 @@
  *      A request whose TTFT slack is already <= 0 goes to the prefill worker with the least predicted queue time
  *        (it cannot meet its SLO any more; it must not starve) [R].
  *    After a Path-1 prefill the request is placed like a disaggregated one (decode queue -> multiplexing worker with
- *    the fewest unfinished tokens, with migration).  Role transitions are not modelled.
+ *    the fewest unfinished tokens, with migration).
+ *  - Role transitions (role_transitions = 1, MULTIPLEXED only), checked at the start of every toggle scan [R]:
+ *      prefill -> multiplexing: "when the watermark of all decode workers exceeds its threshold ... prefill workers can
+ *        be directly assigned as multiplexing workers": if every multiplexing worker holds more than hbm_watermark *
+ *        kv_capacity_tokens KV tokens and at least two prefill workers exist (one must remain for Path 1), the prefill
+ *        worker with the least predicted queue time becomes a multiplexing worker on the spot: it keeps its local queue
+ *        and the requests it finishes prefilling from then on stay resident on it.
+ *      multiplexing -> prefill: "if prefill frequently encounters delays ... a transition from multiplexing workers
+ *        back to prefill workers": a delayed prefill is one dispatched by the no-starvation rule; once delay_threshold
+ *        of them have occurred since the last such transition and at least two multiplexing workers exist, the lowest-
+ *        indexed multiplexing worker with no resident and no arriving decode request becomes a prefill worker (if none
+ *        is free of decode state the transition waits); the counter restarts.
+ *      At most one transition of each direction per scan; with role_transitions = 0 roles are fixed by index.
  *  - Determinism: events are processed in time order, ties by worker index, then by request index.
  */
 #ifndef TROPICAL_SIM_H_
@@ -82,6 +94,13 @@ typedef struct {
     tropical_cost_model_t attn;  /* coefficients of tropical_step_cost for one layer's append + attention */
     double linear_us_per_token;  /* the rest of an iteration, linear in its new tokens */
     double iter_overhead_us;
+    /* NEXT-4: with layer.d_model > 0 an iteration lasts tropical_iter_cost(&attn, &linear, &layer, heads, batch) +
+     * iter_overhead_us (attn then holds the coefficients of the head SHARD Hq/tp, Hkv/tp), and num_layers /
+     * linear_us_per_token above are ignored. */
+    tropical_layer_shape_t layer;
+    tropical_linear_model_t linear;
+    int32_t role_transitions;    /* 1: P:161 role transitions on (policy 2); 0: roles fixed by index */
+    int32_t delay_threshold;     /* >= 1 when role_transitions: delayed prefills that trigger multiplexing -> prefill */
 } tropical_sim_config_t;
 
 typedef struct {
@@ -97,6 +116,7 @@ typedef struct {
     double makespan_us;
     int64_t iterations;
     int64_t multiplexed_prefills;
+    int64_t to_multiplexing, to_prefill; /* role transitions performed */
 } tropical_sim_summary_t;
 
 /* Runs the simulation.  requests [host] must be sorted by arrival_us (ties keep their order); results [host,

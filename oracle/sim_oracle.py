@@ -28,6 +28,25 @@ class CostModel:
 
 
 @dataclass
+class LayerShape:  # include/tropical.h tropical_layer_shape_t (NEXT-4)
+    d_model: int = 0
+    d_ffn: int = 0
+    gated_mlp: int = 1
+    num_layers: int = 1
+    tp: int = 1
+
+
+@dataclass
+class LinearModel:  # include/tropical.h tropical_linear_model_t
+    g0_us: float = 0.0
+    f_us_per_flop: float = 0.0
+    w_us_per_byte: float = 0.0
+    kappa: float = 0.0
+    ar0_us: float = 0.0
+    ar_us_per_byte: float = 0.0
+
+
+@dataclass
 class Config:
     policy: int
     num_workers: int
@@ -47,11 +66,16 @@ class Config:
     attn: CostModel
     linear_us_per_token: float
     iter_overhead_us: float
+    layer: LayerShape = field(default_factory=LayerShape)   # d_model > 0: iterations cost iter_cost_us (NEXT-4)
+    linear: LinearModel = field(default_factory=LinearModel)
+    role_transitions: int = 0
+    delay_threshold: int = 0
 
 
-def step_cost_us(cfg: Config, q_lens: List[int], ctx_lens: List[int]) -> float:
-    """t = t0 + max(aF, bB) + kappa min(aF, bB) + e_p N_p / n_sm + e_d N_d / n_sm (DESIGN.md sections 6, 7)."""
-    Hq, Hkv, d, P = cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim, cfg.page_size
+def step_cost_us(cfg: Config, q_lens: List[int], ctx_lens: List[int], tp: int = 1) -> float:
+    """t = t0 + max(aF, bB) + kappa min(aF, bB) + e_p N_p / n_sm + e_d N_d / n_sm (DESIGN.md sections 6, 7), on the
+    head shard Hq/tp, Hkv/tp (the path shards by kv head with no collective)."""
+    Hq, Hkv, d, P = cfg.num_q_heads // tp, cfg.num_kv_heads // tp, cfg.head_dim, cfg.page_size
     qc = pages = T = csum = 0.0
     iters = units = 0
     for q, c in zip(q_lens, ctx_lens):
@@ -78,7 +102,29 @@ def step_cost_us(cfg: Config, q_lens: List[int], ctx_lens: List[int]) -> float:
     return m.t0_us + hi + m.kappa * lo + m.e_prefill_iter_us * iters / nsm + m.e_decode_unit_us * units / nsm
 
 
+def iter_cost_us(cfg: Config, q_lens: List[int], ctx_lens: List[int]) -> float:
+    """include/tropical.h tropical_iter_cost: layers * (attention on the head shard + four GEMMs + two all-reduces)."""
+    sh, lm = cfg.layer, cfg.linear
+    T = float(sum(q_lens))
+    mats = [(sh.d_model, (cfg.num_q_heads + 2 * cfg.num_kv_heads) * cfg.head_dim / sh.tp),     # QKV
+            (cfg.num_q_heads * cfg.head_dim / sh.tp, sh.d_model),                               # O
+            (sh.d_model, (2 if sh.gated_mlp else 1) * sh.d_ffn / sh.tp),                        # (gate and) up
+            (sh.d_ffn / sh.tp, sh.d_model)]                                                     # down
+    weights = sum(k * n for k, n in mats)
+    flops = 2.0 * T * weights
+    nbytes = 2.0 * weights + 2.0 * T * sum(k + n for k, n in mats)
+    linear = allreduce = 0.0
+    if T > 0:
+        tf, tw = lm.f_us_per_flop * flops, lm.w_us_per_byte * nbytes
+        linear = lm.g0_us + max(tf, tw) + lm.kappa * min(tf, tw)
+        if sh.tp > 1:
+            allreduce = 2.0 * (lm.ar0_us + lm.ar_us_per_byte * 2.0 * T * sh.d_model)
+    return sh.num_layers * (step_cost_us(cfg, q_lens, ctx_lens, sh.tp) + linear + allreduce)
+
+
 def iter_time_us(cfg: Config, q_lens: List[int], ctx_lens: List[int]) -> float:
+    if cfg.layer.d_model > 0:
+        return iter_cost_us(cfg, q_lens, ctx_lens) + cfg.iter_overhead_us
     return cfg.num_layers * step_cost_us(cfg, q_lens, ctx_lens) + cfg.linear_us_per_token * sum(q_lens) + cfg.iter_overhead_us
 
 
@@ -112,14 +158,23 @@ def simulate(cfg: Config, requests: List[tuple]):
     results[i] = dict(ttft_us, tpot_us, first_token_us, finish_us, prefill_worker, decode_worker, multiplexed)."""
     R = [_Req(float(a), int(p), int(o)) for a, p, o in requests]
     W = [_Worker() for _ in range(cfg.num_workers)]
-    np_ = 0 if cfg.policy == COLOCATED else cfg.num_prefill_workers
+    # role of each worker: True = dedicated prefill worker (disaggregated / multiplexed policies); P:161 may change it
+    prefill_role = [cfg.policy != COLOCATED and w < cfg.num_prefill_workers for w in range(cfg.num_workers)]
     toggle_q: List[int] = []
     next_arrival = 0
     iterations = 0
     now = 0.0
+    delayed = 0                      # prefills sent by the no-starvation rule since the last multiplexing -> prefill transition
+    transitions = [0, 0]             # [to multiplexing, to prefill]
 
-    def is_prefill_worker(w):  # dedicated prefill worker of the disaggregated / multiplexed policies
-        return cfg.policy != COLOCATED and w < np_
+    def is_prefill_worker(w):
+        return prefill_role[w]
+
+    def prefill_workers():
+        return [w for w in range(cfg.num_workers) if prefill_role[w]]
+
+    def mux_workers():
+        return [w for w in range(cfg.num_workers) if not prefill_role[w]]
 
     def remaining_output(r):
         return R[r].output - 1 - R[r].generated
@@ -157,7 +212,7 @@ def simulate(cfg: Config, requests: List[tuple]):
         return [1] * len(W[w].resident), [R[r].prompt + R[r].generated for r in W[w].resident]
 
     def place_for_decode(r):  # after a prefill on a dedicated prefill worker: P:155 decode queue, P:186 dispatch
-        best = min(range(np_, cfg.num_workers), key=lambda w: (unfinished_tokens(w), w))
+        best = min(mux_workers(), key=lambda w: (unfinished_tokens(w), w))
         W[best].pending.append((now + cfg.migrate_us_per_token * R[r].prompt, r))
         R[r].decode_worker = best
 
@@ -211,12 +266,29 @@ def simulate(cfg: Config, requests: List[tuple]):
         wk.busy_until = now + iter_time_us(cfg, q_lens, ctx_lens)
         iterations += 1
 
+    def role_transitions():  # P:161, readings of include/tropical_sim.h
+        nonlocal delayed
+        threshold = cfg.hbm_watermark * cfg.kv_capacity_tokens
+        if all(resident_kv(w) > threshold for w in mux_workers()) and len(prefill_workers()) >= 2:
+            w = min(prefill_workers(), key=lambda w: (pred_queue(w), w))
+            prefill_role[w] = False
+            transitions[0] += 1
+        if delayed >= cfg.delay_threshold and len(mux_workers()) >= 2:
+            free = [w for w in mux_workers() if not W[w].resident and not W[w].pending]
+            if free:
+                prefill_role[free[0]] = True
+                transitions[1] += 1
+                delayed = 0
+
     def toggle_scan():
+        nonlocal delayed
+        if cfg.role_transitions:
+            role_transitions()
         for r in list(toggle_q):
             waited = now - R[r].arrival
             target, mux = -1, 0
             # Path 2: multiplexing workers with an empty local queue, fewest unfinished tokens first
-            cands = sorted((w for w in range(np_, cfg.num_workers) if not W[w].local_q), key=lambda w: (unfinished_tokens(w), w))
+            cands = sorted((w for w in mux_workers() if not W[w].local_q), key=lambda w: (unfinished_tokens(w), w))
             for w in cands:
                 dq, dc = decode_batch(w)
                 t_dec = iter_time_us(cfg, dq, dc) if dq else 0.0
@@ -236,10 +308,13 @@ def simulate(cfg: Config, requests: List[tuple]):
                     target, mux = w, 1
                     break
             if target < 0:  # Path 1, or the no-starvation rule once the TTFT slack is gone
-                best = min(range(np_), key=lambda w: (pred_queue(w), w))
+                best = min(prefill_workers(), key=lambda w: (pred_queue(w), w))
                 slack_ttft = cfg.ttft_slo_us - waited
                 slack_gone = now >= R[r].arrival + cfg.ttft_slo_us  # the expression the wake-up event is scheduled with
-                if slack_gone or pred_exec(r) + pred_queue(best) < slack_ttft:
+                if slack_gone:
+                    target = best
+                    delayed += 1     # a delayed prefill
+                elif pred_exec(r) + pred_queue(best) < slack_ttft:
                     target = best
             if target >= 0:
                 toggle_q.remove(r)
@@ -258,7 +333,7 @@ def simulate(cfg: Config, requests: List[tuple]):
                 W[w].local_q.append(r)
                 R[r].prefill_worker = w
             elif cfg.policy == DISAGGREGATED:
-                w = min(range(np_), key=lambda w: (pred_queue(w), w))
+                w = min(prefill_workers(), key=lambda w: (pred_queue(w), w))
                 W[w].local_q.append(r)
                 R[r].prefill_worker = w
             else:
@@ -292,7 +367,9 @@ def simulate(cfg: Config, requests: List[tuple]):
         results.append(dict(ttft_us=ttft, tpot_us=tpot,
                             first_token_us=x.first_token, finish_us=x.finish, prefill_worker=x.prefill_worker,
                             decode_worker=x.decode_worker, multiplexed=x.multiplexed))
-    return results, summarize(cfg, results, iterations)
+    summary = summarize(cfg, results, iterations)
+    summary["to_multiplexing"], summary["to_prefill"] = transitions
+    return results, summary
 
 
 def summarize(cfg: Config, results, iterations: int):

@@ -8,6 +8,9 @@ from .binding import (  # noqa: F401
     Batch,
     CostBreakdown,
     CostModel,
+    IterBreakdown,
+    LayerShape,
+    LinearModel,
     KVPool,
     SIM_COLOCATED,
     SIM_DISAGGREGATED,
@@ -21,6 +24,7 @@ from .binding import (  # noqa: F401
     debug_timeline,
     debug_set_split_pages,
     debug_wait_profile,
+    iter_cost,
     kv_append,
     kv_gather,
     kv_migrate,

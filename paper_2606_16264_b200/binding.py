@@ -45,6 +45,22 @@ class CostBreakdown(ctypes.Structure):
                 ("decode_units", ctypes.c_int64)]
 
 
+class LayerShape(ctypes.Structure):
+    """include/tropical.h: tropical_layer_shape_t (NEXT-4)."""
+    _fields_ = [("d_model", ctypes.c_int32), ("d_ffn", ctypes.c_int32), ("gated_mlp", ctypes.c_int32),
+                ("num_layers", ctypes.c_int32), ("tp", ctypes.c_int32)]
+
+
+class LinearModel(ctypes.Structure):
+    _fields_ = [("g0_us", ctypes.c_double), ("f_us_per_flop", ctypes.c_double), ("w_us_per_byte", ctypes.c_double),
+                ("kappa", ctypes.c_double), ("ar0_us", ctypes.c_double), ("ar_us_per_byte", ctypes.c_double)]
+
+
+class IterBreakdown(ctypes.Structure):
+    _fields_ = [("attn_us", ctypes.c_double), ("linear_us", ctypes.c_double), ("allreduce_us", ctypes.c_double),
+                ("gemm_flops", ctypes.c_double), ("gemm_bytes", ctypes.c_double), ("total_us", ctypes.c_double)]
+
+
 class SimRequest(ctypes.Structure):
     _fields_ = [("arrival_us", ctypes.c_double), ("prompt_len", ctypes.c_int32), ("output_len", ctypes.c_int32)]
 
@@ -57,7 +73,9 @@ class SimConfig(ctypes.Structure):
                 ("kv_capacity_tokens", ctypes.c_int64), ("migrate_us_per_token", ctypes.c_double),
                 ("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
                 ("page_size", ctypes.c_int32), ("num_layers", ctypes.c_int32), ("attn", CostModel),
-                ("linear_us_per_token", ctypes.c_double), ("iter_overhead_us", ctypes.c_double)]
+                ("linear_us_per_token", ctypes.c_double), ("iter_overhead_us", ctypes.c_double),
+                ("layer", LayerShape), ("linear", LinearModel), ("role_transitions", ctypes.c_int32),
+                ("delay_threshold", ctypes.c_int32)]
 
 
 class SimResult(ctypes.Structure):
@@ -69,14 +87,15 @@ class SimResult(ctypes.Structure):
 class SimSummary(ctypes.Structure):
     _fields_ = [("attainment", ctypes.c_double), ("ttft_mean_us", ctypes.c_double), ("ttft_p90_us", ctypes.c_double),
                 ("tpot_mean_us", ctypes.c_double), ("tpot_p90_us", ctypes.c_double), ("makespan_us", ctypes.c_double),
-                ("iterations", ctypes.c_int64), ("multiplexed_prefills", ctypes.c_int64)]
+                ("iterations", ctypes.c_int64), ("multiplexed_prefills", ctypes.c_int64),
+                ("to_multiplexing", ctypes.c_int64), ("to_prefill", ctypes.c_int64)]
 
 
 SIM_COLOCATED, SIM_DISAGGREGATED, SIM_MULTIPLEXED = 0, 1, 2
 
 EXPORTS = (
     "tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention",
-    "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost",
+    "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost", "tropical_iter_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
     "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile", "tropical_debug_timeline",
     "tropical_sim_run",
@@ -104,7 +123,7 @@ def lib():
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
     for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_step_host",
-                 "tropical_step_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
+                 "tropical_step_cost", "tropical_iter_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
                  "tropical_debug_read_profile"):
         getattr(L, name).restype = ctypes.c_int
     _lib = L
@@ -385,6 +404,23 @@ def step_cost(num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int
     if rc == 5 and not require_model:
         return None, bd
     _check(rc, "tropical_step_cost")
+    return us.value, bd
+
+
+def iter_cost(shape: LayerShape, num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int,
+              q_lens: Sequence[int], ctx_lens: Sequence[int], attn: Optional[CostModel] = None,
+              linear: Optional[LinearModel] = None):
+    """(predicted us of a whole iteration, IterBreakdown): include/tropical.h tropical_iter_cost.  Host only."""
+    n = len(q_lens)
+    ql = (ctypes.c_int32 * max(n, 1))(*[int(x) for x in q_lens])
+    cl = (ctypes.c_int32 * max(n, 1))(*[int(x) for x in ctx_lens])
+    us = ctypes.c_double(0.0)
+    bd = IterBreakdown()
+    _check(lib().tropical_iter_cost(ctypes.byref(attn) if attn is not None else None,
+                                    ctypes.byref(linear) if linear is not None else None, ctypes.byref(shape),
+                                    ctypes.c_int32(num_q_heads), ctypes.c_int32(num_kv_heads), ctypes.c_int32(head_dim),
+                                    ctypes.c_int32(page_size), ctypes.c_int32(n), ql, cl, ctypes.byref(us),
+                                    ctypes.byref(bd)), "tropical_iter_cost")
     return us.value, bd
 
 

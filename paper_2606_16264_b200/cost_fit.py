@@ -1,6 +1,8 @@
 """Calibration of tropical_step_cost ("offline profiling tools").
 
     python -m paper_2606_16264_b200.cost_fit measure [--out calibration/b200_grid.csv]   # needs a B200
+    python -m paper_2606_16264_b200.cost_fit measure-gemm [--out calibration/b200_gemm.csv]   # needs a B200
+    python -m paper_2606_16264_b200.cost_fit sweep-split  [--out split_sweep.csv]             # needs a B200
     python -m paper_2606_16264_b200.cost_fit fit     [--grid calibration/b200_grid.csv]  # CPU only
 
 `measure` times append + attention (CUDA events, inputs resident) over a grid of synthetic batches --
@@ -24,8 +26,10 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 DEFAULT_GRID = os.path.join(HERE, "calibration", "b200_grid.csv")
 FIT_INC = os.path.join(HERE, "csrc", "cost_model_fit.inc")
+LINEAR_INC = os.path.join(HERE, "csrc", "linear_model_fit.inc")
 
-SHAPES = [(32, 32, 128), (40, 40, 128), (64, 8, 128)]      # BASELINE.json configs[1..4]
+SHAPES = [(32, 32, 128), (40, 40, 128), (64, 8, 128),      # BASELINE.json configs[1..4]
+          (20, 20, 128), (32, 4, 128)]                      # their TP = 2 head shards (NEXT-4)
 PREFILL_TOKENS = [0, 256, 1024, 2048, 4096, 8192]
 DECODE_REQS = [0, 16, 64, 128, 256]
 CTX_MEDIANS = [256, 1024, 4096]
@@ -64,21 +68,27 @@ def grid_points():
         for nd in (0, 128):
             pts.append((2048, pc, nd, 1024 if nd else 0, seed))
             seed += 1
+    # off-grid points (seeds >= 1000, always held out): recipe values drawn between and beyond the grid lines
+    rng = np.random.default_rng(7)
+    for k in range(24):
+        pt = int(rng.choice([0, 0, 384, 768, 1536, 3072, 6144, 12288]))
+        pc = int(rng.choice([0, 0, 512, 3072, 6144])) if pt else 0
+        nd = int(rng.integers(0, 385)) if pt else int(rng.integers(1, 385))
+        cm = int(rng.choice([128, 384, 700, 1500, 2500, 6000])) if nd else 0
+        pts.append((pt, pc, nd, cm, 1000 + k))
     return pts
 
 
 # ------------------------------------------------------------------------------------------ measure (GPU)
-def measure(out_path: str, iters: int, shapes):
+def _points_on_device(shapes, pts):
+    """Yields (Hq, Hkv, d, point, step) with the point's batch resident on the GPU; step() enqueues append + attention."""
     import torch
     from . import binding as tb
 
-    assert torch.cuda.is_available(), "measure needs a GPU"
+    assert torch.cuda.is_available(), "needs a GPU"
     dev = torch.device("cuda")
     g = torch.Generator(device="cuda")
     g.manual_seed(1234)
-    os.makedirs(os.path.dirname(os.path.abspath(out_path)), exist_ok=True)
-    rows = []
-    pts = grid_points()
     for Hq, Hkv, d in shapes:
         need = [int(((q.astype(np.int64) + c + 15) // 16).sum()) for q, c in (grid_lengths(*p) for p in pts)]
         num_pages = 64 * math.ceil(1.1 * max(need) / 64)
@@ -103,29 +113,129 @@ def measure(out_path: str, iters: int, shapes):
             qd, kn, vn = rnd(Hq), rnd(Hkv), rnd(Hkv)
             out = torch.empty_like(qd)
             ws = torch.empty(tb.workspace_bytes(pool, n, T, int(L.max())) + 256, dtype=torch.uint8, device=dev)
-            stream = torch.cuda.current_stream()
 
             def step():
                 tb.kv_append(pool, batch, kn, vn)
                 tb.mixed_attention(pool, batch, qd, out=out, workspace=ws)
 
-            for _ in range(3):
-                step()
-            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
-            torch.cuda.synchronize()
-            for a, b in evs:
-                a.record(stream)
-                step()
-                b.record(stream)
-            torch.cuda.synchronize()
-            us = np.array([a.elapsed_time(b) * 1e3 for a, b in evs])
-            rows.append([Hq, Hkv, d, p[0], p[1], p[2], p[3], p[4], round(float(np.median(us)), 2), round(float(us.min()), 2)])
+            yield Hq, Hkv, d, p, step
         del k_pool, v_pool, pool
         torch.cuda.empty_cache()
+
+
+def _time_us(step, iters):
+    import torch
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        step()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    torch.cuda.synchronize()
+    for a, b in evs:
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    return np.array([a.elapsed_time(b) * 1e3 for a, b in evs])
+
+
+def measure(out_path: str, iters: int, shapes):
+    os.makedirs(os.path.dirname(os.path.abspath(out_path)), exist_ok=True)
+    rows = []
+    for Hq, Hkv, d, p, step in _points_on_device(shapes, grid_points()):
+        us = _time_us(step, iters)
+        rows.append([Hq, Hkv, d, p[0], p[1], p[2], p[3], p[4], round(float(np.median(us)), 2), round(float(us.min()), 2)])
     with open(out_path, "w", newline="") as f:
         w = csv.writer(f)
         w.writerow(COLUMNS)
         w.writerows(rows)
+    print(f"wrote {len(rows)} points to {out_path}")
+
+
+# Decode split size (pages per split-K unit, csrc/plan.cuh): step time under forced (coarser) splits, the evidence
+# behind plan_kernel's rule (profiles/r2c_split_sweep.md).  0 = the kernel's own choice.
+SWEEP_SPLITS = [0, 16, 24, 32, 48, 64, 96, 128, 256]
+
+
+def sweep_split(out_path: str, iters: int, shapes):
+    from . import binding as tb
+    pts = []
+    for nd in (16, 64, 128, 256):
+        for cm in (256, 1024, 4096):
+            pts.append((0, 0, nd, cm, 100 + nd + cm))
+    pts += [(2048, 0, 64, 1024, 71), (2048, 0, 128, 1024, 135), (4096, 0, 256, 1500, 263), (512, 0, 32, 2048, 39)]
+    rows = []
+    for Hq, Hkv, d, p, step in _points_on_device(shapes, pts):
+        us = []
+        for split in SWEEP_SPLITS:
+            tb.debug_set_split_pages(split)
+            us.append(round(float(np.median(_time_us(step, iters))), 1))
+        tb.debug_set_split_pages(0)
+        rows.append([Hq, Hkv, d, p[0], p[2], p[3]] + us)
+        print(rows[-1], flush=True)
+    with open(out_path, "w", newline="") as f:
+        w = csv.writer(f)
+        w.writerow(["Hq", "Hkv", "d", "prefill_tokens", "n_decode", "ctx_median"] + [f"us_split_{s}" for s in SWEEP_SPLITS])
+        w.writerows(rows)
+    print(f"wrote {len(rows)} rows to {out_path}")
+
+
+# ------------------------------------------------------------------------------------------ measure-gemm (GPU)
+# NEXT-4: the linear layers of one transformer layer -- QKV, O, (gate +) up, down -- as library GEMMs
+# (torch.matmul -> cuBLAS, bf16) on one GPU's shard of a tensor-parallel layer: heads and FFN columns split tp ways.
+# Calibration data for tropical_iter_cost's linear term; these GEMMs are not kernels of this repository.
+GEMM_GRID = os.path.join(HERE, "calibration", "b200_gemm.csv")
+GEMM_LAYERS = [  # (d_model, d_ffn, gated, Hq, Hkv, d, tp)
+    (4096, 11008, 1, 32, 32, 128, 1),   # 7B-like (C2 / C3 heads)
+    (5120, 13824, 1, 40, 40, 128, 1),   # 13B-like (C4 heads)
+    (5120, 13824, 1, 40, 40, 128, 2),
+    (8192, 28672, 1, 64, 8, 128, 1),    # 70B-layer-like (C5 heads)
+    (8192, 28672, 1, 64, 8, 128, 2),
+]
+GEMM_TOKENS = [1, 16, 64, 128, 256, 512, 1024, 2048, 4096, 8192]
+GEMM_COLUMNS = ["d_model", "d_ffn", "gated", "Hq", "Hkv", "d", "tp", "tokens", "us_median", "us_min"]
+
+
+def layer_matrices(d_model, d_ffn, gated, Hq, Hkv, d, tp):
+    """(K, N) of the four weight matrices one GPU of a tp-way tensor-parallel layer holds."""
+    return [(d_model, (Hq + 2 * Hkv) * d // tp), (Hq * d // tp, d_model),
+            (d_model, (2 if gated else 1) * d_ffn // tp), (d_ffn // tp, d_model)]
+
+
+def measure_gemm(out_path: str, iters: int):
+    import torch
+    assert torch.cuda.is_available(), "measure-gemm needs a GPU"
+    dev = torch.device("cuda")
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    rows = []
+    for layer in GEMM_LAYERS:
+        mats = layer_matrices(*layer)
+        w = [torch.randn(k, n, device=dev, dtype=torch.bfloat16) for k, n in mats]
+        for T in GEMM_TOKENS:
+            x = [torch.randn(T, k, device=dev, dtype=torch.bfloat16) for k, _ in mats]
+
+            def run():
+                for xi, wi in zip(x, w):
+                    torch.matmul(xi, wi)
+
+            for _ in range(3):
+                run()
+            times = []
+            for k in range(iters):
+                flush.fill_(k & 1)  # the weights of a real model do not stay in L2 from one layer to the next
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                run()
+                e1.record()
+                torch.cuda.synchronize()
+                times.append(e0.elapsed_time(e1) * 1e3)
+            times.sort()
+            rows.append(list(layer) + [T, round(times[len(times) // 2], 2), round(times[0], 2)])
+        del w
+        torch.cuda.empty_cache()
+    with open(out_path, "w", newline="") as f:
+        wr = csv.writer(f)
+        wr.writerow(GEMM_COLUMNS)
+        wr.writerows(rows)
     print(f"wrote {len(rows)} points to {out_path}")
 
 
@@ -137,7 +247,7 @@ def read_grid(path: str):
 
 
 def is_held_out(row) -> bool:
-    return row["seed"] % 5 == 0
+    return row["seed"] % 5 == 0 or row["seed"] >= 1000   # every fifth grid point and every off-grid point
 
 
 def point_features(row):
@@ -155,40 +265,107 @@ def predict(theta, X, n_sm=148.0):
     return t0 + np.maximum(tc, hb) + kappa * np.minimum(tc, hb) + ep * Np / n_sm + ed * Nd / n_sm
 
 
+# Physical lower bounds of the two roofline coefficients (nominal peaks of the part: 2250 TFLOP/s dense bf16,
+# 8 TB/s HBM3e): a fit below them would predict steps faster than the hardware can run.  The measured copy figure of
+# MEASURED_PEAKS.json is not used here: it is a read + write mix, and the step kernel has been measured above it on
+# pure reads (6.8 TB/s of DRAM reads on C4, profiles/r1f_final.md).
+A_MIN_US_PER_FLOP = 1e6 / 2250e12
+B_MIN_US_PER_BYTE = 1e6 / 8000e9
+
+
 def fit_shape(rows):
     from scipy.optimize import least_squares
     X = np.array([point_features(r) for r in rows])
     y = np.array([r["us_median"] for r in rows])
     train = np.array([not is_held_out(r) for r in rows])
+    off = np.array([r["seed"] >= 1000 for r in rows])
     scale = np.array([10.0, 1e-9, 1e-7, 1.0, 1.0, 0.01])   # parameter magnitudes (us, us/FLOP, us/byte, -, us, us)
+    lo = np.array([0, A_MIN_US_PER_FLOP / scale[1], B_MIN_US_PER_BYTE / scale[2], 0, 0, 0])
+    hi = np.array([20, 50, 50, 1, 50, 500])
     res_best = None
     for k0 in (0.1, 0.5, 0.9):
         x0 = np.array([1.0, 1.5, 1.6, k0, 0.5, 1.0])
         fun = lambda x: (predict(x * scale, X[train]) - y[train]) / y[train]
-        res = least_squares(fun, x0, bounds=(np.zeros(6), np.array([20, 50, 50, 1, 50, 500])))
+        res = least_squares(fun, x0, bounds=(lo, hi))
         if res_best is None or res.cost < res_best.cost:
             res_best = res
     theta = res_best.x * scale
     rel = np.abs(predict(theta, X) - y) / y
     stats = dict(n=len(rows), n_train=int(train.sum()), mape_train=float(rel[train].mean()),
-                 mape_held=float(rel[~train].mean()), max_held=float(rel[~train].max()), max_all=float(rel.max()))
+                 mape_held=float(rel[~train].mean()), max_held=float(rel[~train].max()), max_all=float(rel.max()),
+                 mape_off_grid=float(rel[off].mean()) if off.any() else float("nan"),
+                 max_off_grid=float(rel[off].max()) if off.any() else float("nan"))
     return theta, stats
 
 
-def fit(grid_path: str, write: bool):
+# ---- linear layers (NEXT-4): t = g0 + max(f F, w B) + kappa min(f F, w B), one coefficient set for every layer shape
+def read_gemm(path: str):
+    with open(path) as f:
+        return [{k: (float(v) if k.startswith("us_") else int(v)) for k, v in r.items()}
+                for r in csv.DictReader(l for l in f if not l.startswith("#"))]
+
+
+def gemm_features(r):
+    mats = layer_matrices(r["d_model"], r["d_ffn"], r["gated"], r["Hq"], r["Hkv"], r["d"], r["tp"])
+    W = float(sum(k * n for k, n in mats))
+    T = float(r["tokens"])
+    return 2.0 * T * W, 2.0 * W + 2.0 * T * sum(k + n for k, n in mats)
+
+
+def predict_linear(theta, X):
+    g0, f, w, kappa = theta
+    tf, tw = f * X[:, 0], w * X[:, 1]
+    return g0 + np.maximum(tf, tw) + kappa * np.minimum(tf, tw)
+
+
+def fit_linear(rows):
+    """Every fifth point (in file order) is held out."""
+    from scipy.optimize import least_squares
+    X = np.array([gemm_features(r) for r in rows])
+    y = np.array([r["us_median"] for r in rows])
+    train = np.array([i % 5 != 2 for i in range(len(rows))])
+    scale = np.array([10.0, 1e-9, 1e-7, 1.0])
+    lo = np.array([0, A_MIN_US_PER_FLOP / scale[1], B_MIN_US_PER_BYTE / scale[2], 0])
+    hi = np.array([50, 50, 50, 1])
+    best = None
+    for k0 in (0.1, 0.5, 0.9):
+        res = least_squares(lambda x: (predict_linear(x * scale, X[train]) - y[train]) / y[train],
+                            np.array([2.0, 0.8, 1.8, k0]), bounds=(lo, hi))
+        if best is None or res.cost < best.cost:
+            best = res
+    theta = best.x * scale
+    rel = np.abs(predict_linear(theta, X) - y) / y
+    return theta, dict(n=len(rows), mape_train=float(rel[train].mean()), mape_held=float(rel[~train].mean()),
+                       max_held=float(rel[~train].max()), max_all=float(rel.max()))
+
+
+def fit(grid_path: str, write: bool, gemm_path: str = None):
     rows = read_grid(grid_path)
     shapes = sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows})
     lines = ["// Generated by `python -m paper_2606_16264_b200.cost_fit fit` from calibration/b200_grid.csv.",
-             "// {Hq, Hkv, d, {t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us, n_sm}}"]
+             "// {Hq, Hkv, d, {t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us, n_sm}}",
+             "// a >= 1 / (2250 TFLOP/s) and b >= 1 / (8 TB/s) are enforced by the fit (nominal peaks of the part)."]
     for s in shapes:
         theta, st = fit_shape([r for r in rows if (r["Hq"], r["Hkv"], r["d"]) == s])
         print(f"shape {s}: theta={['%.4g' % t for t in theta]} {st}")
-        lines.append("{%d, %d, %d, {%.6g, %.6g, %.6g, %.6g, %.6g, %.6g, 148}},  // held-out MAPE %.1f %%, max %.1f %%"
-                     % (*s, *theta, 100 * st["mape_held"], 100 * st["max_held"]))
+        lines.append("{%d, %d, %d, {%.6g, %.6g, %.6g, %.6g, %.6g, %.6g, 148}},  // held-out MAPE %.1f %%, max %.1f %%; "
+                     "off-grid MAPE %.1f %%, max %.1f %%"
+                     % (*s, *theta, 100 * st["mape_held"], 100 * st["max_held"], 100 * st["mape_off_grid"],
+                        100 * st["max_off_grid"]))
+    gemm_path = gemm_path or GEMM_GRID
+    theta_l, st_l = fit_linear(read_gemm(gemm_path))
+    print(f"linear layers: theta={['%.4g' % t for t in theta_l]} {st_l}")
+    lin = ["// Generated by `python -m paper_2606_16264_b200.cost_fit fit` from calibration/b200_gemm.csv.",
+           "// {g0_us, f_us_per_flop, w_us_per_byte, kappa, ar0_us, ar_us_per_byte}; held-out MAPE %.1f %%, max %.1f %%;"
+           % (100 * st_l["mape_held"], 100 * st_l["max_held"]),
+           "// all-reduce coefficients 0: not measurable on one GPU (DESIGN.md section 7).",
+           "{%.6g, %.6g, %.6g, %.6g, 0, 0}" % tuple(theta_l)]
     if write:
         with open(FIT_INC, "w") as f:
             f.write("\n".join(lines) + "\n")
-        print("wrote", FIT_INC)
+        with open(LINEAR_INC, "w") as f:
+            f.write("\n".join(lin) + "\n")
+        print("wrote", FIT_INC, "and", LINEAR_INC)
 
 
 def main(argv=None):
@@ -198,6 +375,13 @@ def main(argv=None):
     m.add_argument("--out", default=DEFAULT_GRID)
     m.add_argument("--iters", type=int, default=15)
     m.add_argument("--shapes", default="all", help="'all' or e.g. 64/8/128")
+    sw = sub.add_parser("sweep-split")
+    sw.add_argument("--out", default="split_sweep.csv")
+    sw.add_argument("--iters", type=int, default=20)
+    sw.add_argument("--shapes", default="all")
+    mg = sub.add_parser("measure-gemm")
+    mg.add_argument("--out", default=GEMM_GRID)
+    mg.add_argument("--iters", type=int, default=20)
     f = sub.add_parser("fit")
     f.add_argument("--grid", default=DEFAULT_GRID)
     f.add_argument("--no-write", action="store_true")
@@ -205,6 +389,11 @@ def main(argv=None):
     if a.cmd == "measure":
         shapes = SHAPES if a.shapes == "all" else [tuple(int(x) for x in a.shapes.split("/"))]
         measure(a.out, a.iters, shapes)
+    elif a.cmd == "sweep-split":
+        shapes = SHAPES[:3] if a.shapes == "all" else [tuple(int(x) for x in a.shapes.split("/"))]
+        sweep_split(a.out, a.iters, shapes)
+    elif a.cmd == "measure-gemm":
+        measure_gemm(a.out, a.iters)
     else:
         fit(a.grid, not a.no_write)
 

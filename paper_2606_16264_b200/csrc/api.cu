@@ -367,7 +367,13 @@ int tropical_debug_timeline(uint64_t* out_ns, int32_t reset) {
 
 const char* tropical_last_cuda_error(void) { return g_cuda_err; }
 
-const char* tropical_version(void) { return "tropical-b200 0.1 (sm_100a)"; }
+const char* tropical_version(void) {
+#ifdef TROPICAL_WHATIF_BUILD
+    return "tropical-b200 0.2 (sm_100a) WHATIF measurement build: attention results are wrong by design";
+#else
+    return "tropical-b200 0.2 (sm_100a)";
+#endif
+}
 
 }  // extern "C"
 

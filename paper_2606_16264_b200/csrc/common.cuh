@@ -34,6 +34,15 @@ static inline int timeline_read(unsigned long long* out16, int reset) {
 __device__ __forceinline__ void tl_mark(int, bool) {}
 #endif
 
+// Measurement builds only, WRONG RESULTS by design (profiles/r2b_whatif.md: what each part of the fused step costs under
+// the board's power limit): -DTROPICAL_WHATIF_NO_MMA issues the prefill MMAs with N = 16 (1/8 of the tensor work),
+// -DTROPICAL_WHATIF_NO_EXP replaces the softmax exponentials by one FMA, -DTROPICAL_WHATIF_NO_DECODE_MATH keeps 1/8 of
+// the decode ldmatrix + MMA work, -DTROPICAL_WHATIF_HALF_KV loads half of every full prefill K/V tile.
+#if defined(TROPICAL_WHATIF_NO_MMA) || defined(TROPICAL_WHATIF_NO_EXP) || defined(TROPICAL_WHATIF_NO_DECODE_MATH) || \
+    defined(TROPICAL_WHATIF_HALF_KV)
+#define TROPICAL_WHATIF_BUILD 1
+#endif
+
 constexpr int kPageSize = 16;  // BASELINE.json: page size 16 in every config
 
 struct PoolDesc {

@@ -202,6 +202,9 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
             for (int ks = 0; ks < D / 16; ++ks) {
                 const uint32_t addr = ((kbase + k_lane) ^ (uint32_t)((ks & 3) * 32)) + (ks >> 2) * C::HALF_BYTES;
                 uint32_t a0, a1, a2, a3;
+#ifdef TROPICAL_WHATIF_NO_DECODE_MATH
+                if (ks > 0) continue;
+#endif
                 ldmatrix_x4(addr, a0, a1, a2, a3);
                 if (ks & 1) mma_bf16_16816(sb, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
                 else mma_bf16_16816(sa, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
@@ -268,6 +271,9 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
             for (int db = 0; db < D / 16; ++db) {
                 const uint32_t addr = ((vbase + v_lane) ^ (uint32_t)((db & 3) * 32)) + (db >> 2) * C::HALF_BYTES;
                 uint32_t a0, a1, a2, a3;
+#ifdef TROPICAL_WHATIF_NO_DECODE_MATH
+                if (db > 0) continue;
+#endif
                 ldmatrix_x4_trans(addr, a0, a1, a2, a3);
                 mma_bf16_16816(o[db], a0, a1, a2, a3, pb0, pb1);
             }

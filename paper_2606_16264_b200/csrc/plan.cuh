@@ -12,6 +12,7 @@ constexpr int kKvTile = 128;         // keys per prefill KV iteration (8 pages)
 constexpr int kHeadBlock = 8;        // q heads of one kv group handled by one decode unit (MMA M rows used)
 constexpr int kTargetUnits = 9472;   // ~8 decode units per resident decode warp (148 SMs x 8 warps x 8)
 constexpr int kMinSplitPages = 8;    // never split finer than 128 tokens
+constexpr int kSmallBatchSplitPages = 32;  // ... nor finer than 512 tokens when a request has at least 1024 (see plan_kernel)
 
 enum { HDR_N_ITEMS = 0, HDR_N_UNITS = 1, HDR_SPLIT_PAGES = 2, HDR_TICKET_PREFILL = 3, HDR_TICKET_DECODE = 4,
        HDR_PROF = 16 /* 4 x u64: kernel start (min), prefill end, WG1 decode end, WG0 decode end (max) */,
@@ -91,6 +92,20 @@ __device__ __forceinline__ int plan_block_scan(int v, int* s_warp, int* total) {
     return base + incl - v;
 }
 
+// block-wide maximum of one non-negative int per thread
+__device__ __forceinline__ int plan_block_max(int v, int* s_warp) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, off));
+    __syncthreads();  // s_warp may still be read from a previous scan
+    if (lane == 0) s_warp[warp] = v;
+    __syncthreads();
+    int m = 0;
+#pragma unroll
+    for (int w = 0; w < kPlanThreads / 32; ++w) m = max(m, s_warp[w]);
+    return m;
+}
+
 __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split) {
     // the step kernel (a programmatic dependent of this one) may start its prologue now; it waits for this kernel's
     // completion before it reads the workspace
@@ -109,15 +124,29 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     const int chunk = (n + kPlanThreads - 1) / kPlanThreads;  // requests per thread (contiguous: prefix sums)
     const int i0 = tid * chunk, i1 = min(n, i0 + chunk);
 
-    int my_pages = 0;
+    int my_pages = 0, my_max = 0;
     for (int i = i0; i < i1; ++i)
-        if (__ldg(b.q_lens + i) == 1) my_pages += (__ldg(b.ctx_lens + i) + 1 + kPageSize - 1) / kPageSize;
+        if (__ldg(b.q_lens + i) == 1) {
+            const int pg = (__ldg(b.ctx_lens + i) + 1 + kPageSize - 1) / kPageSize;
+            my_pages += pg;
+            my_max = max(my_max, pg);
+        }
     int total_pages;
     plan_block_scan(my_pages, s_warp, &total_pages);
+    const int max_pages = plan_block_max(my_max, s_warp);  // pages of the longest decode request
     const long long page_heads = (long long)total_pages * Hkv * HB;
     int split = (int)((page_heads + kTargetUnits - 1) / kTargetUnits);
     if (split < kMinSplitPages) split = kMinSplitPages;
     split = (split + 7) / 8 * 8;  // whole 128-key blocks: only a request's last unit is ragged
+    // Small batches: a unit pays ~2.5 us of start-up (first TMA round trip, partial write, its share of the combine) and
+    // the combine of a split group is serial in its splits, so 8-page units (64 splits of an 8192-token request) cost
+    // 20-45 % of such a step.  Units of up to kSmallBatchSplitPages pages, but at least two per request, are within
+    // 1.5 % of the best forced split over the sweep in profiles/r2c_split_sweep.md; large batches keep the unit target.
+    {
+        int floor_split = max_pages / 2 / 8 * 8;
+        floor_split = min(kSmallBatchSplitPages, max(kMinSplitPages, floor_split));
+        if (split < floor_split) split = floor_split;
+    }
     // test hook: coarser splits only -- make_layout's max_units bound holds for split >= the automatic value
     if (forced_split > split) split = forced_split;
 

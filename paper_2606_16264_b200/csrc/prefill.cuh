@@ -128,12 +128,20 @@ __device__ __forceinline__ void prefill_load_tile(const PrefillArgs& A, PrefillB
     using C = PrefillCfg<D>;
     const int np = min(8, n_pages - kt * 8);
     const int p = lane / C::CB, cb = lane % C::CB;
+#ifdef TROPICAL_WHATIF_HALF_KV
+    const bool act = p < np && lane < 8 * C::CB && (np < 8 || p < 4);
+#else
     const bool act = p < np && lane < 8 * C::CB;
+#endif
     const int page = act ? __ldg(pt + kt * 8 + p) : 0;
     const int r0 = (page * A.pool.Hkv + it.hk) * kPageSize;
     const uint32_t off = cb * C::HALF_BYTES + p * C::PAGE_BOX;
     mbar_wait(&B->kv_empty[cur.slot], cur.phase ^ 1, 103);
+#ifdef TROPICAL_WHATIF_HALF_KV
+    if (lane == 0) mbar_arrive_expect_tx(&B->kv_full[cur.slot], (np < 8 ? np : 4) * C::CB * C::PAGE_BOX);
+#else
     if (lane == 0) mbar_arrive_expect_tx(&B->kv_full[cur.slot], np * C::CB * C::PAGE_BOX);
+#endif
     __syncwarp();
     if (act) tma_load_2d(ring + cur.slot * C::TILE_BYTES + off, tm, cb * 64, r0, &B->kv_full[cur.slot]);
 }
@@ -204,8 +212,13 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
     const uint32_t q_a = uni(smem_u32(tiles));
     const uint32_t ring_a = q_a + C::Q_TILES * C::TILE_BYTES;
     const uint32_t tm = uni(B->tmem_base);
+#ifdef TROPICAL_WHATIF_NO_MMA
+    constexpr uint32_t IDESC_S = make_idesc_bf16(128, 16, false);
+    constexpr uint32_t IDESC_O = make_idesc_bf16(128, 16, true);
+#else
     constexpr uint32_t IDESC_S = make_idesc_bf16(128, 128, false);
     constexpr uint32_t IDESC_O = make_idesc_bf16(128, D, true);
+#endif
     uint32_t item_it = 0;
     uint32_t g0 = 0, g1 = 0;      // S / P / PV iterations of query tile A, B so far (barrier phases)
     uint32_t cnt0 = 0, cnt1 = 0;  // items that carried tile A, B so far (o_empty phases)

@@ -40,18 +40,32 @@ struct Sim {
     std::vector<Worker> W;
     std::vector<int> toggle_q;
     std::vector<int32_t> q_buf, c_buf;
-    int np;  // dedicated prefill workers
+    std::vector<char> prefill_role;  // 1: dedicated prefill worker (policies 1, 2); may change under P:161
+    int delayed = 0;                 // prefills dispatched by the no-starvation rule since the last transition
+    int64_t to_multiplexing = 0, to_prefill = 0;
     double now = 0;
     int64_t iterations = 0;
     int status = TROPICAL_OK;
 
-    explicit Sim(const tropical_sim_config_t& c) : cfg(c), np(c.policy == TROPICAL_SIM_COLOCATED ? 0 : c.num_prefill_workers) {}
+    explicit Sim(const tropical_sim_config_t& c) : cfg(c), prefill_role(c.num_workers, 0) {
+        if (c.policy != TROPICAL_SIM_COLOCATED)
+            for (int w = 0; w < c.num_prefill_workers; ++w) prefill_role[w] = 1;
+    }
 
-    bool is_prefill_worker(int w) const { return cfg.policy != TROPICAL_SIM_COLOCATED && w < np; }
+    bool is_prefill_worker(int w) const { return prefill_role[w] != 0; }
+    int count_role(char role) const { return (int)std::count(prefill_role.begin(), prefill_role.end(), role); }
     int remaining_output(int r) const { return R[r].output - 1 - R[r].generated; }
 
     // duration of an iteration over the batch currently in q_buf / c_buf
     double iter_time() {
+        if (cfg.layer.d_model > 0) {  // NEXT-4: whole-iteration predictor (attention on the head shard + GEMMs + all-reduce)
+            double it = 0;
+            const int rc = tropical_iter_cost(&cfg.attn, &cfg.linear, &cfg.layer, cfg.num_q_heads, cfg.num_kv_heads,
+                                              cfg.head_dim, cfg.page_size, (int32_t)q_buf.size(), q_buf.data(),
+                                              c_buf.data(), &it, nullptr);
+            if (rc != TROPICAL_OK) status = rc;
+            return it + cfg.iter_overhead_us;
+        }
         double us = 0;
         const int rc = tropical_step_cost(&cfg.attn, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim, cfg.page_size,
                                           (int32_t)q_buf.size(), q_buf.data(), c_buf.data(), &us, nullptr);
@@ -96,20 +110,23 @@ struct Sim {
         return t;
     }
     int least_queue_prefill_worker() {
-        int best = 0;
+        int best = -1;
         double bq = kInf;
-        for (int w = 0; w < np; ++w) {
+        for (int w = 0; w < cfg.num_workers; ++w) {
+            if (!is_prefill_worker(w)) continue;
             const double q = pred_queue(w);
-            if (q < bq) { bq = q; best = w; }
+            if (best < 0 || q < bq) { bq = q; best = w; }
         }
         return best;
     }
-    int fewest_unfinished(int lo, int hi) const {
-        int best = lo;
-        long long bt = std::numeric_limits<long long>::max();
-        for (int w = lo; w < hi; ++w) {
+    // worker with the fewest unfinished tokens among all workers (role < 0) or those of one role
+    int fewest_unfinished(int role) const {
+        int best = -1;
+        long long bt = 0;
+        for (int w = 0; w < cfg.num_workers; ++w) {
+            if (role >= 0 && prefill_role[w] != role) continue;
             const long long t = unfinished_tokens(w);
-            if (t < bt) { bt = t; best = w; }
+            if (best < 0 || t < bt) { bt = t; best = w; }
         }
         return best;
     }
@@ -132,7 +149,7 @@ struct Sim {
                     R[r].finish = now;
                     R[r].decode_worker = w;
                 } else if (is_prefill_worker(w)) {  // P:155 decode queue, P:186 dispatch, P:58 migration
-                    const int best = fewest_unfinished(np, cfg.num_workers);
+                    const int best = fewest_unfinished(0);
                     W[best].pending.push_back({now + cfg.migrate_us_per_token * R[r].prompt, r});
                     R[r].decode_worker = best;
                 } else {
@@ -171,15 +188,39 @@ struct Sim {
         ++iterations;
     }
 
+    // P:161 role transitions [R]: readings in include/tropical_sim.h
+    void role_transitions() {
+        // prefill -> multiplexing: "when the watermark of all decode workers exceeds its threshold"
+        bool all_above = true;
+        for (int w = 0; w < cfg.num_workers; ++w)
+            if (!is_prefill_worker(w) && !((double)resident_kv(w) > cfg.hbm_watermark * (double)cfg.kv_capacity_tokens))
+                all_above = false;
+        if (all_above && count_role(1) >= 2) {
+            prefill_role[least_queue_prefill_worker()] = 0;
+            ++to_multiplexing;
+        }
+        // multiplexing -> prefill: "if prefill frequently encounters delays"
+        if (delayed >= cfg.delay_threshold && count_role(0) >= 2) {
+            for (int w = 0; w < cfg.num_workers; ++w) {
+                if (is_prefill_worker(w) || !W[w].resident.empty() || !W[w].pending.empty()) continue;
+                prefill_role[w] = 1;
+                ++to_prefill;
+                delayed = 0;
+                break;
+            }
+        }
+    }
+
     void toggle_scan() {
+        if (cfg.role_transitions) role_transitions();
         const std::vector<int> snapshot = toggle_q;
         for (int r : snapshot) {
             const double waited = now - R[r].arrival;
             int target = -1, mux = 0;
             // Path 2: multiplexing workers with an empty local queue, fewest unfinished tokens first
             std::vector<std::pair<long long, int>> cands;
-            for (int w = np; w < cfg.num_workers; ++w)
-                if (W[w].local_q.empty()) cands.push_back({unfinished_tokens(w), w});
+            for (int w = 0; w < cfg.num_workers; ++w)
+                if (!is_prefill_worker(w) && W[w].local_q.empty()) cands.push_back({unfinished_tokens(w), w});
             std::sort(cands.begin(), cands.end());
             for (const auto& cw : cands) {
                 const int w = cw.second;
@@ -217,7 +258,12 @@ struct Sim {
                 // the no-starvation rule fires on the very expression the wake-up below is scheduled with: testing
                 // `slack_ttft <= 0` instead can miss it by one rounding of (now - arrival)
                 const bool slack_gone = now >= R[r].arrival + cfg.ttft_slo_us;
-                if (slack_gone || pred_exec(r) + pred_queue(best) < slack_ttft) target = best;
+                if (slack_gone) {
+                    target = best;
+                    ++delayed;  // a delayed prefill
+                } else if (pred_exec(r) + pred_queue(best) < slack_ttft) {
+                    target = best;
+                }
             }
             if (target >= 0) {
                 toggle_q.erase(std::find(toggle_q.begin(), toggle_q.end(), r));
@@ -236,7 +282,7 @@ struct Sim {
             while (next_arrival < R.size() && R[next_arrival].arrival <= now) {
                 const int r = (int)next_arrival++;
                 if (cfg.policy == TROPICAL_SIM_COLOCATED) {
-                    const int w = fewest_unfinished(0, cfg.num_workers);
+                    const int w = fewest_unfinished(-1);
                     W[w].local_q.push_back(r);
                     R[r].prefill_worker = w;
                 } else if (cfg.policy == TROPICAL_SIM_DISAGGREGATED) {
@@ -277,6 +323,7 @@ extern "C" int tropical_sim_run(const tropical_sim_config_t* cfg, int32_t n, con
         return TROPICAL_ERR_INVALID_ARG;
     if (!(cfg->ttft_slo_us > 0) || !(cfg->tpot_slo_us > 0) || cfg->chunk_tokens < 0 || cfg->migrate_us_per_token < 0)
         return TROPICAL_ERR_INVALID_ARG;
+    if (cfg->role_transitions != 0 && (cfg->role_transitions != 1 || cfg->delay_threshold < 1)) return TROPICAL_ERR_INVALID_ARG;
     Sim S(*cfg);
     S.R.resize(n);
     for (int i = 0; i < n; ++i) {
@@ -327,6 +374,8 @@ extern "C" int tropical_sim_run(const tropical_sim_config_t* cfg, int32_t n, con
         }
         s.iterations = S.iterations;
         s.multiplexed_prefills = mux;
+        s.to_multiplexing = S.to_multiplexing;
+        s.to_prefill = S.to_prefill;
         *summary = s;
     }
     return TROPICAL_OK;

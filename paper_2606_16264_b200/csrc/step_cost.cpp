@@ -21,6 +21,11 @@ const BuiltinFit kBuiltin[] = {
 #include "cost_model_fit.inc"
 };
 
+// Coefficients of the linear layers (NEXT-4), fitted by `cost_fit fit` to calibration/b200_gemm.csv.
+const tropical_linear_model_t kBuiltinLinear =
+#include "linear_model_fit.inc"
+    ;
+
 void features(int Hq, int Hkv, int d, int P, int n, const int32_t* q, const int32_t* c,
               tropical_cost_breakdown_t* f) {
     double qc = 0, pages = 0, T = 0, csum = 0;
@@ -82,5 +87,47 @@ extern "C" int tropical_step_cost(const tropical_cost_model_t* model, int32_t Hq
         *out_us = model->t0_us + hi + model->kappa * lo + model->e_prefill_iter_us * (double)f.prefill_iters / nsm +
                   model->e_decode_unit_us * (double)f.decode_units / nsm;
     }
+    return TROPICAL_OK;
+}
+
+extern "C" int tropical_iter_cost(const tropical_cost_model_t* attn, const tropical_linear_model_t* linear,
+                                  const tropical_layer_shape_t* shape, int32_t Hq, int32_t Hkv, int32_t d, int32_t P,
+                                  int32_t num_reqs, const int32_t* q_lens, const int32_t* ctx_lens, double* out_us,
+                                  tropical_iter_breakdown_t* breakdown) {
+    if (shape == nullptr || (out_us == nullptr && breakdown == nullptr)) return TROPICAL_ERR_INVALID_ARG;
+    if (shape->d_model <= 0 || shape->d_ffn <= 0 || shape->num_layers < 1 || shape->tp < 1) return TROPICAL_ERR_INVALID_ARG;
+    if (Hq <= 0 || Hkv <= 0 || d <= 0 || Hq % Hkv != 0) return TROPICAL_ERR_INVALID_ARG;
+    const int tp = shape->tp;
+    if (Hkv % tp != 0 || shape->d_ffn % tp != 0) return TROPICAL_ERR_INVALID_ARG;
+    double attn_us = 0;
+    const int rc = tropical_step_cost(attn, Hq / tp, Hkv / tp, d, P, num_reqs, q_lens, ctx_lens, &attn_us, nullptr);
+    if (rc != TROPICAL_OK) return rc;
+    if (linear == nullptr) linear = &kBuiltinLinear;
+    double T = 0;
+    for (int i = 0; i < num_reqs; ++i) T += q_lens[i];
+    // (K, N) of the four weight matrices this GPU holds
+    const double mats[4][2] = {{(double)shape->d_model, (double)(Hq + 2 * Hkv) * d / tp},
+                               {(double)Hq * d / tp, (double)shape->d_model},
+                               {(double)shape->d_model, (shape->gated_mlp ? 2.0 : 1.0) * shape->d_ffn / tp},
+                               {(double)shape->d_ffn / tp, (double)shape->d_model}};
+    double W = 0, act = 0;
+    for (const auto& m : mats) {
+        W += m[0] * m[1];
+        act += m[0] + m[1];
+    }
+    tropical_iter_breakdown_t b;
+    b.attn_us = attn_us;
+    b.gemm_flops = 2.0 * T * W;
+    b.gemm_bytes = 2.0 * W + 2.0 * T * act;
+    b.linear_us = 0;
+    b.allreduce_us = 0;
+    if (T > 0) {
+        const double tf = linear->f_us_per_flop * b.gemm_flops, tw = linear->w_us_per_byte * b.gemm_bytes;
+        b.linear_us = linear->g0_us + (tf > tw ? tf : tw) + linear->kappa * (tf > tw ? tw : tf);
+        if (tp > 1) b.allreduce_us = 2.0 * (linear->ar0_us + linear->ar_us_per_byte * 2.0 * T * shape->d_model);
+    }
+    b.total_us = shape->num_layers * (b.attn_us + b.linear_us + b.allreduce_us);
+    if (breakdown != nullptr) *breakdown = b;
+    if (out_us != nullptr) *out_us = b.total_us;
     return TROPICAL_OK;
 }

@@ -120,30 +120,70 @@ def test_step_cost_properties_with_explicit_model():
     empty, _ = tb.step_cost(8, 8, 128, 16, [], [], model=m)
     assert empty == 5.0
     us, bd = tb.step_cost(8, 8, 128, 16, [512, 1, 1], [0, 700, 90], model=m)
-    assert us >= max(bd.t_tc_us, bd.t_hbm_us)
+    assert us >= 5.0 + max(bd.t_tc_us, bd.t_hbm_us) and bd.t_tc_us == 1e-9 * bd.flops and bd.t_hbm_us == 2e-7 * bd.bytes
     with pytest.raises(tb.TropicalError):
         tb.step_cost(6, 4, 128, 16, [1], [1], model=m)
 
 
+NOMINAL_TFLOPS, NOMINAL_HBM_GBS = 2250.0, 8000.0   # dense bf16 and HBM3e peaks of the part: constants, not fitted
+
+
 def test_builtin_cost_model_reproduces_measured_grid():
     """A6: the compiled-in coefficients (csrc/cost_model_fit.inc) against the B200 measurements they were fitted to
-    (paper_2606_16264_b200/calibration/b200_grid.csv).  Held-out rows (seed % 5 == 0) were not used by the fit.
-    The paper gives no accuracy target; the bars are this build's."""
+    (paper_2606_16264_b200/calibration/b200_grid.csv).  Held-out rows (every fifth grid point, and every off-grid point:
+    recipe values between and beyond the grid lines) were not used by the fit.  The paper gives no accuracy target
+    (P:157); the bars are SURVEY.md 8(c)'s: held-out MAPE <= 10 %, every point within 25 % -- except steps shorter than
+    60 us, where the overlap of consecutive launches moves the measurement itself by ~10 % (bar 30 % there; DESIGN.md
+    section 7).  Every prediction must also respect the roofline of the part's NOMINAL peaks, which the fit cannot move."""
     import numpy as np
     from paper_2606_16264_b200 import cost_fit
     rows = cost_fit.read_grid(cost_fit.DEFAULT_GRID)
-    assert len(rows) >= 200
-    for shape in sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows}):
-        rel_all, rel_held = [], []
+    assert len(rows) >= 400
+    shapes = sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows})
+    assert (20, 20, 128) in shapes and (32, 4, 128) in shapes      # the TP = 2 head shards of C4 / C5 (NEXT-4)
+    for shape in shapes:
+        rel_all, rel_held, rel_off, rel_short = [], [], [], []
         for r in rows:
             if (r["Hq"], r["Hkv"], r["d"]) != shape:
                 continue
             q, c = cost_fit.grid_lengths(r["prefill_tokens"], r["prefill_ctx"], r["n_decode"], r["ctx_median"], r["seed"])
             us, bd = tb.step_cost(*shape, 16, q.tolist(), c.tolist())
-            assert us >= max(bd.t_tc_us, bd.t_hbm_us)
+            assert us >= max(bd.flops / (NOMINAL_TFLOPS * 1e6), bd.bytes / (NOMINAL_HBM_GBS * 1e3))
             rel = abs(us - r["us_median"]) / r["us_median"]
-            rel_all.append(rel)
+            (rel_all if r["us_median"] >= 60.0 else rel_short).append(rel)
             if cost_fit.is_held_out(r):
                 rel_held.append(rel)
-        assert np.mean(rel_held) <= 0.15, (shape, np.mean(rel_held))
-        assert np.max(rel_all) <= 0.40, (shape, np.max(rel_all))
+            if r["seed"] >= 1000:
+                rel_off.append(rel)
+        assert len(rel_off) >= 20
+        assert np.mean(rel_held) <= 0.10, (shape, np.mean(rel_held))
+        assert np.mean(rel_off) <= 0.10, (shape, np.mean(rel_off))
+        assert np.max(rel_all) <= 0.25, (shape, np.max(rel_all))
+        assert np.max(rel_short) <= 0.30, (shape, np.max(rel_short))
+
+
+def test_builtin_linear_model_reproduces_measured_gemms():
+    """NEXT-4: the compiled-in linear-layer coefficients (csrc/linear_model_fit.inc) against the library-GEMM times of
+    calibration/b200_gemm.csv (7B-, 13B- and 70B-layer-like shapes, TP 1 and 2, 1 .. 8192 tokens), through
+    tropical_iter_cost with the attention term switched off."""
+    import numpy as np
+    from paper_2606_16264_b200 import cost_fit
+    rows = cost_fit.read_gemm(cost_fit.GEMM_GRID)
+    assert len(rows) >= 50
+    zero = tb.CostModel(0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 148.0)
+    rel = []
+    for r in rows:
+        shape = tb.LayerShape(r["d_model"], r["d_ffn"], r["gated"], 1, r["tp"])
+        T = r["tokens"]
+        us, bd = tb.iter_cost(shape, r["Hq"], r["Hkv"], r["d"], 16, [T] if T > 1 else [1], [0], attn=zero)
+        assert bd.attn_us == 0.0 and bd.allreduce_us == 0.0 and us == bd.linear_us
+        assert us >= max(bd.gemm_flops / (NOMINAL_TFLOPS * 1e6), bd.gemm_bytes / (NOMINAL_HBM_GBS * 1e3))
+        rel.append(abs(us - r["us_median"]) / r["us_median"])
+    assert np.mean(rel) <= 0.08 and np.max(rel) <= 0.20, (np.mean(rel), np.max(rel))
+    # a whole iteration of the 13B-like model with the built-in fits: 40 layers, TP = 2 shard of C4's batch
+    import synth
+    _, Hq, Hkv, d, P, q, c, _ = synth.config_lengths("C4")
+    us1, bd1 = tb.iter_cost(tb.LayerShape(5120, 13824, 1, 40, 1), Hq, Hkv, d, P, q.tolist(), c.tolist())
+    us2, bd2 = tb.iter_cost(tb.LayerShape(5120, 13824, 1, 40, 2), Hq, Hkv, d, P, q.tolist(), c.tolist())
+    assert bd2.attn_us < bd1.attn_us and bd2.linear_us < bd1.linear_us and us2 < us1
+    assert us1 == pytest.approx(40 * (bd1.attn_us + bd1.linear_us))

@@ -28,11 +28,15 @@ def _ocfg(policy, cm=FLAT, **kw):
 
 def _ccfg(o: so.Config):
     a = o.attn
+    sh, lm = o.layer, o.linear
     return tb.SimConfig(o.policy, o.num_workers, o.num_prefill_workers, o.chunk_tokens, o.ttft_slo_us, o.tpot_slo_us,
                         o.decode_guard, o.hbm_watermark, o.kv_capacity_tokens, o.migrate_us_per_token, o.num_q_heads,
                         o.num_kv_heads, o.head_dim, o.page_size, o.num_layers,
                         tb.CostModel(a.t0_us, a.a_us_per_flop, a.b_us_per_byte, a.kappa, a.e_prefill_iter_us,
-                                     a.e_decode_unit_us, a.n_sm), o.linear_us_per_token, o.iter_overhead_us)
+                                     a.e_decode_unit_us, a.n_sm), o.linear_us_per_token, o.iter_overhead_us,
+                        tb.LayerShape(sh.d_model, sh.d_ffn, sh.gated_mlp, sh.num_layers, sh.tp),
+                        tb.LinearModel(lm.g0_us, lm.f_us_per_flop, lm.w_us_per_byte, lm.kappa, lm.ar0_us, lm.ar_us_per_byte),
+                        o.role_transitions, o.delay_threshold)
 
 
 # ------------------------------------------------------------------------------------------ part 1: oracle pins
@@ -208,6 +212,96 @@ def test_no_starvation_wake_up_fires_despite_rounding():
     assert osum["attainment"] == 0.0 and csum.attainment == 0.0      # TTFT = slo + 110 > slo
 
 
+def test_iteration_cost_worked_by_hand():
+    """NEXT-4 (include/tropical.h tropical_iter_cost): golden batch A (q = [130, 1], c = [0, 17]) of a 4/2/64 model with
+    TP = 2, so one GPU runs the head shard 2/1/64.  Step features of the shard, by hand from the formulas of
+    tests/golden/step_cost_features.txt: F = 8737792 / 2 = 4368896; B = 4*1*64*17 + 2*(4*1*64*131) + 2*(2*2*64*131)
+    + 4*11 = 4352 + 67072 + 67072 + 44 = 138540; N_p = 3 iterations x 2 heads = 6; N_d = 2 pages x 1 head = 2.
+      step = 5 + 4.368896 + 0.5 * 1.3854 + 2 * 6 / 4 + 3 * 2 / 4 = 14.561596
+    Linear layers of d_model 8, d_ffn 16 (gated), per GPU: QKV 8 x 256, O 128 x 8, gate+up 8 x 16, down 8 x 8:
+      W = 2048 + 1024 + 128 + 64 = 3264; T = 131; F = 2 * 131 * 3264 = 855168;
+      B = 2 * 3264 + 2 * 131 * (264 + 136 + 24 + 16) = 6528 + 115280 = 121808
+      linear (g0 7, f 1e-5, w 1e-4, kappa 0.25) = 7 + 12.1808 + 0.25 * 8.55168 = 21.31872
+      all-reduce (1.5 us + 1e-3 us/B, two per layer over 2 * 131 * 8 B) = 2 * (1.5 + 2.096) = 7.192
+      iteration of 3 layers = 3 * (14.561596 + 21.31872 + 7.192) = 129.216948"""
+    cm = (5.0, 1e-6, 1e-5, 0.5, 2.0, 3.0, 4.0)
+    lin = (7.0, 1e-5, 1e-4, 0.25, 1.5, 1e-3)
+    cfg = _ocfg(so.COLOCATED, cm=cm, num_q_heads=4, num_kv_heads=2, head_dim=64, iter_overhead_us=2.0,
+                layer=so.LayerShape(8, 16, 1, 3, 2), linear=so.LinearModel(*lin))
+    assert so.iter_cost_us(cfg, [130, 1], [0, 17]) == pytest.approx(129.216948, rel=1e-12)
+    assert so.iter_time_us(cfg, [130, 1], [0, 17]) == pytest.approx(131.216948, rel=1e-12)
+    got, bd = tb.iter_cost(tb.LayerShape(8, 16, 1, 3, 2), 4, 2, 64, 16, [130, 1], [0, 17], attn=tb.CostModel(*cm),
+                           linear=tb.LinearModel(*lin))
+    assert got == pytest.approx(129.216948, rel=1e-12)
+    assert (bd.gemm_flops, bd.gemm_bytes) == (855168.0, 121808.0)
+    assert bd.attn_us == pytest.approx(14.561596) and bd.linear_us == pytest.approx(21.31872)
+    assert bd.allreduce_us == pytest.approx(7.192)
+    # tp = 1: no all-reduce, whole heads: step = 24.122972 (test above); W doubles except ... by hand:
+    # QKV 8 x 512, O 256 x 8, gate+up 8 x 32, down 16 x 8: W = 4096 + 2048 + 256 + 128 = 6528, F = 1710336,
+    # B = 13056 + 262 * (520 + 264 + 40 + 24) = 13056 + 222176 = 235232 -> 7 + 23.5232 + 0.25 * 17.10336 = 34.79904
+    got1, bd1 = tb.iter_cost(tb.LayerShape(8, 16, 1, 1, 1), 4, 2, 64, 16, [130, 1], [0, 17], attn=tb.CostModel(*cm),
+                             linear=tb.LinearModel(*lin))
+    assert bd1.allreduce_us == 0.0 and got1 == pytest.approx(24.122972 + 34.79904, rel=1e-12)
+    cfg1 = _ocfg(so.COLOCATED, cm=cm, num_q_heads=4, num_kv_heads=2, head_dim=64,
+                 layer=so.LayerShape(8, 16, 1, 1, 1), linear=so.LinearModel(*lin))
+    assert so.iter_cost_us(cfg1, [130, 1], [0, 17]) == pytest.approx(24.122972 + 34.79904, rel=1e-12)
+    with pytest.raises(tb.TropicalError):   # tp must divide the kv heads
+        tb.iter_cost(tb.LayerShape(8, 16, 1, 1, 4), 4, 2, 64, 16, [1], [1], attn=tb.CostModel(*cm))
+
+
+def test_prefill_worker_becomes_multiplexing_worker_when_every_decode_worker_is_above_the_watermark():
+    """P:161, first sentence, by hand.  Workers 0, 1 prefill, worker 2 multiplexing; flat cost with 1 us per token and no
+    overhead; KV capacity 100 tokens, watermark 0.5 (threshold 50 tokens); no migration time.
+      t=0    A (prompt 60, 100 outputs): Path 2 refused (0 + 60 > 50), Path 1 -> worker 0 (exec 60 < SLO), runs 0..60.
+      t=60   A's first token; its cache goes to worker 2 (the only multiplexing worker): worker 2 now holds 60 > 50 tokens
+             = every multiplexing worker is above the watermark, two prefill workers exist -> the one with the least
+             predicted queue (both 0: worker 0) becomes a multiplexing worker.  A decodes on worker 2, 1 us per token.
+      t=100  B (prompt 10, 2 outputs): Path 2 candidates {0, 2} by unfinished tokens: worker 0 (0) first: empty, 0 + 10 <=
+             50 -> multiplexed on worker 0: prefill 100..110 (TTFT 10), one decode iteration 110..111, stays on worker 0.
+    With fixed roles B is refused by worker 2 (100 + 10 > 50) and takes Path 1: worker 0, then migrates to worker 2."""
+    kw = dict(num_workers=3, num_prefill_workers=2, kv_capacity_tokens=100, hbm_watermark=0.5, linear_us_per_token=1.0,
+              iter_overhead_us=0.0, tpot_slo_us=1e9)
+    reqs = [(0.0, 60, 100), (100.0, 10, 2)]
+    for sim in (lambda c: so.simulate(c, reqs), lambda c: _as_dicts(tb.sim_run(_ccfg(c), reqs))):
+        res, summ = sim(_ocfg(so.MULTIPLEXED, role_transitions=1, delay_threshold=1000, **kw))
+        assert (res[0]["prefill_worker"], res[0]["decode_worker"], res[0]["first_token_us"]) == (0, 2, 60.0)
+        assert (res[1]["prefill_worker"], res[1]["decode_worker"], res[1]["multiplexed"]) == (0, 0, 1)
+        assert res[1]["ttft_us"] == pytest.approx(10.0) and res[1]["finish_us"] == pytest.approx(111.0)
+        assert (summ["to_multiplexing"], summ["to_prefill"]) == (1, 0)
+        res, summ = sim(_ocfg(so.MULTIPLEXED, **kw))       # fixed roles
+        assert (res[1]["prefill_worker"], res[1]["decode_worker"], res[1]["multiplexed"]) == (0, 2, 0)
+        assert (summ["to_multiplexing"], summ["to_prefill"]) == (0, 0)
+
+
+def test_multiplexing_worker_becomes_prefill_worker_when_prefills_keep_being_delayed():
+    """P:161, second sentence, by hand.  Worker 0 prefill, workers 1, 2 multiplexing; flat cost, 1 us per token, no
+    overhead; TTFT SLO 5 us; capacity 100, watermark 0.5, so 80-token prompts are refused by Path 2 (80 > 50) and by
+    Path 1 (80 us > any slack): every request waits for the no-starvation rule at arrival + 5.  delay_threshold = 2.
+      t=5  A (arrival 0) delayed -> worker 0, runs 5..85.        delayed = 1
+      t=6  B (arrival 1) delayed -> worker 0's queue.             delayed = 2
+      t=7  scan: 2 delayed prefills, two multiplexing workers, worker 1 holds no decode state -> worker 1 becomes a
+           prefill worker.  C (arrival 2) delayed -> least predicted queue: worker 0 = (85 - 7) + 80, worker 1 = 0 ->
+           worker 1, runs 7..87 (TTFT 85).  B runs 85..165 on worker 0.
+    With fixed roles C queues behind B on worker 0: 165..245 (TTFT 243)."""
+    kw = dict(num_workers=3, num_prefill_workers=1, kv_capacity_tokens=100, hbm_watermark=0.5, linear_us_per_token=1.0,
+              iter_overhead_us=0.0, ttft_slo_us=5.0)
+    reqs = [(0.0, 80, 1), (1.0, 80, 1), (2.0, 80, 1)]
+    for sim in (lambda c: so.simulate(c, reqs), lambda c: _as_dicts(tb.sim_run(_ccfg(c), reqs))):
+        res, summ = sim(_ocfg(so.MULTIPLEXED, role_transitions=1, delay_threshold=2, **kw))
+        assert [r["prefill_worker"] for r in res] == [0, 0, 1]
+        assert [r["first_token_us"] for r in res] == pytest.approx([85.0, 165.0, 87.0])
+        assert (summ["to_multiplexing"], summ["to_prefill"]) == (0, 1)
+        res, summ = sim(_ocfg(so.MULTIPLEXED, **kw))
+        assert [r["prefill_worker"] for r in res] == [0, 0, 0] and res[2]["first_token_us"] == pytest.approx(245.0)
+
+
+def _as_dicts(out):
+    res, summ = out
+    fields = ("ttft_us", "tpot_us", "first_token_us", "finish_us", "prefill_worker", "decode_worker", "multiplexed")
+    return ([{f: getattr(r, f) for f in fields} for r in res],
+            {f: getattr(summ, f) for f, _ in tb.binding.SimSummary._fields_})
+
+
 def _trace(seed, n, mean_gap_us):
     rng = random.Random(seed)
     t, out = 0.0, []
@@ -250,6 +344,26 @@ def test_cpp_simulator_matches_oracle(policy, seed, gap, chunk):
     assert csum.iterations == osum["iterations"] and csum.multiplexed_prefills == osum["multiplexed_prefills"]
     for f in ("attainment", "ttft_mean_us", "ttft_p90_us", "tpot_mean_us", "tpot_p90_us", "makespan_us"):
         assert getattr(csum, f) == pytest.approx(osum[f], rel=1e-9)
+
+
+@pytest.mark.parametrize("seed,gap,thr", [(4, 9000.0, 2), (5, 3000.0, 1), (6, 20000.0, 1)])
+def test_cpp_simulator_matches_oracle_with_role_transitions_and_the_iteration_predictor(seed, gap, thr):
+    """P:161 transitions + NEXT-4 iteration times (TP = 2 shard of a 64/8/128 model) on seeded long-tail traces: small
+    KV capacity so that the watermark rule fires, a tight TTFT SLO so that prefills get delayed."""
+    o = _ocfg(so.MULTIPLEXED, cm=FIT, num_workers=6, num_prefill_workers=3, chunk_tokens=1024, ttft_slo_us=5e3,
+              tpot_slo_us=2.5e4, kv_capacity_tokens=6000, hbm_watermark=0.6, migrate_us_per_token=0.04, iter_overhead_us=25.0,
+              layer=so.LayerShape(1024, 4096, 1, 4, 2), linear=so.LinearModel(20.0, 7e-10, 1.6e-7, 0.3, 8.0, 2e-6),
+              role_transitions=1, delay_threshold=thr)
+    reqs = _trace(200 + seed, 90, gap)
+    ores, osum = so.simulate(o, reqs)
+    cres, csum = _as_dicts(tb.sim_run(_ccfg(o), reqs))
+    for a, b in zip(cres, ores):
+        assert (a["prefill_worker"], a["decode_worker"], a["multiplexed"]) == (b["prefill_worker"], b["decode_worker"], b["multiplexed"])
+        for f in ("ttft_us", "tpot_us", "first_token_us", "finish_us"):
+            assert a[f] == pytest.approx(b[f], rel=1e-9, abs=1e-9)
+    assert (csum["to_multiplexing"], csum["to_prefill"]) == (osum["to_multiplexing"], osum["to_prefill"])
+    assert osum["to_multiplexing"] + osum["to_prefill"] > 0      # the traces do exercise the transitions
+    assert csum["iterations"] == osum["iterations"]
 
 
 def test_cpp_simulator_on_the_worked_examples():
