@@ -205,11 +205,14 @@ def describe(name):
 class StepTimer:
     """The step of one config on the current device: append + attention through the C-ABI binding."""
 
-    def __init__(self, s, tb, torch):
+    def __init__(self, s, tb, torch, two_call=False, dev=None):
         from paper_2606_16264_b200.harness import DeviceStep
         self.s, self.tb, self.torch = s, tb, torch
+        # False (default): the step is ONE call, tropical_mixed_step (KV append fused into the step kernel);
+        # True: tropical_kv_append followed by tropical_mixed_attention (three launches, the r1 / r2a chain)
+        self.two_call = two_call
         self.cnt = step_counts((s.num_q_heads, s.num_kv_heads, s.head_dim, s.page_size, s.q_lens, s.ctx_lens))
-        self.dev = DeviceStep(s)
+        self.dev = dev if dev is not None else DeviceStep(s)
         self.stream = torch.cuda.current_stream()
         # A step whose working set fits the 126 MB L2 is timed cold: a 512 MB buffer is rewritten between timed steps
         # (untimed) and the per-step event times are summed.  The big configs (> 0.5 GB per step) need no flush.
@@ -221,11 +224,16 @@ class StepTimer:
         tb, dev = self.tb, self.dev
         if ev is not None:
             ev[0].record(self.stream)
-        tb.kv_append(dev.pool, dev.batch, dev.k_new, dev.v_new)
-        n = tb.last_launch_count()
+        n = 0
+        if self.two_call:
+            tb.kv_append(dev.pool, dev.batch, dev.k_new, dev.v_new)
+            n = tb.last_launch_count()
         if ev is not None:
             ev[1].record(self.stream)
-        tb.mixed_attention(dev.pool, dev.batch, dev.q, out=dev.out, workspace=dev.workspace)
+        if self.two_call:
+            tb.mixed_attention(dev.pool, dev.batch, dev.q, out=dev.out, workspace=dev.workspace)
+        else:
+            tb.mixed_step(dev.pool, dev.batch, dev.q, dev.k_new, dev.v_new, out=dev.out, workspace=dev.workspace)
         n += tb.last_launch_count()
         if ev is not None:
             ev[2].record(self.stream)
@@ -433,7 +441,7 @@ def run_ours(args, rank, world):
     if args.config == "MIG":
         return run_migration(args, rank, world, local, tb, torch, dist, peaks)
     s, gen_s = make_workload(args.config, rank, args.part)
-    st = StepTimer(s, tb, torch)
+    st = StepTimer(s, tb, torch, two_call=args.two_call)
     cnt = st.cnt
     warm = max(args.warmup, 3)
     st.warm(warm)
@@ -465,7 +473,9 @@ def run_ours(args, rank, world):
         return
     t_bytes_us, t_flops_us, t_roof, t_nom = roofline_times(cnt, peaks)
     attn_med = float(np.median(attn_us))
-    achieved = cnt["attn_bytes"] / (attn_med * 1e3)  # GB/s
+    # algorithmic bytes of the dominant launch: the whole step's when the append runs inside the step kernel
+    kernel_bytes = cnt["attn_bytes"] if args.two_call else cnt["step_bytes"]
+    achieved = kernel_bytes / (attn_med * 1e3)  # GB/s
     if args.no_cpu:
         cpu_us, cpu_desc, cores = float("nan"), "skipped (--no-cpu)", 0
     else:
@@ -478,7 +488,12 @@ def run_ours(args, rank, world):
                                ("" if args.part == "all" else f", its {args.part} requests only (analysis run)"), "replicas": world,
                    "l2": "step touches %.2f GB >> 126 MB L2, no flush needed" % (cnt["step_bytes"] / 1e9)
                    if not st.flush else "L2 flushed (512 MB rewritten, untimed) between timed steps; per-step event times summed",
-                   "new_tokens_per_step": int(cnt["new_tokens"])},
+                   "new_tokens_per_step": int(cnt["new_tokens"]),
+                   "step": ("tropical_kv_append + tropical_mixed_attention (3 launches)" if args.two_call else
+                            "tropical_mixed_step: one call; " +
+                            ("its fused kernel variant, KV append inside the step kernel (2 launches)"
+                             if st.launches_per_step == 2 else
+                             "decode-heavy step: its append kernel in front of the plain step kernel (3 launches)"))},
         "tokens_per_s": round(whole_job_tokens_per_s(cnt["new_tokens"], world, us), 1),
         "us_per_step": {"mean_timed_region": round(us, 2), "median": round(float(np.median(step_us)), 2),
                         "min": round(float(step_us.min()), 2), "max": round(float(step_us.max()), 2),
@@ -490,12 +505,17 @@ def run_ours(args, rank, world):
                           "achieved_tflops": round(cnt["flops"] / (us * 1e6), 1),
                           "peaks": peaks, "nominal": NOMINAL},
         "roofline": {"bound": "hbm",
-                     "kernel": "launches of tropical_mixed_attention: tile directory + persistent step kernel (>= 95 % of it)",
+                     "kernel": ("the attention launches: tile directory + persistent step kernel (>= 95 % of it)"
+                                if args.two_call else
+                                "launches of tropical_mixed_step: append kernel, tile directory, persistent step kernel (>= 95 % of it)"
+                                if st.launches_per_step == 3 else
+                                "launches of tropical_mixed_step: tile directory + persistent step kernel with the KV append "
+                                "inside (>= 98 % of it)"),
                      "achieved": round(achieved, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
                      "frac": round(achieved / peaks["hbm_gbs"], 4), "traffic": ncu_traffic(args.config),
                      "kernel_us": round(attn_med, 2), "kernel_us_min": round(float(attn_us.min()), 2),
                      "kernel_share_of_step": round(float(np.median(attn_us / step_us)), 4),
-                     "algorithmic_bytes": cnt["attn_bytes"], "of": peaks["source"],
+                     "algorithmic_bytes": kernel_bytes, "of": peaks["source"],
                      "timing": f"median of {n_k} event pairs around the attention call, second pass"},
         "cpu_baseline": {"value": round(cpu_us, 1), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc},
         "e2e": {"value": round(e2e_us, 2), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
@@ -532,6 +552,14 @@ def run_extras(args, tb, torch, peaks, local, st_c5):
                         "clocks": rep["clocks"]}
     except Exception as exc:  # an extra must never cost the headline line
         extra["MIG"] = {"error": repr(exc)}
+    try:  # the same C5 step as two calls (append kernel + attention): what fusing the append is worth, same box
+        st2 = StepTimer(st_c5.s, tb, torch, two_call=True, dev=st_c5.dev)   # same resident pools and inputs
+        st2.warm(3)
+        us2 = st2.timed(steps) * 1e3 / steps
+        extra["C5_two_call"] = {"workload": "C5 as tropical_kv_append + tropical_mixed_attention (3 launches)",
+                                "value": round(us2, 2), "unit": UNIT, "steps": steps}
+    except Exception as exc:
+        extra["C5_two_call"] = {"error": repr(exc)}
     try:
         s4, _ = make_workload("C4", 0)
         st = StepTimer(s4, tb, torch)
@@ -637,6 +665,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--part", default="all", choices=["all", "prefill", "decode"],
                     help="analysis runs: only the prefill (q > 1) or only the decode (q = 1) requests of the config")
+    ap.add_argument("--two-call", action="store_true",
+                    help="time the step as tropical_kv_append + tropical_mixed_attention instead of the fused tropical_mixed_step")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-extra", action="store_true", help="skip extra.C4 / extra.MIG on the default run")
     ap.add_argument("--sustain-seconds", type=float, default=2.0, help="length of the sustained loop (0 = skip)")

@@ -145,6 +145,18 @@ int tropical_mixed_attention(const tropical_kv_pool_t *pool, const tropical_batc
                              const void *q, void *out, float *lse, float sm_scale,
                              void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* One multiplexed iteration in ONE call -- rows A0-A5 with the KV append (A1) fused in: the same results as
+ * tropical_kv_append followed by tropical_mixed_attention (pool bit-identical afterwards, out / lse identical to that
+ * pair's), in two launches instead of three and with the append off the critical path.  The attention roles read this
+ * step's K / V rows directly from k_new / v_new (TMA boxes over [T][Hkv][d]; a decode request's own new row is patched
+ * into the page-head it has just loaded) while otherwise idle warps of the same persistent kernel copy the rows into
+ * their (page, slot) of the pool; nothing reads those slots from the pool during the step.
+ *   k_new, v_new [device] bf16 [T][Hkv][d], 16-byte aligned; every other argument as in tropical_mixed_attention.
+ * The pool IS written (exactly the rows tropical_kv_append would write).  Idempotent, graph-capturable. */
+int tropical_mixed_step(const tropical_kv_pool_t *pool, const tropical_batch_t *batch, const void *q,
+                        const void *k_new, const void *v_new, void *out, float *lse, float sm_scale,
+                        void *workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* Opt-in debug check of the DEVICE-resident contents of a batch, which the other calls cannot validate without a
  * sync (out-of-range page ids there are undefined behaviour): q_lens / ctx_lens >= 0, q_offsets the exclusive prefix
  * sum of q_lens with q_offsets[num_reqs] == total_q, ctx + q <= max_kv_len, ceil((ctx + q) / page_size) <=
@@ -158,7 +170,7 @@ int tropical_validate_batch(const tropical_kv_pool_t *pool, const tropical_batch
 
 /* End-to-end step from HOST buffers (what bench.py's "e2e" times): copies this step's inputs
  * host->device into caller-provided device staging, runs append + attention, copies out back,
- * and synchronises the stream before returning.  The KV pool stays device resident (it is the
+ * (the fused tropical_mixed_step), and synchronises the stream before returning.  The KV pool stays device resident (it is the
  * worker's cache).  Host buffers should be pinned for the copies to be async.
  *   staging [device] >= tropical_step_host_staging_bytes(...), 256-byte aligned.
  *   h_*: [host] same shapes as the device-pointer API.  h_lse nullable. */

@@ -29,6 +29,11 @@ void tropical_debug_set_grid(int num_ctas);
  * tropical_workspace_bytes assumes split >= automatic): a smaller value is ignored. */
 void tropical_debug_set_split_pages(int pages);
 
+/* tropical_mixed_step chooses between its fused kernel variant (append inside the step kernel) and the append kernel in
+ * front of the plain variant from the batch scalars (prefill-dominated steps fuse).  mode 1 / 0 forces the fused variant
+ * on / off for every step, so that tests put every batch shape through both; -1 restores the choice. */
+void tropical_debug_set_fused(int mode);
+
 /* Only in special builds (else TROPICAL_ERR_UNSUPPORTED).  Synchronises the device.
  *  -DTROPICAL_WAIT_PROF: cycles spent in and calls of every mbarrier wait of the step kernel, summed over warps,
  *    indexed by the wait's tag (the numbers next to the mbar_wait calls in csrc/); reset != 0 zeroes the counters.

@@ -94,10 +94,10 @@ class SimSummary(ctypes.Structure):
 SIM_COLOCATED, SIM_DISAGGREGATED, SIM_MULTIPLEXED = 0, 1, 2
 
 EXPORTS = (
-    "tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention",
+    "tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention", "tropical_mixed_step",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost", "tropical_iter_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
-    "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_wait_profile", "tropical_debug_read_profile", "tropical_debug_timeline",
+    "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_set_fused", "tropical_debug_wait_profile", "tropical_debug_read_profile", "tropical_debug_timeline",
     "tropical_sim_run",
 )
 
@@ -122,7 +122,7 @@ def lib():
     L.tropical_status_string.restype = ctypes.c_char_p
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
-    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_step_host",
+    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_mixed_step", "tropical_step_host",
                  "tropical_step_cost", "tropical_iter_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
                  "tropical_debug_read_profile"):
         getattr(L, name).restype = ctypes.c_int
@@ -141,6 +141,11 @@ def version() -> str:
 def debug_set_grid(num_ctas: int) -> None:
     """Test hook: cap the CTAs of the persistent step kernel (0 = one per SM)."""
     lib().tropical_debug_set_grid(ctypes.c_int(int(num_ctas)))
+
+
+def debug_set_fused(mode: int) -> None:
+    """Test hook: tropical_mixed_step's kernel variant: 1 = always the fused one, 0 = never, -1 = its own choice."""
+    lib().tropical_debug_set_fused(ctypes.c_int(int(mode)))
 
 
 def debug_set_split_pages(pages: int) -> None:
@@ -349,6 +354,28 @@ def mixed_attention(pool: KVPool, batch: Batch, q: torch.Tensor, out: Optional[t
     _check(lib().tropical_mixed_attention(ctypes.byref(p), ctypes.byref(b), _ptr(q), _ptr(out), _ptr(lse),
                                           ctypes.c_float(sm_scale), _ptr(ws), ctypes.c_size_t(ws.numel()),
                                           _stream(stream)), "tropical_mixed_attention")
+    return out
+
+
+def mixed_step(pool: KVPool, batch: Batch, q: torch.Tensor, k_new: torch.Tensor, v_new: torch.Tensor,
+               out: Optional[torch.Tensor] = None, lse: Optional[torch.Tensor] = None, sm_scale: float = 0.0,
+               workspace: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """One multiplexed iteration in one call: KV append fused into the attention step (tropical_mixed_step)."""
+    _dev2(q, "q")
+    _dev2(k_new, "k_new")
+    _dev2(v_new, "v_new")
+    if out is None:
+        out = torch.empty_like(q)
+    _dev2(out, "out")
+    p, b = pool.c(), batch.c()
+    if workspace is None:
+        workspace = _alloc_ws(workspace_bytes(pool, b.num_reqs, b.total_q, b.max_kv_len), q.device)
+    ws = _aligned(workspace)
+    if lse is not None and not (lse.is_cuda and lse.dtype == torch.float32 and lse.is_contiguous()):
+        raise ValueError("lse must be a contiguous float32 CUDA tensor")
+    _check(lib().tropical_mixed_step(ctypes.byref(p), ctypes.byref(b), _ptr(q), _ptr(k_new), _ptr(v_new), _ptr(out),
+                                     _ptr(lse), ctypes.c_float(sm_scale), _ptr(ws), ctypes.c_size_t(ws.numel()),
+                                     _stream(stream)), "tropical_mixed_step")
     return out
 
 

@@ -75,14 +75,15 @@ BatchDesc to_batch(const tropical_batch_t* b) {
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-int mixed_attention_impl(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* q, void* out,
-                         float* lse, float sm_scale, void* workspace, size_t workspace_bytes, cudaStream_t stream,
-                         int* launches) {
+// k_new / v_new != nullptr: the fused step
+int mixed_attention_impl(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* q,
+                         const void* k_new, const void* v_new, void* out, float* lse, float sm_scale, void* workspace,
+                         size_t workspace_bytes, cudaStream_t stream, int* launches) {
     (void)workspace_bytes;
     const float scale = sm_scale > 0.f ? sm_scale : 1.0f / sqrtf((float)pool->head_dim);
     const float scale_log2 = scale * 1.4426950408889634f;
-    cudaError_t e = launch_mixed_attention(to_pool(pool), to_batch(batch), q, out, lse, scale_log2, workspace, stream,
-                                           launches);
+    cudaError_t e = launch_mixed_attention(to_pool(pool), to_batch(batch), q, k_new, v_new, out, lse, scale_log2,
+                                           workspace, stream, launches);
     if (e != cudaSuccess) return cuda_fail(e, "mixed_attention");
     return TROPICAL_OK;
 }
@@ -223,7 +224,24 @@ int tropical_mixed_attention(const tropical_kv_pool_t* pool, const tropical_batc
     if (q == nullptr || out == nullptr) return TROPICAL_ERR_INVALID_ARG;
     const size_t need = tropical_workspace_bytes(pool, batch->num_reqs, batch->total_q, batch->max_kv_len);
     if (workspace == nullptr || ((uintptr_t)workspace & 255) || workspace_bytes < need) return TROPICAL_ERR_WORKSPACE;
-    return mixed_attention_impl(pool, batch, q, out, lse, sm_scale, workspace, workspace_bytes,
+    return mixed_attention_impl(pool, batch, q, nullptr, nullptr, out, lse, sm_scale, workspace, workspace_bytes,
+                                (cudaStream_t)cuda_stream, &g_launches);
+}
+
+int tropical_mixed_step(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* q, const void* k_new,
+                        const void* v_new, void* out, float* lse, float sm_scale, void* workspace,
+                        size_t workspace_bytes, void* cuda_stream) {
+    g_launches = 0;
+    int rc = check_pool(pool);
+    if (rc != TROPICAL_OK) return rc;
+    rc = check_batch(pool, batch);
+    if (rc != TROPICAL_OK) return rc;
+    if (batch->total_q == 0) return TROPICAL_OK;
+    if (q == nullptr || out == nullptr || k_new == nullptr || v_new == nullptr) return TROPICAL_ERR_INVALID_ARG;
+    if (((uintptr_t)k_new & 15) || ((uintptr_t)v_new & 15)) return TROPICAL_ERR_INVALID_ARG;  // TMA global address
+    const size_t need = tropical_workspace_bytes(pool, batch->num_reqs, batch->total_q, batch->max_kv_len);
+    if (workspace == nullptr || ((uintptr_t)workspace & 255) || workspace_bytes < need) return TROPICAL_ERR_WORKSPACE;
+    return mixed_attention_impl(pool, batch, q, k_new, v_new, out, lse, sm_scale, workspace, workspace_bytes,
                                 (cudaStream_t)cuda_stream, &g_launches);
 }
 
@@ -302,11 +320,8 @@ int tropical_step_host(const tropical_kv_pool_t* pool, const tropical_host_batch
     b.q_offsets = d_qo;
     b.page_table = d_pt;
     int launches = 0;
-    e = launch_kv_append(to_pool(pool), to_batch(&b), d_k, d_v, stream);
-    if (e != cudaSuccess) return cuda_fail(e, "kv_append");
-    launches += 1;
-    rc = mixed_attention_impl(pool, &b, d_q, d_out, h_lse ? d_lse : nullptr, sm_scale, workspace, workspace_bytes,
-                              stream, &launches);
+    rc = mixed_attention_impl(pool, &b, d_q, d_k, d_v, d_out, h_lse ? d_lse : nullptr, sm_scale, workspace,
+                              workspace_bytes, stream, &launches);  // the fused step: append inside
     if (rc != TROPICAL_OK) return rc;
     e = cudaMemcpyAsync(h_out, d_out, bq, cudaMemcpyDeviceToHost, stream);
     if (e != cudaSuccess) return cuda_fail(e, "step_host D2H");
@@ -347,6 +362,7 @@ int tropical_debug_read_profile(const void* workspace, uint64_t* out_ns, void* c
 void tropical_debug_set_grid(int num_ctas) { set_debug_grid(num_ctas); }
 
 void tropical_debug_set_split_pages(int pages) { set_debug_split_pages(pages); }
+void tropical_debug_set_fused(int mode) { set_debug_fused(mode); }
 
 int tropical_debug_wait_profile(uint64_t* cycles, uint64_t* calls, int32_t n, int32_t reset) {
     if (cycles == nullptr || calls == nullptr || n <= 0) return TROPICAL_ERR_INVALID_ARG;

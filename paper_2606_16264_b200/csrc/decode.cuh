@@ -45,6 +45,10 @@ struct DecodeArgs {
     float2* part_ml;
     float* part_o;
     int* group_cnt;   // per split group (request, kv head, head block): units finished so far; zeroed by the plan kernel
+    // Fused step (tropical_mixed_step): this step's rows [T][Hkv][D], not yet in the pool -- the attention roles read them
+    // from here and idle warps copy them into the pool meanwhile (append_worker).  nullptr: the rows are in the pool.
+    const uint16_t* k_new;
+    const uint16_t* v_new;
 };
 
 // Ring state of one decode warp; persists across units so barrier parities stay consistent.
@@ -56,6 +60,78 @@ struct DecodeRing {
     uint32_t c_phase;  // parity of c_slot's current use
     int i_slot;        // next stage to fill
 };
+
+// Fused step: the request's own new token is not in the pool yet.  Its K (or V) row replaces slot `slot` of the page-head
+// that TMA has just landed in the stage at `stage_s` (SWIZZLE_128B layout: [half][16 slots][128 B], 16-byte chunk c of
+// slot r at r * 128 + ((c ^ (r & 7)) << 4)).  `v` = this lane's 16-byte chunk of the row (lanes < D / 8).
+template <int D>
+__device__ __forceinline__ void patch_new_row(uint32_t stage_s, const uint4& v, int slot, int lane) {
+    if (lane < D / 8) {
+        const uint32_t a = stage_s + (lane >> 3) * DecodeCfg<D>::HALF_BYTES + slot * 128 + (((lane & 7) ^ (slot & 7)) << 4);
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+    }
+    __syncwarp();
+}
+
+// Row A1 inside the step kernel (fused step): warps with nothing else to do -- warp 15 always, the decode workers once
+// their queue is empty -- pop blocks of kAppendTokens new tokens and copy their K / V rows into the pool: lanes look up
+// (page, slot) of the block's tokens, then the warp moves 16-byte chunks, 8 independent rows in flight per lane.  Same
+// bit copy as kv_append_kernel.  Nobody reads these slots from the pool during this step.
+constexpr int kAppendTokens = 2;
+template <int D>
+__device__ __noinline__ void append_worker(const DecodeArgs& A) {
+    if (A.k_new == nullptr) return;
+    constexpr int CH = D / 8;     // 16-byte chunks per row
+    constexpr int RPW = 32 / CH;  // rows (kv heads) per warp pass
+    constexpr int SEG = 2 * kAppendTokens;  // (token, K|V) segments of a block, all in flight together
+    const int lane = threadIdx.x & 31;
+    const int T = A.b.total_q, Hkv = A.pool.Hkv;
+    const int n_tickets = (T + kAppendTokens - 1) / kAppendTokens;
+    int* ticket = const_cast<int*>(A.hdr) + HDR_TICKET_APPEND;
+    const uint4* src_kv[2] = {reinterpret_cast<const uint4*>(A.k_new), reinterpret_cast<const uint4*>(A.v_new)};
+    uint4* dst_kv[2] = {reinterpret_cast<uint4*>(const_cast<uint16_t*>(A.pool.k_pool)),
+                        reinterpret_cast<uint4*>(const_cast<uint16_t*>(A.pool.v_pool))};
+    const int sub = lane / CH, chunk = lane % CH;
+    for (;;) {
+        // look before taking a ticket: at the end of a step every decode worker passes here, and ~1800 atomics on one
+        // address would serialise the kernel's tail
+        if (*reinterpret_cast<volatile int*>(ticket) >= n_tickets) break;
+        int tk = 0;
+        if (lane == 0) tk = atomicAdd(ticket, 1);
+        tk = __shfl_sync(0xffffffffu, tk, 0);
+        if (tk >= n_tickets) break;
+        const int t0 = tk * kAppendTokens, nt = min(kAppendTokens, T - t0);
+        long long base = 0;  // lane i < nt: (page, head 0, slot) of token t0 + i, in 16-byte units
+        if (lane < nt) {
+            const int tok = t0 + lane;
+            const int req = find_request(A.b.q_offsets, A.b.num_reqs, tok);
+            const int pos = __ldg(A.b.ctx_lens + req) + tok - __ldg(A.b.q_offsets + req);
+            const int page = __ldg(A.b.page_table + (size_t)req * A.b.stride + pos / kPageSize);
+            base = ((long long)page * Hkv * kPageSize + pos % kPageSize) * CH;
+        }
+        // segment g = (token g / 2, K|V g % 2): this lane's chunk of kv head `sub`, then heads sub + RPW, ...
+        const uint4* src[SEG];
+        uint4* dst[SEG];
+#pragma unroll
+        for (int g = 0; g < SEG; ++g) {
+            const int i = min(g >> 1, nt - 1);
+            const long long b = __shfl_sync(0xffffffffu, base, i);
+            src[g] = src_kv[g & 1] + ((size_t)(t0 + i) * Hkv + sub) * CH + chunk;
+            dst[g] = dst_kv[g & 1] + b + (long long)sub * kPageSize * CH + chunk;
+        }
+        for (int h = sub; h < Hkv; h += RPW) {
+            uint4 v[SEG];
+#pragma unroll
+            for (int g = 0; g < SEG; ++g) v[g] = __ldg(src[g]);
+#pragma unroll
+            for (int g = 0; g < SEG; ++g) {
+                if ((g >> 1) < nt) *dst[g] = v[g];   // an odd last block: its second token's segments repeat the first's reads
+                src[g] += RPW * CH;
+                dst[g] += RPW * kPageSize * CH;
+            }
+        }
+    }
+}
 
 __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
     uint32_t d;
@@ -110,7 +186,9 @@ __device__ __noinline__ void combine_group(const DecodeArgs& A, size_t u_first, 
     if (A.lse != nullptr && k == 0) A.lse[(size_t)tok * A.pool.Hq + h0 + r] = (M + log2f(l)) * 0.6931471805599453f;
 }
 
-template <int D>
+// FUSED: the fused step (tropical_mixed_step with the append inside the kernel).  The plain variant compiles none of the
+// new-row handling: every instruction in the page loop is paid 300 000 times per C5 step.
+template <int D, bool FUSED>
 __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CUtensorMap* tm_k, const CUtensorMap* tm_v,
                                                    DecodeRing& R) {
     using C = DecodeCfg<D>;
@@ -155,6 +233,9 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
                 qb[ks][1] = row < nh ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + 8 + cq) : 0u;
             }
         }
+        // Fused step: the unit that holds the request's last page takes the new token's K / V row from k_new / v_new
+        // (fused step) page of this unit that holds the request's own new token, whose row is not in the pool yet: -1 = none
+        const int p_patch = (FUSED && (p0 + np) * kPageSize >= L) ? np - 1 : -1;
         // O^T accumulators: o[db][0,1] = d row (db*16 + row) x heads (cq, cq+1); o[db][2,3] = d row + 8
         float o[D / 16][4];
 #pragma unroll
@@ -195,8 +276,14 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
 
         for (int p = 0; p < np; ++p) {
             // ---------------- S^T = K Q^T for the 16 keys of this page
+            const int nvalid = L - (p0 + p) * kPageSize;  // >= 1 by construction of the unit; <= 16 on the request's last page
+            const bool patch = FUSED && p == p_patch;  // the page that holds this step's token (slot nvalid - 1)
+            const size_t new_row = ((size_t)tok * Hkv + kvh) * (D / 8) + lane;  // this lane's 16-byte chunk of the new row
+            uint4 kn = make_uint4(0u, 0u, 0u, 0u);
+            if (patch && lane < D / 8) kn = __ldg(reinterpret_cast<const uint4*>(A.k_new) + new_row);  // in flight while the page lands
             mbar_wait(R.full + R.c_slot, R.c_phase, 201);
             const uint32_t kbase = ring_s + R.c_slot * C::PAGE_BYTES;
+            if (patch) patch_new_row<D>(kbase, kn, nvalid - 1, lane);
             float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
@@ -209,11 +296,11 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
                 if (ks & 1) mma_bf16_16816(sb, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
                 else mma_bf16_16816(sa, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
             }
+            if (patch) fence_proxy_async();  // generic write of the new row before a TMA refill of the stage
             __syncwarp();  // every lane has read the K stage
             consume_advance();
             if (issued < n_sub) issue_one();
 
-            const int nvalid = L - (p0 + p) * kPageSize;  // >= 1 by construction of the unit
             // sa/sb[0,1]: key `row`, heads cq, cq+1;  [2,3]: key row + 8.  Scores relative to the running reference
             // maximum m (shared by the 8 row groups of a head): x = s * scale - m.
             float s00 = sa[0] + sb[0], s01 = sa[1] + sb[1], s10 = sa[2] + sb[2], s11 = sa[3] + sb[3];
@@ -256,8 +343,11 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
             const uint32_t pb1 = movmatrix_trans(pack_bf16x2(v10, v11));
 
             // ---------------- O^T += V^T P^T
+            uint4 vn = make_uint4(0u, 0u, 0u, 0u);
+            if (patch && lane < D / 8) vn = __ldg(reinterpret_cast<const uint4*>(A.v_new) + new_row);
             mbar_wait(R.full + R.c_slot, R.c_phase, 202);
             const uint32_t vbase = ring_s + R.c_slot * C::PAGE_BYTES;
+            if (patch) patch_new_row<D>(vbase, vn, nvalid - 1, lane);
             if (nvalid < kPageSize) {  // ragged last page: unused slots may hold NaN bits; 0 * NaN = NaN in the MMA
                 const int nz = (kPageSize - nvalid) * 8 * C::CB;
                 for (int idx = lane; idx < nz; idx += 32) {
@@ -277,7 +367,7 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
                 ldmatrix_x4_trans(addr, a0, a1, a2, a3);
                 mma_bf16_16816(o[db], a0, a1, a2, a3, pb0, pb1);
             }
-            if (nvalid < kPageSize) fence_proxy_async();  // generic zero-fill before the next TMA refill
+            if (nvalid < kPageSize || patch) fence_proxy_async();  // generic zero-fill / new row before the next TMA refill
             __syncwarp();  // every lane is done with the V stage
             consume_advance();
             if (issued < n_sub) issue_one();
@@ -342,6 +432,7 @@ __device__ __forceinline__ void decode_warp_worker(const DecodeArgs& A, const CU
             }
         }
     }
+    if constexpr (FUSED) append_worker<D>(A);  // what is left of this step's rows to copy into the pool
 }
 
 }  // namespace tropical

@@ -27,10 +27,13 @@ cudaError_t launch_kv_migrate(const MigrateArgs& args, int max_kv_len, cudaStrea
 cudaError_t launch_validate_batch(const PoolDesc& pool, const BatchDesc& b, int* first_bad_dev, cudaStream_t stream);
 cudaError_t launch_attention_simt(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
                                   float scale_log2, cudaStream_t stream);
-cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
-                                   float scale_log2, void* workspace, cudaStream_t stream, int* launches);
+// k_new / v_new != nullptr: the fused step (the rows are read from there and appended to the pool inside the kernel)
+cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, const void* k_new,
+                                   const void* v_new, void* out, float* lse, float scale_log2, void* workspace,
+                                   cudaStream_t stream, int* launches);
 void set_debug_grid(int num_ctas);
 void set_debug_split_pages(int pages);
+void set_debug_fused(int mode);
 int read_wait_profile(unsigned long long* cycles, unsigned long long* calls, int n, int reset);
 size_t profile_offset_bytes();
 int read_timeline_append(unsigned long long* out16, int reset);  // 0 unless built with -DTROPICAL_TIMELINE

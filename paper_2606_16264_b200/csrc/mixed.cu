@@ -40,6 +40,11 @@ __device__ __forceinline__ void prof_mark(const int* hdr, int which, bool is_min
 //   warps 0-3       : prefill softmax warpgroup (both query tiles of a two-tile item, alternately)
 //   warps 8, 9, 10  : prefill K producer (TMA; pops the item tickets), tcgen05 MMA issuer, V producer
 //   warps 4-7, 11-14: decode warp workers, a private TMA ring each (HBM streaming; csrc/decode.cuh)
+//   warp 15         : FUSED variant only: copies this step's K / V rows into the pool (append_worker); else idle
+// (Softmax on warps 12-15 -- the issue arbiter is said to prefer the highest warp id of a sub-partition -- was measured:
+// no gain, profiles/r2e_fused_step.md.)
+// Two variants: FUSED = false is the step kernel of tropical_mixed_attention (this step's rows are in the pool);
+// FUSED = true is tropical_mixed_step's for prefill-dominated steps: the rows are read from k_new / v_new and appended here.
 // Prefill items and decode units are popped from two ticket counters, so on every SM the tensor pipe (prefill) and
 // the HBM stream (decode) are busy at the same time -- the paper's multiplexing at SM granularity.  When the prefill
 // queue is empty the four softmax warps become decode workers too, with rings carved out of the (now idle) prefill
@@ -63,10 +68,18 @@ struct MixedCfg {
     static_assert(SMEM <= 232448, "shared memory per CTA");
 };
 
-template <int D>
+// Tensor maps of a step: Q, the K / V pools as page-head halves (16 slots) and single slots, and -- fused step only --
+// this step's rows k_new / v_new as 16-token and single-token boxes.
+struct StepMaps {
+    CUtensorMap q, k16, v16, k1, v1, kn16, vn16, kn1, vn1;
+};
+
+template <int D, bool FUSED>
 __global__ void __launch_bounds__(kMixedThreads, 1)
-mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap tm_q,
-             const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v) {
+mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ StepMaps TM) {
+    const CUtensorMap* const tm_q = &TM.q;
+    const CUtensorMap* const tm_k = &TM.k16;
+    const CUtensorMap* const tm_v = &TM.v16;
     using C = PrefillCfg<D>;
     using M = MixedCfg<D>;
     extern __shared__ uint8_t smem_raw[];
@@ -77,9 +90,9 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
     const int warp = uni((int)(threadIdx.x >> 5));
     if (threadIdx.x == 0) tl_mark(5, true);
     if (threadIdx.x == 0) {
-        tma_prefetch_desc(&tm_q);
-        tma_prefetch_desc(&tm_k);
-        tma_prefetch_desc(&tm_v);
+        tma_prefetch_desc(tm_q);
+        tma_prefetch_desc(tm_k);
+        tma_prefetch_desc(tm_v);
         prefill_init_bars(PB);
         for (int i = 0; i < M::N_DEC_BARS; ++i) mbar_init(dec_full + i, 1);
         fence_mbar_init();
@@ -107,19 +120,21 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
         named_bar_sync(1, 128);
         DecodeRing R = make_ring(tiles + warp * M::LATE_RING, dec_full + M::DEC_WARPS * M::DEC_STAGES + warp * M::LATE_STAGES,
                                  M::LATE_STAGES);
-        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
+        decode_warp_worker<D, FUSED>(DA, tm_k, tm_v, R);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
     } else if (warp == 8) {
-        prefill_producer<D, 0>(PA, PB, tiles, &tm_q, &tm_k);
+        prefill_producer<D, 0, FUSED>(PA, PB, tiles, tm_q, KvMaps{&TM.k16, &TM.k1, &TM.kn16, &TM.kn1});
     } else if (warp == 9) {
         prefill_mma<D>(PA, PB, tiles);
     } else if (warp == 10) {
-        prefill_producer<D, 1>(PA, PB, tiles, &tm_q, &tm_v);
+        prefill_producer<D, 1, FUSED>(PA, PB, tiles, tm_q, KvMaps{&TM.v16, &TM.v1, &TM.vn16, &TM.vn1});
     } else if (warp != 15) {
         const int dw = warp < 8 ? warp - 4 : warp - 7;
         DecodeRing R = make_ring(rings + dw * M::DEC_RING, dec_full + dw * M::DEC_STAGES, M::DEC_STAGES);
-        decode_warp_worker<D>(DA, &tm_k, &tm_v, R);
+        decode_warp_worker<D, FUSED>(DA, tm_k, tm_v, R);
         if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 2, false);
+    } else if (FUSED) {
+        append_worker<D>(DA);  // warp 15: copies this step's rows into the pool beside the attention roles
     }
     tc_fence_before();
     __syncthreads();
@@ -131,7 +146,7 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ CUtensorMap 
 constexpr int kMaxDevices = 64;
 struct DeviceState {
     std::atomic<int> num_sms{0};
-    std::atomic<int> smem_attr_set{0};  // bit 0: mixed_kernel<128>, bit 1: mixed_kernel<64>, bit 2: plan_kernel carve-out
+    std::atomic<int> smem_attr_set{0};  // bits 0, 1: mixed_kernel<128 / 64, plain>, bit 2: plan_kernel carve-out, bits 3, 4: fused variants
 };
 static DeviceState g_dev[kMaxDevices];
 
@@ -218,9 +233,27 @@ static std::atomic<int> g_split_pages{0};  // test hook: 0 = automatic
 void set_debug_split_pages(int pages) { g_split_pages.store(pages > 0 ? (pages + 7) / 8 * 8 : 0); }
 void set_debug_grid(int num_ctas) { g_grid_cap.store(num_ctas > 0 ? num_ctas : 0); }
 
-template <int D>
-static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
-                                  float scale_log2, void* workspace, cudaStream_t stream, int* launches) {
+static std::atomic<int> g_fused_mode{-1};  // test hook: -1 = the heuristic below, 0 = never fuse, 1 = always fuse
+void set_debug_fused(int mode) { g_fused_mode.store(mode < 0 ? -1 : (mode ? 1 : 0)); }
+
+// tropical_mixed_step: fuse the append into the step kernel, or run the append kernel in front of the plain one?
+// Measured (profiles/r2e_fused_step.md): the fused variant takes the append off the critical path (C3, prefill-only:
+// 62 -> 50 us) but its extra work in the hot loops -- the new-row patch of the decode page loop, the append warp --
+// costs 1-4 % on steps that stream a large decode batch (C2 +0.4 %, C5 +4 %), where the separate append is 2 % of the
+// step to begin with.  The host sees only the scalars of the batch, not its contexts: a step is taken as
+// prefill-dominated when its requests carry at least kFusedMinTokensPerReq new tokens on average, i.e. when it has at
+// most one decode request per ~64 prefill tokens.
+constexpr int kFusedMinTokensPerReq = 64;
+static bool choose_fused(const BatchDesc& b) {
+    const int mode = g_fused_mode.load(std::memory_order_relaxed);
+    if (mode >= 0) return mode == 1;
+    return (long long)b.total_q >= (long long)kFusedMinTokensPerReq * b.num_reqs;
+}
+
+template <int D, bool FUSED>
+static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, const void* q, const void* k_new,
+                                  const void* v_new, void* out, float* lse, float scale_log2, void* workspace,
+                                  cudaStream_t stream, int* launches) {
     const WorkspaceLayout w = make_layout(pool.Hq, pool.Hkv, D, b.num_reqs, b.total_q);
     char* ws = (char*)workspace;
     PlanPtrs P;
@@ -257,11 +290,23 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     if (e != cudaSuccess) return e;
     ++*launches;
 
-    CUtensorMap tm_q, tm_k, tm_v;
+    StepMaps TM;
     const long long rows = (long long)pool.num_pages * pool.Hkv * kPageSize;
-    if (!encode_pool_map(&tm_k, pool.k_pool, rows, D) || !encode_pool_map(&tm_v, pool.v_pool, rows, D) ||
-        !encode_q_map(&tm_q, q, b.total_q, pool.Hq, D, 1, kQTile))
+    constexpr bool fused = FUSED;
+    if (!encode_pool_map(&TM.k16, pool.k_pool, rows, D) || !encode_pool_map(&TM.v16, pool.v_pool, rows, D) ||
+        !encode_q_map(&TM.q, q, b.total_q, pool.Hq, D, 1, kQTile))
         return cudaErrorInvalidValue;
+    if (fused) {
+        if (!encode_pool_map(&TM.k1, pool.k_pool, rows, D, 1) || !encode_pool_map(&TM.v1, pool.v_pool, rows, D, 1) ||
+            !encode_q_map(&TM.kn16, k_new, b.total_q, pool.Hkv, D, 1, kPageSize) ||
+            !encode_q_map(&TM.vn16, v_new, b.total_q, pool.Hkv, D, 1, kPageSize) ||
+            !encode_q_map(&TM.kn1, k_new, b.total_q, pool.Hkv, D, 1, 1) ||
+            !encode_q_map(&TM.vn1, v_new, b.total_q, pool.Hkv, D, 1, 1))
+            return cudaErrorInvalidValue;
+    } else {  // never dereferenced
+        TM.k1 = TM.kn16 = TM.kn1 = TM.k16;
+        TM.v1 = TM.vn16 = TM.vn1 = TM.v16;
+    }
 
     PrefillArgs PA;
     PA.pool = pool;
@@ -287,15 +332,17 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     A.part_ml = (float2*)(ws + w.part_ml);
     A.part_o = (float*)(ws + w.part_o);
     A.group_cnt = P.group_cnt;
+    A.k_new = FUSED ? (const uint16_t*)k_new : nullptr;
+    A.v_new = FUSED ? (const uint16_t*)v_new : nullptr;
 
 #ifdef TROPICAL_DEBUG_WAIT
     debug_wait_setup();
 #endif
     // A3 + A4 + A5 in one persistent launch
     const size_t smem = MixedCfg<D>::SMEM;
-    const int attr_bit = D == 128 ? 1 : 2;
+    const int attr_bit = (D == 128 ? 1 : 2) << (FUSED ? 3 : 0);  // bits 0, 1: plain variants; bits 3, 4: fused variants
     if (!(ds.smem_attr_set.load(std::memory_order_acquire) & attr_bit)) {
-        e = cudaFuncSetAttribute(mixed_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(mixed_kernel<D, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         ds.smem_attr_set.fetch_or(attr_bit, std::memory_order_release);
     }
@@ -307,17 +354,29 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     mcfg.stream = stream;
     mcfg.attrs = attr;  // programmatic stream serialization: its prologue overlaps the directory kernel (which triggers at once)
     mcfg.numAttrs = 1;
-    e = cudaLaunchKernelEx(&mcfg, mixed_kernel<D>, PA, A, tm_q, tm_k, tm_v);
+    e = cudaLaunchKernelEx(&mcfg, mixed_kernel<D, FUSED>, PA, A, TM);
     if (e != cudaSuccess) return e;
     ++*launches;
 
     return cudaSuccess;
 }
 
-cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, void* out, float* lse,
-                                   float scale_log2, void* workspace, cudaStream_t stream, int* launches) {
-    if (pool.D == 128) return launch_mixed_t<128>(pool, b, q, out, lse, scale_log2, workspace, stream, launches);
-    return launch_mixed_t<64>(pool, b, q, out, lse, scale_log2, workspace, stream, launches);
+cudaError_t launch_mixed_attention(const PoolDesc& pool, const BatchDesc& b, const void* q, const void* k_new,
+                                   const void* v_new, void* out, float* lse, float scale_log2, void* workspace,
+                                   cudaStream_t stream, int* launches) {
+    if (k_new != nullptr && choose_fused(b)) {  // tropical_mixed_step, append inside the step kernel
+        if (pool.D == 128)
+            return launch_mixed_t<128, true>(pool, b, q, k_new, v_new, out, lse, scale_log2, workspace, stream, launches);
+        return launch_mixed_t<64, true>(pool, b, q, k_new, v_new, out, lse, scale_log2, workspace, stream, launches);
+    }
+    if (k_new != nullptr) {  // tropical_mixed_step on a decode-heavy step: the append kernel in front of the plain variant
+        const cudaError_t e = launch_kv_append(pool, b, k_new, v_new, stream);
+        if (e != cudaSuccess) return e;
+        ++*launches;
+    }
+    if (pool.D == 128)
+        return launch_mixed_t<128, false>(pool, b, q, nullptr, nullptr, out, lse, scale_log2, workspace, stream, launches);
+    return launch_mixed_t<64, false>(pool, b, q, nullptr, nullptr, out, lse, scale_log2, workspace, stream, launches);
 }
 
 // measurement builds (-DTROPICAL_TIMELINE): this translation unit's copy of the timestamps (slots 2 .. 8)

@@ -15,6 +15,7 @@ constexpr int kMinSplitPages = 8;    // never split finer than 128 tokens
 constexpr int kSmallBatchSplitPages = 32;  // ... nor finer than 512 tokens when a request has at least 1024 (see plan_kernel)
 
 enum { HDR_N_ITEMS = 0, HDR_N_UNITS = 1, HDR_SPLIT_PAGES = 2, HDR_TICKET_PREFILL = 3, HDR_TICKET_DECODE = 4,
+       HDR_TICKET_APPEND = 5 /* fused step: blocks of new tokens whose rows are copied into the pool */,
        HDR_PROF = 16 /* 4 x u64: kernel start (min), prefill end, WG1 decode end, WG0 decode end (max) */,
        HDR_INTS = 64 };
 
@@ -190,6 +191,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         P.hdr[HDR_SPLIT_PAGES] = split;
         P.hdr[HDR_TICKET_PREFILL] = 0;
         P.hdr[HDR_TICKET_DECODE] = 0;
+        P.hdr[HDR_TICKET_APPEND] = 0;
         unsigned long long* prof = reinterpret_cast<unsigned long long*>(P.hdr + HDR_PROF);
         prof[0] = ~0ull;
         prof[1] = prof[2] = prof[3] = 0ull;

@@ -69,6 +69,15 @@ struct PrefillArgs {
     const int2* items;
 };
 
+// Tensor maps of one of K / V for the prefill producers: the pool as 16-slot boxes (one page-head half) and as single
+// slots, and this step's rows [T][Hkv][D] as 16-token and single-token boxes (fused step only).
+struct KvMaps {
+    const CUtensorMap* pool16;
+    const CUtensorMap* pool1;
+    const CUtensorMap* new16;
+    const CUtensorMap* new1;
+};
+
 struct PrefillItem {
     int req, qt, h, hk, nt;   // nt query tiles: heads h .. h + nt - 1 (same kv head hk)
     int c, ql, tok0;          // context length, chunk length, first packed row of the request
@@ -121,10 +130,13 @@ __device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
 // tile is 16 TMA boxes).
 
 // One KV tile (8 page-heads) of item `it` into the cursor's slot: lane -> (page p, half cb), one box per lane.
-template <int D>
+// Fused step: keys below the request's prior context c come from the pool, keys from c on are this step's rows and
+// come from k_new / v_new (token row tok0 + key - c); the one page that holds both (c not a multiple of 16) is loaded
+// slot by slot.  The bytes per tile are the same in every case.
+template <int D, bool FUSED>
 __device__ __forceinline__ void prefill_load_tile(const PrefillArgs& A, PrefillBars* B, uint8_t* ring,
                                                   const PrefillItem& it, const int* pt, int n_pages, int kt,
-                                                  const CUtensorMap* tm, const RingCursor& cur, int lane) {
+                                                  const KvMaps& tm, const RingCursor& cur, int lane) {
     using C = PrefillCfg<D>;
     const int np = min(8, n_pages - kt * 8);
     const int p = lane / C::CB, cb = lane % C::CB;
@@ -143,14 +155,28 @@ __device__ __forceinline__ void prefill_load_tile(const PrefillArgs& A, PrefillB
     if (lane == 0) mbar_arrive_expect_tx(&B->kv_full[cur.slot], np * C::CB * C::PAGE_BOX);
 #endif
     __syncwarp();
-    if (act) tma_load_2d(ring + cur.slot * C::TILE_BYTES + off, tm, cb * 64, r0, &B->kv_full[cur.slot]);
+    if (act) {
+        uint8_t* dst = ring + cur.slot * C::TILE_BYTES + off;
+        const int key0 = (kt * 8 + p) * kPageSize;
+        if (!FUSED || key0 + kPageSize <= it.c) {
+            tma_load_2d(dst, tm.pool16, cb * 64, r0, &B->kv_full[cur.slot]);
+        } else if (key0 >= it.c) {
+            tma_load_3d(dst, tm.new16, cb * 64, it.hk, it.tok0 + key0 - it.c, &B->kv_full[cur.slot]);
+        } else {
+#pragma unroll 1
+            for (int r = 0; r < kPageSize; ++r) {  // rare (one page per chunk whose context is not a multiple of 16): keep it small
+                if (key0 + r < it.c) tma_load_2d(dst + r * 128, tm.pool1, cb * 64, r0 + r, &B->kv_full[cur.slot]);
+                else tma_load_3d(dst + r * 128, tm.new1, cb * 64, it.hk, it.tok0 + key0 + r - it.c, &B->kv_full[cur.slot]);
+            }
+        }
+    }
 }
 
 // KIND 0: pops the item tickets, loads the Q tiles and the K tiles.  KIND 1: the V tiles of the same item sequence
 // (item ids come through the mailbox).
-template <int D, int KIND>
+template <int D, int KIND, bool FUSED>
 __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBars* B, uint8_t* tiles,
-                                                 const CUtensorMap* tm_q, const CUtensorMap* tm_kv) {
+                                                 const CUtensorMap* tm_q, const KvMaps tm_kv) {
     using C = PrefillCfg<D>;
     const int lane = threadIdx.x & 31;
     const int n_items = uni(A.hdr[HDR_N_ITEMS]);
@@ -191,9 +217,9 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
         }
         const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
         for (int kt = 0; kt < it.n_kt; ++kt) {  // ring entries 2 kt (K) and 2 kt + 1 (V)
-            if (KIND == 0) prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt, tm_kv, cur, lane);
+            if (KIND == 0) prefill_load_tile<D, FUSED>(A, B, ring, it, pt, n_pages, kt, tm_kv, cur, lane);
             cur.advance(C::KV_SLOTS);
-            if (KIND == 1) prefill_load_tile<D>(A, B, ring, it, pt, n_pages, kt, tm_kv, cur, lane);
+            if (KIND == 1) prefill_load_tile<D, FUSED>(A, B, ring, it, pt, n_pages, kt, tm_kv, cur, lane);
             cur.advance(C::KV_SLOTS);
         }
         ++item_it;

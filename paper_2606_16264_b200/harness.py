@@ -49,10 +49,25 @@ class DeviceStep:
                                workspace=self.workspace)
         return self.out
 
-    def step(self, sm_scale=0.0, impl="product"):
-        """append + attention, synchronised; returns (out f64 [T,Hq,d], lse f64 [T,Hq]) on the host."""
-        self.append()
-        self.attention(sm_scale, impl)
+    def fused_step(self, sm_scale=0.0):
+        """tropical_mixed_step: the append fused into the attention step (one call)."""
+        tb.mixed_step(self.pool, self.batch, self.q, self.k_new, self.v_new, out=self.out, lse=self.lse,
+                      sm_scale=sm_scale, workspace=self.workspace)
+        return self.out
+
+    def step(self, sm_scale=0.0, impl="fused"):
+        """One iteration, synchronised; returns (out f64 [T,Hq,d], lse f64 [T,Hq]) on the host.  impl "fused": the single
+        call tropical_mixed_step with its fused kernel variant forced (append inside the step kernel); "auto": the same
+        call with its own choice of variant; "product" / "simt": tropical_kv_append followed by the attention call."""
+        if impl in ("fused", "auto"):
+            tb.debug_set_fused(1 if impl == "fused" else -1)
+            try:
+                self.fused_step(sm_scale)
+            finally:
+                tb.debug_set_fused(-1)
+        else:
+            self.append()
+            self.attention(sm_scale, impl)
         torch.cuda.synchronize()
         return self.out_f64(), self.lse.cpu().numpy().astype(np.float64)
 

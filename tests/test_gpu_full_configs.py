@@ -17,13 +17,16 @@ from tests.gpu_harness import MAX_ABS_TOL, MEAN_ABS_TOL, DeviceStep, bits
 pytestmark = pytest.mark.gpu
 
 
+@pytest.mark.parametrize("impl", ["auto", "fused", "product"])
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
-def test_full_config_all_rows_parity(name):
+def test_full_config_all_rows_parity(name, impl):
     s = synth.make_config(name, poison=True, values="tiled")
     kp, vp = s.copy_pools()
     oracle.kv_append(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new)
     dev = DeviceStep(s)
-    out, lse = dev.step()
+    # "auto": tropical_mixed_step as bench.py times it (its own choice of kernel variant); "fused": the same call with the
+    # fused variant forced (append inside the step kernel); "product": tropical_kv_append + tropical_mixed_attention
+    out, lse = dev.step(impl=impl)
     # A1 / A2 at full size: whole pool bit-identical (also proves attention wrote nothing into it)
     assert np.array_equal(bits(dev.k_pool), kp), "K pool differs"
     assert np.array_equal(bits(dev.v_pool), vp), "V pool differs"

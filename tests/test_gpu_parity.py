@@ -21,23 +21,32 @@ def _step(seed, Hq, Hkv, d, q_lens, ctx_lens, **kw):
     return synth.make_step(np.random.default_rng(seed), Hq, Hkv, d, 16, q_lens, ctx_lens, **kw)
 
 
-def _check_step(s, impl="product", sm_scale=0.0, lse_tol=2e-3):
+def _check_step(s, impl="both", sm_scale=0.0, lse_tol=2e-3):
+    """impl "product": tropical_kv_append + tropical_mixed_attention; "fused": the single call tropical_mixed_step (append
+    inside the step kernel, new rows read from k_new / v_new); "both" (default): each against the oracle, and the two
+    outputs bit-identical to one another (same bits in, same work decomposition)."""
     ref_out, ref_lse, kp, vp = oracle.step(s, sm_scale)
-    dev = DeviceStep(s)
-    out, lse = dev.step(sm_scale, impl)
-    # A1/A2: pool bit-identical to the oracle's over the whole pool; attention never writes it
-    assert np.array_equal(bits(dev.k_pool), kp), "K pool differs"
-    assert np.array_equal(bits(dev.v_pool), vp), "V pool differs"
-    assert np.isfinite(out).all()
-    mx, mean = errors(out, ref_out)
-    assert mx <= MAX_ABS_TOL and mean <= MEAN_ABS_TOL, (mx, mean)
-    if s.total_q:
-        assert np.abs(lse - ref_lse).max() <= lse_tol
+    outs = []
+    for one in (("product", "fused") if impl == "both" else (impl,)):
+        dev = DeviceStep(s)
+        out, lse = dev.step(sm_scale, one)
+        # A1/A2: pool bit-identical to the oracle's over the whole pool; the attention roles never write elsewhere
+        assert np.array_equal(bits(dev.k_pool), kp), f"K pool differs ({one})"
+        assert np.array_equal(bits(dev.v_pool), vp), f"V pool differs ({one})"
+        assert np.isfinite(out).all()
+        mx, mean = errors(out, ref_out)
+        assert mx <= MAX_ABS_TOL and mean <= MEAN_ABS_TOL, (one, mx, mean)
+        if s.total_q:
+            assert np.abs(lse - ref_lse).max() <= lse_tol
+        outs.append(bits(dev.out).copy())
+        del dev
+    if len(outs) == 2:
+        assert np.array_equal(outs[0], outs[1]), "fused step and append + attention differ"
     return mx, mean
 
 
 # ------------------------------------------------------------------ BASELINE configs[0]
-@pytest.mark.parametrize("impl", ["product", "simt"])
+@pytest.mark.parametrize("impl", ["product", "fused", "auto", "simt"])
 def test_C1_tiny_mixed_step(impl):
     s = synth.make_config("C1")
     mx, mean = _check_step(s, impl)
@@ -153,9 +162,10 @@ def _needle_step(d, c, ql, targets_fn, Hq=2, Hkv=1, seed=0, values="normal"):
     return s, targets, Vb
 
 
+@pytest.mark.parametrize("impl", ["fused", "product"])
 @pytest.mark.parametrize("d", [64, 128])
-@pytest.mark.parametrize("c,ql", [(300, 200), (0, 257), (4090, 1), (1000, 1), (127, 130)])
-def test_needle_selects_target_row_bitwise(d, c, ql):
+@pytest.mark.parametrize("c,ql", [(300, 200), (0, 257), (4090, 1), (1000, 1), (127, 130), (16, 129), (15, 2), (4095, 1)])
+def test_needle_selects_target_row_bitwise(d, c, ql, impl):
     edges = [0, 15, 16, 17, 127, 128, 129, 255, 256, 257, 511, 512, 513, 1023, 1024, 1025]
 
     def target(t):
@@ -171,19 +181,20 @@ def test_needle_selects_target_row_bitwise(d, c, ql):
 
     s, targets, Vb = _needle_step(d, c, ql, target)
     dev = DeviceStep(s)
-    dev.step()
+    dev.step(impl=impl)   # fused: the just-appended rows reach the tiles from k_new / v_new, not through the pool
     got = bits(dev.out)
     for t, j in enumerate(targets):
         for h in range(s.num_q_heads):
             assert np.array_equal(got[t, h], Vb[j, 0]), f"row {t} head {h}: expected V[{j}]"
 
 
-def test_negative_needle_future_key_not_selected():
+@pytest.mark.parametrize("impl", ["fused", "product"])
+def test_negative_needle_future_key_not_selected(impl):
     c, ql, d = 40, 50, 128
     s, targets, Vb = _needle_step(d, c, ql, lambda t: min(c + t + 1, c + ql - 1))
     ref, _, _, _ = oracle.step(s)
     dev = DeviceStep(s)
-    out, _ = dev.step()
+    out, _ = dev.step(impl=impl)
     assert errors(out, ref)[0] <= MAX_ABS_TOL
     got = bits(dev.out)
     assert not np.array_equal(got[3, 0], Vb[c + 3 + 1, 0])
@@ -215,6 +226,41 @@ def test_append_then_attention_ordering_stress():
             got = bits(dev.out)
             assert np.array_equal(got, v_sets[rep & 1][:, :, :]), f"repetition {rep}: stale or poisoned rows were read"
     torch.cuda.synchronize()
+
+
+def test_fused_step_never_reads_the_slots_it_appends():
+    """tropical_mixed_step: the attention roles take this step's rows from k_new / v_new while other warps of the same
+    kernel copy them into the pool.  The target slots hold NaN patterns when the kernel starts and V alternates between
+    two draws, 100 times, on a mixed batch whose chunk starts in the middle of a page (context 1000 = 62.5 pages) next to
+    decode requests whose new token lands on every slot position: needle queries select just-appended rows bit-exactly,
+    and after every repetition the pool holds exactly the appended rows."""
+    d, H = 128, 8
+    rng = np.random.default_rng(41)
+    ql, c = 600, 1000
+    s, targets, Vb = _needle_step(d, c, ql, lambda t: c + t, Hq=H, Hkv=H, seed=7)
+    dev = DeviceStep(s)
+    v_alt = f32_to_bf16_bits(rng.standard_normal((ql, 1, d)).astype(np.float32))
+    v_sets = [s.v_new.copy(), np.ascontiguousarray(np.broadcast_to(v_alt, (ql, H, d)))]
+    v_dev = [torch.from_numpy(v.view(np.int16)).cuda() for v in v_sets]
+    pos = torch.arange(c, c + ql, device="cuda")
+    pages, slots = dev.batch.page_table[0, (pos // 16).long()].long(), (pos % 16).long()
+    for rep in range(100):
+        dev.k_pool[pages, :, slots] = synth.POISON_BF16
+        dev.v_pool[pages, :, slots] = synth.POISON_BF16
+        dev.out.zero_()
+        tb.debug_set_fused(1)   # the fused variant whatever the batch (this one would choose it anyway)
+        try:
+            tb.mixed_step(dev.pool, dev.batch, dev.q, dev.k_new, v_dev[rep & 1], out=dev.out, workspace=dev.workspace)
+        finally:
+            tb.debug_set_fused(-1)
+        if rep % 10 == 9 or rep < 4:
+            torch.cuda.synchronize()
+            assert np.array_equal(bits(dev.out), v_sets[rep & 1]), f"repetition {rep}: poisoned or stale rows were read"
+            assert np.array_equal(bits(dev.v_pool[pages, :, slots]), v_sets[rep & 1]), f"repetition {rep}: append incomplete"
+            assert np.array_equal(bits(dev.k_pool[pages, :, slots]), s.k_new)
+    torch.cuda.synchronize()
+    # decode requests whose new token lands on each of the 16 slots of its page, poisoned pool, both paths
+    _check_step(_step(42, 8, 2, 128, [1] * 16 + [37], [200 + k for k in range(16)] + [5], poison=True))
 
 
 def test_head_sharded_step_equals_unsharded_bit_for_bit():
@@ -384,6 +430,47 @@ def test_step_is_cuda_graph_capturable_and_idempotent():
         assert np.array_equal(bits(dev.out), eager)
     assert np.array_equal(bits(dev.k_pool), kp) and np.array_equal(bits(dev.v_pool), vp)
     assert errors(dev.out_f64(), ref)[0] <= MAX_ABS_TOL
+
+
+def test_fused_step_is_cuda_graph_capturable():
+    s = _step(18, 8, 2, 128, [200, 1, 1, 1, 33], [56, 700, 2049, 17, 0])
+    ref, _, kp, vp = oracle.step(s)
+    dev = DeviceStep(s)
+    dev.step(impl="fused")
+    eager = bits(dev.out).copy()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    tb.debug_set_fused(1)
+    try:
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                dev.fused_step()
+    finally:
+        tb.debug_set_fused(-1)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(3):
+        dev.out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(bits(dev.out), eager)
+    assert np.array_equal(bits(dev.k_pool), kp) and np.array_equal(bits(dev.v_pool), vp)
+    assert errors(dev.out_f64(), ref)[0] <= MAX_ABS_TOL
+
+
+def test_mixed_step_chooses_its_variant_from_the_batch_scalars():
+    """tropical_mixed_step fuses the append into the step kernel on prefill-dominated steps (>= 64 new tokens per request
+    on average: 2 launches) and runs the append kernel in front of the plain variant otherwise (3 launches); both
+    leave the same pool and the same output bits."""
+    outs = []
+    for q, c, launches in (([200, 1], [56, 700], 2), ([200] + [1] * 7, [56] + [700] * 7, 3)):
+        s = _step(21, 8, 2, 128, q, c)
+        ref, _, kp, vp = oracle.step(s)
+        dev = DeviceStep(s)
+        dev.step(impl="auto")
+        assert tb.last_launch_count() == launches
+        assert np.array_equal(bits(dev.k_pool), kp) and np.array_equal(bits(dev.v_pool), vp)
+        assert errors(dev.out_f64(), ref)[0] <= MAX_ABS_TOL
 
 
 def test_more_requests_than_plan_threads():
