@@ -5,7 +5,7 @@
     python -m paper_2606_16264_b200.cost_fit sweep-split  [--out split_sweep.csv]             # needs a B200
     python -m paper_2606_16264_b200.cost_fit fit     [--grid calibration/b200_grid.csv]  # CPU only
 
-`measure` times append + attention (CUDA events, inputs resident) over a grid of synthetic batches --
+`measure` times the step -- tropical_mixed_step: KV append + attention in one call -- (CUDA events, inputs resident) over a grid of synthetic batches --
 prefill tokens x decode requests x decode-context median (lognormal, sigma 0.9), plus chunk-on-context points
 (PAPER.md:159 chunked prefill: later chunks see more prior context) -- for each head configuration and writes
 one CSV row per point.  `fit` regenerates every point's lengths from its recipe columns, fits the six
@@ -114,9 +114,8 @@ def _points_on_device(shapes, pts):
             out = torch.empty_like(qd)
             ws = torch.empty(tb.workspace_bytes(pool, n, T, int(L.max())) + 256, dtype=torch.uint8, device=dev)
 
-            def step():
-                tb.kv_append(pool, batch, kn, vn)
-                tb.mixed_attention(pool, batch, qd, out=out, workspace=ws)
+            def step():   # the product step: one call, append fused or in front (tropical_mixed_step's own choice)
+                tb.mixed_step(pool, batch, qd, kn, vn, out=out, workspace=ws)
 
             yield Hq, Hkv, d, p, step
         del k_pool, v_pool, pool

@@ -41,6 +41,10 @@ __device__ __forceinline__ void prof_mark(const int* hdr, int which, bool is_min
 //   warps 8, 9, 10  : prefill K producer (TMA; pops the item tickets), tcgen05 MMA issuer, V producer
 //   warps 4-7, 11-14: decode warp workers, a private TMA ring each (HBM streaming; csrc/decode.cuh)
 //   warp 15         : FUSED variant only: copies this step's K / V rows into the pool (append_worker); else idle
+// FUSED variant (prefill-dominated steps, where the decode warps have little to do): warps 4-7 are a SECOND softmax
+// warpgroup -- warpgroup w owns query tile w of every item, so each scheduler has two softmax warps hiding one
+// another's latencies -- and MHA items carry two row tiles of one head (csrc/plan.cuh) so that both always have work;
+// they turn into decode workers when the prefill queue is empty, like warps 0-3.
 // (Softmax on warps 12-15 -- the issue arbiter is said to prefer the highest warp id of a sub-partition -- was measured:
 // no gain, profiles/r2e_fused_step.md.)
 // Two variants: FUSED = false is the step kernel of tropical_mixed_attention (this step's rows are in the pool);
@@ -93,7 +97,7 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ StepMaps TM)
         tma_prefetch_desc(tm_q);
         tma_prefetch_desc(tm_k);
         tma_prefetch_desc(tm_v);
-        prefill_init_bars(PB);
+        prefill_init_bars(PB, FUSED ? 8 : 4);
         for (int i = 0; i < M::N_DEC_BARS; ++i) mbar_init(dec_full + i, 1);
         fence_mbar_init();
     }
@@ -112,20 +116,25 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ StepMaps TM)
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    if (warp < 4) {
-        prefill_softmax<D>(PA, PB, warp);
-        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 1, false);
-        // The terminating ticket was seen after the last item's final epilogue: every prefill MMA has completed, so
-        // every TMA load into the tile memory has been consumed and the producers issue nothing more.
-        named_bar_sync(1, 128);
-        DecodeRing R = make_ring(tiles + warp * M::LATE_RING, dec_full + M::DEC_WARPS * M::DEC_STAGES + warp * M::LATE_STAGES,
-                                 M::LATE_STAGES);
+    if (warp < (FUSED ? 8 : 4)) {
+        // one code instance for both softmax warpgroups of the FUSED variant (they share the instruction cache)
+        const int wg = FUSED ? warp >> 2 : 0, sw = warp & 3;  // warpgroup = query tile it owns; sw = TMEM lane quadrant
+        prefill_softmax<D, FUSED, FUSED ? 2 : 1>(PA, PB, sw, wg);
+        if ((threadIdx.x & 31) == 0 && wg == 0) prof_mark(PA.hdr, 1, false);
+        // The terminating ticket was seen after the last item's final epilogue (of BOTH warpgroups in the two-warpgroup
+        // variant): every prefill MMA has completed, so every TMA load into the tile memory has been consumed and the
+        // producers issue nothing more.  Warpgroup 0 then streams decode units through rings carved out of the tile
+        // memory, warpgroup 1 through the rings of the decode workers it replaced.
+        named_bar_sync(1, FUSED ? 256 : 128);
+        DecodeRing R = wg == 0 ? make_ring(tiles + sw * M::LATE_RING,
+                                           dec_full + M::DEC_WARPS * M::DEC_STAGES + sw * M::LATE_STAGES, M::LATE_STAGES)
+                               : make_ring(rings + sw * M::DEC_RING, dec_full + sw * M::DEC_STAGES, M::DEC_STAGES);
         decode_warp_worker<D, FUSED>(DA, tm_k, tm_v, R);
-        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, 3, false);
+        if ((threadIdx.x & 31) == 0) prof_mark(PA.hdr, wg == 0 ? 3 : 2, false);
     } else if (warp == 8) {
         prefill_producer<D, 0, FUSED>(PA, PB, tiles, tm_q, KvMaps{&TM.k16, &TM.k1, &TM.kn16, &TM.kn1});
     } else if (warp == 9) {
-        prefill_mma<D>(PA, PB, tiles);
+        prefill_mma<D, FUSED>(PA, PB, tiles);
     } else if (warp == 10) {
         prefill_producer<D, 1, FUSED>(PA, PB, tiles, tm_q, KvMaps{&TM.v16, &TM.v1, &TM.vn16, &TM.vn1});
     } else if (warp != 15) {
@@ -286,7 +295,8 @@ static cudaError_t launch_mixed_t(const PoolDesc& pool, const BatchDesc& b, cons
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, plan_kernel, b, pool.Hq, pool.Hkv, P, g_split_pages.load(std::memory_order_relaxed));
+    cudaError_t e = cudaLaunchKernelEx(&cfg, plan_kernel, b, pool.Hq, pool.Hkv, P, g_split_pages.load(std::memory_order_relaxed),
+                                       FUSED ? 1 : 0);  // row-pair items: only the variant with two softmax warpgroups reads them
     if (e != cudaSuccess) return e;
     ++*launches;
 

@@ -48,7 +48,8 @@ __host__ __device__ inline WorkspaceLayout make_layout(int Hq, int Hkv, int D, i
 struct PlanPtrs {
     int* hdr;
     int4* req_info;
-    int2* items;   // {req, (qtile << 16) | (pair << 15) | head}: pair = the item also carries head + 1 (same kv group)
+    int2* items;   // {req, (qtile << 16) | (two << 15) | (rows << 14) | head}: two = the item carries a second query tile:
+                   // head + 1 of the same kv group at the same rows (rows = 0), or the next 128 rows of the same head (rows = 1)
     int4* units;   // {req, kvh | (hb << 16), page_start, page_count}
     int* group_cnt;  // [n_units] zeroed here: finished units per split group (indexed by the group's first unit)
 };
@@ -107,7 +108,8 @@ __device__ __forceinline__ int plan_block_max(int v, int* s_warp) {
     return m;
 }
 
-__global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split) {
+__global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split,
+                                                            int row_pairs) {
     // the step kernel (a programmatic dependent of this one) may start its prologue now; it waits for this kernel's
     // completion before it reads the workspace
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -118,10 +120,17 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
     const int g = Hq / Hkv;
     const int HB = (g + kHeadBlock - 1) / kHeadBlock;
     const int n = b.num_reqs;
-    // prefill items per 128-row query tile: under GQA with an even group, two heads of a kv group share one item
-    // (and its K/V tiles in shared memory); otherwise one head per item
+    // Prefill items.  Under GQA with an even group an item carries two heads of a kv group at the same 128 rows (`pair`):
+    // they share every K/V tile in shared memory.  Otherwise (MHA, odd groups) an item is one head's tile -- or, with
+    // row_pairs (the step kernel variant with two softmax warpgroups, csrc/mixed.cu), two consecutive row tiles of the
+    // same head, paired from the top so that the lone tile of an odd count is the lightest one, tile 0.
     const int pair = (g % 2 == 0) ? 1 : 0;
+    const int rowp = (!pair && row_pairs) ? 1 : 0;
     const int ipt = pair ? Hq / 2 : Hq;
+    auto items_of = [&](int q) {
+        const int ntile = (q + kQTile - 1) / kQTile;
+        return (rowp ? (ntile + 1) / 2 : ntile) * ipt;
+    };
     const int chunk = (n + kPlanThreads - 1) / kPlanThreads;  // requests per thread (contiguous: prefix sums)
     const int i0 = tid * chunk, i1 = min(n, i0 + chunk);
 
@@ -158,7 +167,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
             const int pages = (__ldg(b.ctx_lens + i) + 1 + kPageSize - 1) / kPageSize;
             my_units += ((pages + split - 1) / split) * Hkv * HB;
         } else if (q > 1) {
-            my_items += ((q + kQTile - 1) / kQTile) * ipt;
+            my_items += items_of(q);
         }
     }
     int n_units, n_items;
@@ -174,7 +183,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
             ubase += info.z * Hkv * HB;
         } else if (q > 1) {
             info.x = 2;
-            ibase += ((q + kQTile - 1) / kQTile) * ipt;
+            ibase += items_of(q);
         }
         if (blockIdx.x == 0) P.req_info[i] = info;
         if (n <= kPlanStagedReqs) {  // every block keeps its own copy of the directory for the ticket search below
@@ -240,8 +249,14 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq,
         const int i = owner(s_ib, 3, e);
         const int local = e - (staged ? s_ib[i] : P.req_info[i].w);
         const int ntile = staged ? s_pg[i] : (b.q_lens[i] + kQTile - 1) / kQTile;
-        const int qt = ntile - 1 - local / ipt;  // heaviest (most KV tiles) first
-        P.items[e] = make_int2(i, (qt << 16) | (pair << 15) | ((local % ipt) << pair));
+        if (!rowp) {
+            const int qt = ntile - 1 - local / ipt;  // heaviest (most KV tiles) first
+            P.items[e] = make_int2(i, (qt << 16) | (pair << 15) | ((local % ipt) << pair));
+        } else {
+            const int hi = ntile - 1 - 2 * (local / ipt);  // tiles (hi - 1, hi), heaviest pair first; tile 0 alone if odd
+            const int two = hi >= 1 ? 1 : 0;
+            P.items[e] = make_int2(i, ((hi - two) << 16) | (two << 15) | (1 << 14) | (local % ipt));
+        }
     }
     // Programmatic dependent launch: this kernel may have started while the kernel before it on the stream (the
     // append, which triggers at its first instruction) was still running.  The step kernel behind this one reads what

@@ -79,40 +79,52 @@ struct KvMaps {
 };
 
 struct PrefillItem {
-    int req, qt, h, hk, nt;   // nt query tiles: heads h .. h + nt - 1 (same kv head hk)
+    int req, qt, h, hk, nt;   // nt query tiles.  rows == 0: heads h .. h + nt - 1 (same kv head hk) at row tile qt;
+    int rows;                 // rows == 1 (two-warpgroup variant only): row tiles qt .. qt + nt - 1 of head h
     int c, ql, tok0;          // context length, chunk length, first packed row of the request
-    int l_tile;               // keys visible to the last row of the tile: c + min(ql, (qt+1)*128)
-    int n_kt;                 // KV tiles
+    int l_tile;               // keys visible to the last row of the item's LAST tile: c + min(ql, (qt_last+1)*128)
+    int n_kt;                 // KV tiles of the last tile (the item's K/V extent)
+    int n_kt0;                // KV tiles of tile 0: n_kt, or one fewer when it is the earlier row tile of a pair
+    __device__ __forceinline__ int head(int w) const { return h + (rows ? 0 : w); }
+    __device__ __forceinline__ int row0(int w) const { return (qt + (rows ? w : 0)) * kQTile; }  // first row of tile w in the chunk
+    __device__ __forceinline__ int kv_tiles(int w) const { return w == 0 ? n_kt0 : n_kt; }
 };
 
+// ROWS = false (the plain step kernel): row-pair items do not occur, `rows` folds to 0 and n_kt0 to n_kt at compile time
+template <bool ROWS>
 __device__ __forceinline__ PrefillItem load_item(const PrefillArgs& A, int id) {
     PrefillItem it;
     const int2 v = A.items[id];
     it.req = v.x;
     it.qt = v.y >> 16;
     it.nt = ((v.y >> 15) & 1) + 1;
-    it.h = v.y & 0x7fff;
+    it.rows = ROWS ? (v.y >> 14) & 1 : 0;
+    it.h = v.y & 0x3fff;
     it.hk = it.h / (A.pool.Hq / A.pool.Hkv);
     it.c = __ldg(A.b.ctx_lens + it.req);
     it.ql = __ldg(A.b.q_lens + it.req);
     it.tok0 = __ldg(A.b.q_offsets + it.req);
-    it.l_tile = it.c + min(it.ql, (it.qt + 1) * kQTile);
+    const int qt_last = it.qt + (it.rows ? it.nt - 1 : 0);
+    it.l_tile = it.c + min(it.ql, (qt_last + 1) * kQTile);
     it.n_kt = (it.l_tile + kKvTile - 1) / kKvTile;
+    it.n_kt0 = ROWS ? (it.c + min(it.ql, (it.qt + 1) * kQTile) + kKvTile - 1) / kKvTile : it.n_kt;
     return it;
 }
 
 // the same item with every field broadcast from lane 0 (warp-uniform for the compiler: see uni())
+template <bool ROWS>
 __device__ __forceinline__ PrefillItem load_item_uniform(const PrefillArgs& A, int id) {
-    PrefillItem it = load_item(A, id);
+    PrefillItem it = load_item<ROWS>(A, id);
     it.req = uni(it.req); it.qt = uni(it.qt); it.h = uni(it.h); it.hk = uni(it.hk); it.nt = uni(it.nt);
     it.c = uni(it.c); it.ql = uni(it.ql); it.tok0 = uni(it.tok0); it.l_tile = uni(it.l_tile); it.n_kt = uni(it.n_kt);
+    if (ROWS) { it.rows = uni(it.rows); it.n_kt0 = uni(it.n_kt0); } else { it.n_kt0 = it.n_kt; }
     return it;
 }
 
-__device__ __forceinline__ void prefill_init_bars(PrefillBars* B) {
+__device__ __forceinline__ void prefill_init_bars(PrefillBars* B, int softmax_warps) {
     for (int i = 0; i < 2; ++i) {
         mbar_init(&B->item_full[i], 1);
-        mbar_init(&B->item_empty[i], 6);  // lane 0 of: MMA warp, V producer warp, each of the 4 softmax warps
+        mbar_init(&B->item_empty[i], 2 + softmax_warps);  // lane 0 of: MMA warp, V producer warp, each softmax warp
         mbar_init(&B->s_full[i], 1);
         mbar_init(&B->p_full[i], 128);
         mbar_init(&B->pv_done[i], 1);
@@ -202,7 +214,7 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
             if (lane == 0) mbar_arrive(&B->item_empty[ms]);
         }
         if (id >= n_items) break;
-        const PrefillItem it = load_item_uniform(A, id);
+        const PrefillItem it = load_item_uniform<FUSED>(A, id);
         const int* pt = A.b.page_table + (size_t)it.req * A.b.stride;
         if (KIND == 0) {
             mbar_wait(&B->q_empty, (item_it & 1) ^ 1, 102);
@@ -211,8 +223,8 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
                 for (int w = 0; w < it.nt; ++w)
 #pragma unroll
                     for (int cb = 0; cb < C::CB; ++cb)
-                        tma_load_3d(q_s + w * C::TILE_BYTES + cb * C::HALF_BYTES, tm_q, cb * 64, it.h + w,
-                                    it.tok0 + it.qt * kQTile, &B->q_full);
+                        tma_load_3d(q_s + w * C::TILE_BYTES + cb * C::HALF_BYTES, tm_q, cb * 64, it.head(w),
+                                    it.tok0 + it.row0(w), &B->q_full);
             }
         }
         const int n_pages = (it.l_tile + kPageSize - 1) / kPageSize;
@@ -230,7 +242,7 @@ __device__ __forceinline__ void prefill_producer(const PrefillArgs& A, PrefillBa
 // MMA warp.  All 32 lanes run the (warp-uniform) control flow; one elected lane issues the tcgen05 instructions.
 // Per KV tile kt and query tile w: PV_w(kt) as soon as P_w(kt) is posted, then S_w(kt+1) into the S slot PV_w(kt) has
 // just read -- so while warpgroup A exponentiates S_A(kt+1) the tensor pipe runs PV_B(kt) and S_B(kt+1).
-template <int D>
+template <int D, bool ROWS>
 __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B, uint8_t* tiles) {
     using C = PrefillCfg<D>;
     const int lane = threadIdx.x & 31;
@@ -274,7 +286,7 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
         __syncwarp();
         if (lane == 0) mbar_arrive(&B->item_empty[ms]);
         if (id >= n_items) break;
-        const PrefillItem it = load_item_uniform(A, id);
+        const PrefillItem it = load_item_uniform<ROWS>(A, id);
 
         mbar_wait(&B->q_full, item_it & 1, 106, item_it);
         mbar_wait(&B->kv_full[cur.slot], cur.phase, 104, item_it);  // K(0)
@@ -309,6 +321,7 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
             }
 #pragma unroll 1
             for (int w = 0; w < it.nt; ++w) {
+                if (ROWS && kt >= it.kv_tiles(w)) continue;  // the earlier row tile of a pair sees one KV tile fewer
                 const uint32_t gw = w ? g1 : g0;
                 if (kt == 0) mbar_wait(&B->o_empty[w], ((w ? cnt1 : cnt0) & 1) ^ 1, 108, item_it);  // previous epilogue has read O_w
                 mbar_wait(&B->p_full[w], gw & 1, 109, item_it * 100000 + kt * 1000 + it.n_kt);
@@ -321,8 +334,10 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
                     tc_commit(&B->pv_done[w]);
                 }
                 __syncwarp();
-                if (has_next) {
-                    if (w == 0) {
+                if (ROWS ? kt + 1 < it.kv_tiles(w) : has_next) {
+                    // K(kt+1): waited by the first tile that needs it (with row pairs tile 0 may not: a repeated wait on
+                    // a completed phase returns at once)
+                    if (ROWS || w == 0) {
                         mbar_wait(&B->kv_full[kcur.slot], kcur.phase, 104, item_it * 100000 + kt);
                         tc_fence_after();
                     }
@@ -348,8 +363,10 @@ __device__ __forceinline__ void prefill_mma(const PrefillArgs& A, PrefillBars* B
 // ------------------------------------------------------------------------------------------------
 // softmax warpgroup (4 warps, 128 threads: thread r <-> query row r <-> TMEM lane r, for both query tiles)
 __device__ __forceinline__ float max4(float a, float b, float c, float d) { return fmaxf(fmaxf(a, b), fmaxf(c, d)); }
-template <int D>
-__device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBars* B, int wg_warp) {
+// NWG = 1: one warpgroup alternates between the item's two query tiles.  NWG = 2 (the variant for prefill-dominated
+// steps): warpgroup `wg` owns tile wg -- two softmax warps per scheduler, so each hides the other's latencies.
+template <int D, bool ROWS, int NWG>
+__device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBars* B, int wg_warp, int wg) {
     using C = PrefillCfg<D>;
     const int lane = threadIdx.x & 31;
     const int r = wg_warp * 32 + lane;
@@ -366,16 +383,20 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
         __syncwarp();
         if (lane == 0) mbar_arrive(&B->item_empty[ms]);
         if (id >= n_items) break;
-        const PrefillItem it = load_item(A, id);
-        const int t = it.qt * kQTile + r;
-        const int limit = it.c + min(t, it.ql - 1);  // last visible key of this row (rows past the chunk mirror its last row)
+        const PrefillItem it = load_item<ROWS>(A, id);
+        // row of this thread in tile w: t0 + w * t_step; its last visible key: c + min(t, ql - 1) (rows past the chunk
+        // mirror its last row)
+        const int t0 = it.qt * kQTile + r, t_step = it.rows ? kQTile : 0;
+        const int w_begin = NWG == 2 ? wg : 0, w_end = NWG == 2 ? min(it.nt, wg + 1) : it.nt;
         // running maximum / sum of this row in query tile A and B; the first chunk raises m from -inf (grow_fix)
         float mA = -INFINITY, lA = 0.f, mB = -INFINITY, lB = 0.f;
 
         for (int kt = 0; kt < it.n_kt; ++kt) {
 #pragma unroll 1
-          for (int w = 0; w < it.nt; ++w) {  // the warpgroup alternates between the two query tiles: while it works on
-            // S_B(kt) the tensor pipe runs PV_A(kt) and S_A(kt+1)
+          for (int w = w_begin; w < w_end; ++w) {  // NWG = 1: the warpgroup alternates between the two query tiles: while
+            // it works on S_B(kt) the tensor pipe runs PV_A(kt) and S_A(kt+1)
+            if (ROWS && kt >= it.kv_tiles(w)) continue;  // the earlier row tile of a pair sees one KV tile fewer
+            const int limit = it.c + min(t0 + w * t_step, it.ql - 1);
             const uint32_t s_col = tm + C::TM_S + w * 128, o_col = tm + C::TM_O + w * 128;
             float m_used = w ? mB : mA, l = w ? lB : lA;
             const uint32_t g = (w ? gB : gA) + kt;
@@ -497,13 +518,14 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
         }
 
         // epilogue: out = O / l
-        const bool valid = t < it.ql;
 #pragma unroll 1
-        for (int w = 0; w < it.nt; ++w) {
+        for (int w = w_begin; w < w_end; ++w) {
+        const int t = t0 + w * t_step;
+        const bool valid = t < it.ql;
         const uint32_t o_col = tm + C::TM_O + w * 128;
         const float m_used = w ? mB : mA, l = w ? lB : lA;
-        const int head = it.h + w;
-        mbar_wait(&B->pv_done[w], ((w ? gB : gA) + it.n_kt - 1) & 1, 113, item_it * 100000 + id);
+        const int head = it.head(w);
+        mbar_wait(&B->pv_done[w], ((w ? gB : gA) + it.kv_tiles(w) - 1) & 1, 113, item_it * 100000 + id);
         tc_fence_after();
         const float inv = 1.f / l;
         uint16_t* orow = A.out + ((size_t)(it.tok0 + t) * A.pool.Hq + head) * D;
@@ -529,7 +551,7 @@ __device__ __forceinline__ void prefill_softmax(const PrefillArgs& A, PrefillBar
         if (valid && A.lse != nullptr)
             A.lse[(size_t)(it.tok0 + t) * A.pool.Hq + head] = (m_used + log2f(l)) * 0.6931471805599453f;
         }
-        gA += it.n_kt;
+        gA += it.n_kt0;
         if (it.nt > 1) gB += it.n_kt;
         ++item_it;
     }
