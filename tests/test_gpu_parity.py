@@ -312,16 +312,20 @@ def test_poison_pool_outputs_finite_and_pool_untouched_elsewhere():
     assert changed_rows.sum() == s.total_q * s.num_kv_heads  # exactly the appended rows changed
 
 
-def test_run_to_run_deterministic():
+@pytest.mark.parametrize("impl", ["fused", "product"])
+def test_run_to_run_deterministic(impl):
     s = _step(13, 8, 2, 128, [300, 1, 1, 1], [0, 2000, 5000, 64])
     dev = DeviceStep(s)
-    dev.step()
+    dev.step(impl=impl)
     a = bits(dev.out).copy()
     for _ in range(3):
         dev.out.zero_()
-        dev.attention()
-        torch.cuda.synchronize()
+        dev.step(impl=impl)
         assert np.array_equal(bits(dev.out), a)
+    dev.out.zero_()
+    dev.attention()     # the plain variant on the pool the step has left: the same bits as either variant
+    torch.cuda.synchronize()
+    assert np.array_equal(bits(dev.out), a)
 
 
 def test_product_path_matches_simt_cross_check():
