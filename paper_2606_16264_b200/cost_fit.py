@@ -272,7 +272,17 @@ A_MIN_US_PER_FLOP = 1e6 / 2250e12
 B_MIN_US_PER_BYTE = 1e6 / 8000e9
 
 
-def fit_shape(rows):
+FUSED_MIN_TOKENS_PER_REQ = 64   # tropical_mixed_step's choice of kernel variant (csrc/mixed.cu, csrc/step_cost.cpp)
+
+
+def is_fused_step(row) -> bool:
+    q, _ = grid_lengths(row["prefill_tokens"], row["prefill_ctx"], row["n_decode"], row["ctx_median"], row["seed"])
+    return int(q.sum()) >= FUSED_MIN_TOKENS_PER_REQ * len(q)
+
+
+def fit_shape(rows, base=None):
+    """Six coefficients by bounded least squares on relative error.  base = the plain variant's coefficients: then only
+    t0, a and e_p are fitted (a fused-variant step has few decode requests: too few points to identify the rest)."""
     from scipy.optimize import least_squares
     X = np.array([point_features(r) for r in rows])
     y = np.array([r["us_median"] for r in rows])
@@ -281,14 +291,24 @@ def fit_shape(rows):
     scale = np.array([10.0, 1e-9, 1e-7, 1.0, 1.0, 0.01])   # parameter magnitudes (us, us/FLOP, us/byte, -, us, us)
     lo = np.array([0, A_MIN_US_PER_FLOP / scale[1], B_MIN_US_PER_BYTE / scale[2], 0, 0, 0])
     hi = np.array([20, 50, 50, 1, 50, 500])
+    free = np.ones(6, bool)
+    if base is not None:
+        free = np.array([True, True, False, False, True, False])
+    fixed = (np.asarray(base) / scale) if base is not None else np.zeros(6)
+
+    def full(xf):
+        x = fixed.copy()
+        x[free] = xf
+        return x * scale
+
     res_best = None
     for k0 in (0.1, 0.5, 0.9):
-        x0 = np.array([1.0, 1.5, 1.6, k0, 0.5, 1.0])
-        fun = lambda x: (predict(x * scale, X[train]) - y[train]) / y[train]
-        res = least_squares(fun, x0, bounds=(lo, hi))
+        x0 = np.array([1.0, 1.5, 1.6, k0, 0.5, 1.0])[free]
+        fun = lambda xf: (predict(full(xf), X[train]) - y[train]) / y[train]
+        res = least_squares(fun, x0, bounds=(lo[free], hi[free]))
         if res_best is None or res.cost < res_best.cost:
             res_best = res
-    theta = res_best.x * scale
+    theta = full(res_best.x)
     rel = np.abs(predict(theta, X) - y) / y
     stats = dict(n=len(rows), n_train=int(train.sum()), mape_train=float(rel[train].mean()),
                  mape_held=float(rel[~train].mean()), max_held=float(rel[~train].max()), max_all=float(rel.max()),
@@ -342,15 +362,21 @@ def fit(grid_path: str, write: bool, gemm_path: str = None):
     rows = read_grid(grid_path)
     shapes = sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows})
     lines = ["// Generated by `python -m paper_2606_16264_b200.cost_fit fit` from calibration/b200_grid.csv.",
-             "// {Hq, Hkv, d, {t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us, n_sm}}",
+             "// {Hq, Hkv, d, fused, {t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us, n_sm}}",
+             "// fused = 1: steps tropical_mixed_step runs through its fused kernel variant (>= 64 new tokens per request).",
              "// a >= 1 / (2250 TFLOP/s) and b >= 1 / (8 TB/s) are enforced by the fit (nominal peaks of the part)."]
     for s in shapes:
-        theta, st = fit_shape([r for r in rows if (r["Hq"], r["Hkv"], r["d"]) == s])
-        print(f"shape {s}: theta={['%.4g' % t for t in theta]} {st}")
-        lines.append("{%d, %d, %d, {%.6g, %.6g, %.6g, %.6g, %.6g, %.6g, 148}},  // held-out MAPE %.1f %%, max %.1f %%; "
-                     "off-grid MAPE %.1f %%, max %.1f %%"
-                     % (*s, *theta, 100 * st["mape_held"], 100 * st["max_held"], 100 * st["mape_off_grid"],
-                        100 * st["max_off_grid"]))
+        of_shape = [r for r in rows if (r["Hq"], r["Hkv"], r["d"]) == s]
+        plain = [r for r in of_shape if not is_fused_step(r)]
+        fused = [r for r in of_shape if is_fused_step(r)]
+        theta, st = fit_shape(plain)
+        theta_f, st_f = fit_shape(fused, base=theta)
+        for tag, th, stt in ((0, theta, st), (1, theta_f, st_f)):
+            print(f"shape {s} fused={tag}: theta={['%.4g' % t for t in th]} {stt}")
+            lines.append("{%d, %d, %d, %d, {%.6g, %.6g, %.6g, %.6g, %.6g, %.6g, 148}},  // %d points; held-out MAPE %.1f %%, "
+                         "max %.1f %%; off-grid MAPE %.1f %%, max %.1f %%"
+                         % (*s, tag, *th, stt["n"], 100 * stt["mape_held"], 100 * stt["max_held"],
+                            100 * stt["mape_off_grid"], 100 * stt["max_off_grid"]))
     gemm_path = gemm_path or GEMM_GRID
     theta_l, st_l = fit_linear(read_gemm(gemm_path))
     print(f"linear layers: theta={['%.4g' % t for t in theta_l]} {st_l}")

@@ -9,15 +9,19 @@
 
 namespace {
 
+// One coefficient set per head shape and kernel variant of the step: tropical_mixed_step runs prefill-dominated steps
+// (at least kFusedMinTokensPerReq new tokens per request on average, csrc/mixed.cu) through its fused variant -- append
+// inside, two softmax warpgroups -- whose prefill role is up to 35 % faster; one closed form cannot follow that switch.
 struct BuiltinFit {
-    int Hq, Hkv, d;
+    int Hq, Hkv, d, fused;
     tropical_cost_model_t m;
 };
+constexpr int kFusedMinTokensPerReq = 64;  // must equal csrc/mixed.cu's
 
 // Coefficients fitted to measured step times by `python -m paper_2606_16264_b200.cost_fit fit` from the grid
 // that `... cost_fit measure` wrote on a B200 (calibration/b200_grid.csv; provenance in DESIGN.md section 7).
 const BuiltinFit kBuiltin[] = {
-    {0, 0, 0, {0, 0, 0, 0, 0, 0, 148}},  // sentinel: never matches
+    {0, 0, 0, 0, {0, 0, 0, 0, 0, 0, 148}},  // sentinel: never matches
 #include "cost_model_fit.inc"
 };
 
@@ -71,8 +75,11 @@ extern "C" int tropical_step_cost(const tropical_cost_model_t* model, int32_t Hq
     tropical_cost_breakdown_t f;
     features(Hq, Hkv, d, P, num_reqs, q_lens, ctx_lens, &f);
     if (model == nullptr) {
+        long long T = 0;
+        for (int i = 0; i < num_reqs; ++i) T += q_lens[i];
+        const int fused = (num_reqs > 0 && T >= (long long)kFusedMinTokensPerReq * num_reqs) ? 1 : 0;
         for (const BuiltinFit& b : kBuiltin)
-            if (b.Hq == Hq && b.Hkv == Hkv && b.d == d) model = &b.m;
+            if (b.Hq == Hq && b.Hkv == Hkv && b.d == d && b.fused == fused) model = &b.m;
     }
     if (model != nullptr) {
         f.t_tc_us = model->a_us_per_flop * f.flops;

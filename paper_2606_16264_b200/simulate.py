@@ -28,9 +28,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 
 def builtin_model(Hq: int, Hkv: int, d: int) -> tb.CostModel:
     text = open(os.path.join(HERE, "csrc", "cost_model_fit.inc")).read()
-    for m in re.finditer(r"\{(\d+), (\d+), (\d+), \{([^}]*)\}\}", text):
-        if (int(m.group(1)), int(m.group(2)), int(m.group(3))) == (Hq, Hkv, d):
-            return tb.CostModel(*[float(x) for x in m.group(4).split(",")])
+    for m in re.finditer(r"\{(\d+), (\d+), (\d+), (\d+), \{([^}]*)\}\}", text):   # the plain variant's set (fused = 0)
+        if (int(m.group(1)), int(m.group(2)), int(m.group(3)), int(m.group(4))) == (Hq, Hkv, d, 0):
+            return tb.CostModel(*[float(x) for x in m.group(5).split(",")])
     raise KeyError(f"no fitted coefficients for {Hq}/{Hkv}/{d}")
 
 
