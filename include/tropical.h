@@ -145,14 +145,21 @@ int tropical_mixed_attention(const tropical_kv_pool_t *pool, const tropical_batc
                              const void *q, void *out, float *lse, float sm_scale,
                              void *workspace, size_t workspace_bytes, void *cuda_stream);
 
-/* One multiplexed iteration in ONE call -- rows A0-A5 with the KV append (A1) fused in: the same results as
- * tropical_kv_append followed by tropical_mixed_attention (pool bit-identical afterwards, out / lse identical to that
- * pair's), in two launches instead of three and with the append off the critical path.  The attention roles read this
- * step's K / V rows directly from k_new / v_new (TMA boxes over [T][Hkv][d]; a decode request's own new row is patched
- * into the page-head it has just loaded) while otherwise idle warps of the same persistent kernel copy the rows into
- * their (page, slot) of the pool; nothing reads those slots from the pool during the step.
+/* One multiplexed iteration in ONE call -- rows A0-A5 with the KV append (A1) included: the same results as
+ * tropical_kv_append followed by tropical_mixed_attention (pool bit-identical afterwards, out / lse bit-identical to that
+ * pair's).  The library chooses how from the host scalars of the batch:
+ *   - prefill-dominated steps (total_q >= 64 * num_reqs, i.e. at most one decode request per ~64 prefill tokens): the
+ *     FUSED variant of the step kernel, two launches.  Its attention roles read this step's K / V rows directly from
+ *     k_new / v_new (TMA boxes over [T][Hkv][d]; a decode request's own new row is patched into the page-head it has just
+ *     loaded) while otherwise idle warps of the same persistent kernel copy the rows into their (page, slot) of the pool
+ *     -- the append leaves the critical path; nothing reads those slots from the pool during the step.  Since such steps
+ *     leave the decode warps idle, the variant runs two softmax warpgroups and pairs MHA query tiles by rows.
+ *   - other (decode-heavy) steps: the append kernel in front of the plain step kernel, three launches, exactly what the
+ *     two separate calls enqueue (the fused variant's extra work in the decode loop costs more there than it saves).
  *   k_new, v_new [device] bf16 [T][Hkv][d], 16-byte aligned; every other argument as in tropical_mixed_attention.
- * The pool IS written (exactly the rows tropical_kv_append would write).  Idempotent, graph-capturable. */
+ * The pool IS written (exactly the rows tropical_kv_append would write).  Idempotent, graph-capturable.  A preceding
+ * kernel on the stream must have completed its writes of the batch metadata, k_new and v_new before it triggers
+ * programmatic dependents, if it does (see tropical_mixed_attention). */
 int tropical_mixed_step(const tropical_kv_pool_t *pool, const tropical_batch_t *batch, const void *q,
                         const void *k_new, const void *v_new, void *out, float *lse, float sm_scale,
                         void *workspace, size_t workspace_bytes, void *cuda_stream);
