@@ -194,6 +194,16 @@ def make_workload(name: str, rank: int, part: str = "all"):
     return s, time.perf_counter() - t0
 
 
+def config_dict(name, part, cnt, world):
+    """The line's `config`: the workload and how the L2 is kept out of the timing -- the same dict in both arms."""
+    flush = cnt["step_bytes"] < 5e8
+    return {"workload": f"{name} ({describe(name)})" + ("" if part == "all" else f", its {part} requests only (analysis run)"),
+            "replicas": world,
+            "l2": ("step touches %.2f GB >> 126 MB L2, no flush needed" % (cnt["step_bytes"] / 1e9)) if not flush else
+                  "L2 flushed (512 MB rewritten, untimed) between timed steps; per-step event times summed",
+            "new_tokens_per_step": int(cnt["new_tokens"])}
+
+
 def describe(name):
     return {"C1": "tiny mixed 4/4/64", "C2": "decode-only 32/32/128 x64", "C3": "prefill-only 32/32/128 x4",
             "C4": "mixed 13B-like 40/40/128: 2048 chunk + 128 decodes",
@@ -494,16 +504,12 @@ def run_ours(args, rank, world):
         "metric": METRIC, "value": round(us, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": warm, "ms_per_step": round(ms_per_step, 5), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{args.config} ({describe(args.config)})" +
-                               ("" if args.part == "all" else f", its {args.part} requests only (analysis run)"), "replicas": world,
-                   "l2": "step touches %.2f GB >> 126 MB L2, no flush needed" % (cnt["step_bytes"] / 1e9)
-                   if not st.flush else "L2 flushed (512 MB rewritten, untimed) between timed steps; per-step event times summed",
-                   "new_tokens_per_step": int(cnt["new_tokens"]),
-                   "step": ("tropical_kv_append + tropical_mixed_attention (3 launches)" if args.two_call else
-                            "tropical_mixed_step: one call; " +
-                            ("its fused kernel variant, KV append inside the step kernel (2 launches)"
-                             if st.launches_per_step == 2 else
-                             "decode-heavy step: its append kernel in front of the plain step kernel (3 launches)"))},
+        "config": config_dict(args.config, args.part, cnt, world),
+        "step_call": ("tropical_kv_append + tropical_mixed_attention (3 launches)" if args.two_call else
+                      "tropical_mixed_step: one call; " +
+                      ("its fused kernel variant, KV append inside the step kernel (2 launches)"
+                       if st.launches_per_step == 2 else
+                       "decode-heavy step: its append kernel in front of the plain step kernel (3 launches)")),
         "tokens_per_s": round(whole_job_tokens_per_s(cnt["new_tokens"], world, us), 1),
         "us_per_step": {"mean_timed_region": round(us, 2), "median": round(float(np.median(step_us)), 2),
                         "min": round(float(step_us.min()), 2), "max": round(float(step_us.max()), 2),
@@ -661,7 +667,8 @@ def run_reference(args, rank, world):
         "impl": "reference", "metric": METRIC, "value": round(us, 1), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(us / 1e3, 3), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{cfg} ({describe(cfg)})"},
+        "config": config_dict(cfg, "all", step_counts((s.num_q_heads, s.num_kv_heads, s.head_dim, s.page_size, s.q_lens,
+                                                          s.ctx_lens)), world),
         "cpu_baseline": {"value": round(us, 1), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": round(us, 1), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
