@@ -101,7 +101,9 @@ def main(argv=None):
             cols.append(s)
         c, d, m = cols
         print(f"{rate:7.2f} | {c.attainment:11.3f} {c.ttft_p90_us / 1e3:12.1f} | {d.attainment:10.3f} {d.ttft_p90_us / 1e3:12.1f} | "
-              f"{m.attainment:10.3f} {m.ttft_p90_us / 1e3:12.1f} {m.multiplexed_prefills:11d}")
+              f"{m.attainment:10.3f} {m.ttft_p90_us / 1e3:12.1f} {m.multiplexed_prefills:11d}" +
+              (f"   role transitions: {m.to_multiplexing} to multiplexing, {m.to_prefill} to prefill" if a.role_transitions else ""))
+    return 0
 
 
 if __name__ == "__main__":

@@ -387,3 +387,18 @@ def test_sim_argument_validation():
         tb.sim_run(bad, [(0.0, 10, 2)])
     res, summ = tb.sim_run(good, [])
     assert res == [] and summ.iterations == 0
+
+
+def test_simulate_driver_runs_on_the_builtin_fits(capsys):
+    """python -m paper_2606_16264_b200.simulate: the three styles on a synthetic trace with iteration times from
+    tropical_iter_cost and the compiled-in B200 fits (TP = 2 shard, role transitions on): runs, and every attainment is a
+    fraction."""
+    from paper_2606_16264_b200 import simulate
+    assert simulate.main(["--requests", "60", "--rates", "8,24", "--tp", "2", "--role-transitions"]) == 0
+    lines = [l for l in capsys.readouterr().out.splitlines() if "|" in l and l.lstrip()[0].isdigit()]
+    assert len(lines) == 2
+    for l in lines:
+        cols = [c.split() for c in l.split("|")]
+        for att in (cols[1][0], cols[2][0], cols[3][0]):
+            assert 0.0 <= float(att) <= 1.0
+    assert simulate.migrate_us_per_token(40, 128, 40, 900.0) == pytest.approx(40 * 4 * 40 * 128 / 900e3)   # the link is the slower hop
