@@ -488,6 +488,13 @@ def test_more_requests_than_plan_threads():
     _check_step(_step(78, 2, 2, 64, qs, cs))
 
 
+def test_long_contexts():
+    """Contexts far beyond the configs' 8192 tokens: a decode request on 70 001 cached tokens (4376 pages: 137 split-K
+    units per kv head under the automatic split) and a 300-token chunk on 66 000 (517 KV tiles per query tile), next to a
+    short request; both step variants."""
+    _check_step(_step(23, 4, 2, 128, [1, 300, 1], [70001, 66000, 5]))
+
+
 def test_validate_batch_finds_the_first_bad_request():
     s = _step(19, 4, 2, 64, [40, 1, 1, 0, 5], [3, 100, 17, 9, 0])
     dev = DeviceStep(s)
