@@ -307,9 +307,9 @@ class StepTimer:
             buf.fill_(k & 0xff)             # the step's launches are queued behind it (no host launch latency inside)
             self.one_step()
             t = tb.debug_timeline()
-            rows.append([t[f] / 1e3 for f in tb.TIMELINE_FIELDS])
-        med = np.median(np.array(rows), axis=0)
-        return {f: round(float(v), 1) for f, v in zip(tb.TIMELINE_FIELDS, med)}
+            rows.append([t.get(f, float("nan")) / 1e3 for f in tb.TIMELINE_FIELDS])
+        med = np.nanmedian(np.array(rows), axis=0)
+        return {f: round(float(v), 1) for f, v in zip(tb.TIMELINE_FIELDS, med) if v == v}   # no append stamps on a fused step
 
     def sustained(self, seconds, local):
         """The step back to back for >= `seconds`: what a long-running worker sees once the power management has

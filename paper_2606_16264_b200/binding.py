@@ -188,8 +188,12 @@ def debug_timeline(reset: bool = False):
     _check(rc, "tropical_debug_timeline")
     if reset:
         return {}
-    t0 = int(out[0])
-    return {k: int(out[i]) - t0 for i, k in enumerate(TIMELINE_FIELDS)}
+    # relative to the first kernel of the step: the append's start, or -- when the step has no append kernel (the fused
+    # variant of tropical_mixed_step) -- the tile directory's; stamps that were never written stay out
+    unset = (0, 2 ** 64 - 1)
+    vals = {k: int(out[i]) for i, k in enumerate(TIMELINE_FIELDS) if int(out[i]) not in unset}
+    t0 = vals.get("append_start", vals.get("plan_start", 0))
+    return {k: v - t0 for k, v in vals.items()}
 
 
 def last_launch_count() -> int:
