@@ -76,6 +76,46 @@ def kv_append(k_pool, v_pool, q_lens, ctx_lens, q_offsets, page_table, k_new, v_
         _p(k_pool), _p(v_pool), _p(k_new), _p(v_new))
 
 
+def _f32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def rope_rotate(rows, pos, cos, sin) -> np.ndarray:
+    """fp64 rotate-half RoPE of bf16 rows [n, d] at positions pos [n] with tables cos, sin [table_len, d/2] (fp32 values);
+    unrounded (tropical_oracle.c: oracle_rope_rotate)."""
+    rows, cos, sin = _u16(rows), _f32(cos), _f32(sin)
+    n, d = rows.shape
+    assert cos.shape == sin.shape and cos.shape[1] == d // 2
+    pos = _i32(pos)
+    assert pos.shape == (n,) and (n == 0 or (0 <= pos.min() and pos.max() < cos.shape[0]))
+    out = np.empty((n, d), np.float64)
+    _load().oracle_rope_rotate(ctypes.c_int(d), ctypes.c_int64(n), _p(rows), _p(pos), _p(cos), _p(sin), _p(out))
+    return out
+
+
+def double_to_bf16(values) -> np.ndarray:
+    """fp64 -> bf16 bit patterns, round to nearest even straight from the double (oracle_double_to_bf16)."""
+    lib = _load()
+    lib.oracle_double_to_bf16.restype = ctypes.c_uint16
+    v = np.ascontiguousarray(values, np.float64)
+    return np.array([lib.oracle_double_to_bf16(ctypes.c_double(float(x))) for x in v.ravel()], np.uint16).reshape(v.shape)
+
+
+def kv_append_rope(k_pool, v_pool, q_lens, ctx_lens, q_offsets, page_table, k_new, v_new, cos, sin) -> None:
+    """In-place append with rotate-half RoPE applied to the K rows (oracle_kv_append_rope); V rows are copied."""
+    k_pool, v_pool, k_new, v_new = _u16(k_pool), _u16(v_pool), _u16(k_new), _u16(v_new)
+    assert k_pool.flags.writeable and v_pool.flags.writeable
+    _, Hkv, P, d = k_pool.shape
+    cos, sin = _f32(cos), _f32(sin)
+    q_lens, ctx_lens, q_offsets, page_table = _i32(q_lens), _i32(ctx_lens), _i32(q_offsets), _i32(page_table)
+    need = int((q_lens.astype(np.int64) + ctx_lens).max()) if q_lens.size else 0
+    assert cos.shape == sin.shape and cos.shape[1] == d // 2 and cos.shape[0] >= need
+    _load().oracle_kv_append_rope(
+        ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(P), ctypes.c_int(q_lens.shape[0]),
+        _p(q_lens), _p(ctx_lens), _p(q_offsets), _p(page_table), ctypes.c_int(page_table.shape[1]),
+        _p(k_pool), _p(v_pool), _p(k_new), _p(v_new), _p(cos), _p(sin))
+
+
 def kv_gather(k_pool, v_pool, page_table, req: int, n_keys: int) -> Tuple[np.ndarray, np.ndarray]:
     """Dense bf16 copy-out [n_keys, Hkv, d] of request req's first n_keys keys/values."""
     k_pool, v_pool = _u16(k_pool), _u16(v_pool)

@@ -19,8 +19,9 @@
  * Pins (tests/test_oracle_pins.py): brute-force dense attention, torch fp64 SDPA, closed
  * forms, row-sum-to-one, page-size and page-permutation invariance, chunk/decode
  * consistency, needle selection; kv_migrate: gather(dst) == gather(src) by fancy indexing, changed-row
- * count, attention unchanged by the move.  Step-cost model: not in this file (parity unpinned, see
- * DESIGN.md).
+ * count, attention unchanged by the move; RoPE append: identity table == plain append, quarter-turn table == swap
+ * and negate, norm and relative-position invariants, position indexing, rounding against ties worked by hand.
+ * Step-cost model: not in this file (parity unpinned).
  *
  * Layouts (host pointers, bf16 carried as uint16 bit patterns):
  *   q            [T][Hq][d]           k_new, v_new [T][Hkv][d]
@@ -125,6 +126,77 @@ void oracle_kv_migrate(int Hkv, int d, int P, int num_reqs, const int32_t *kv_le
             }
         }
     }
+}
+
+/* SURVEY 8(f) NEXT-4 "fuse RoPE+append": rotary position embedding of this step's K rows on their way into the pool.
+ * The paper says nothing about positional encoding (its substrate's models use it); the definition taken
+ * is the "rotate-half" convention of that model family [DESIGN.md reading R-rope]: channel c < d/2 is paired with
+ * channel c + d/2, the token at position pos = c_i + t uses row pos of the caller's tables cos, sin [table_len][d/2]:
+ *     k'[c]       = k[c] * cos[pos][c] - k[c + d/2] * sin[pos][c]
+ *     k'[c + d/2] = k[c + d/2] * cos[pos][c] + k[c] * sin[pos][c]
+ * The products of a bf16 value (8 significant bits) and an fp32 value (24) are exact in fp64 and so is their sum
+ * unless the exponents are far apart, so out[] below is the real-number result to fp64 accuracy. */
+void oracle_rope_rotate(int d, int64_t n_rows, const uint16_t *rows, const int32_t *pos, const float *cos_t,
+                        const float *sin_t, double *out)
+{
+    const int half = d / 2;
+    for (int64_t r = 0; r < n_rows; ++r) {
+        for (int c = 0; c < half; ++c) {
+            double x = bf16_to_double(rows[r * d + c]), y = bf16_to_double(rows[r * d + c + half]);
+            double cs = (double)cos_t[(int64_t)pos[r] * half + c], sn = (double)sin_t[(int64_t)pos[r] * half + c];
+            out[r * d + c] = x * cs - y * sn;
+            out[r * d + c + half] = y * cs + x * sn;
+        }
+    }
+}
+
+/* fp64 -> bf16, round to nearest even, straight from the double (no intermediate fp32 rounding).  Finite inputs
+ * within the bf16 normal range, +-0 and values that round to +-0 / subnormals are flushed by magnitude < 2^-126 -> 0
+ * (the rotated N(0,1) data of the tests never get there); NaN / inf pass through as the bf16 patterns. */
+uint16_t oracle_double_to_bf16(double v)
+{
+    uint64_t u;
+    memcpy(&u, &v, sizeof u);
+    uint16_t sign = (uint16_t)((u >> 63) << 15);
+    int64_t e = (int64_t)((u >> 52) & 0x7ff);
+    uint64_t m = u & 0xfffffffffffffULL;
+    if (e == 0x7ff) return (uint16_t)(sign | 0x7f80 | (m ? 0x40 : 0));
+    int64_t eb = e - 1023 + 127;                  /* bf16 / fp32 biased exponent */
+    if (e == 0 || eb <= 0) return sign;           /* zero, fp64 subnormal, or below the bf16 normal range */
+    uint64_t keep = m >> 45;                      /* top 7 mantissa bits */
+    uint64_t rest = m & ((1ULL << 45) - 1), half = 1ULL << 44;
+    if (rest > half || (rest == half && (keep & 1))) ++keep;
+    if (keep == 128) { keep = 0; ++eb; }
+    if (eb >= 255) return (uint16_t)(sign | 0x7f80);
+    return (uint16_t)(sign | (uint16_t)(eb << 7) | (uint16_t)keep);
+}
+
+/* Append with RoPE on K: the row that oracle_kv_append would copy is rotated (oracle_rope_rotate), rounded to bf16
+ * (oracle_double_to_bf16) and stored; V rows are copied.  Row by row, in the paper-free definition's order. */
+void oracle_kv_append_rope(int Hkv, int d, int P, int num_reqs, const int32_t *q_lens,
+                           const int32_t *ctx_lens, const int32_t *q_offsets,
+                           const int32_t *page_table, int stride, uint16_t *k_pool, uint16_t *v_pool,
+                           const uint16_t *k_new, const uint16_t *v_new, const float *cos_t, const float *sin_t)
+{
+    double *rot = (double *)malloc(sizeof(double) * (size_t)d);
+    for (int i = 0; i < num_reqs; ++i) {
+        for (int t = 0; t < q_lens[i]; ++t) {
+            int64_t pos = (int64_t)ctx_lens[i] + t;
+            int32_t pos32 = (int32_t)pos;
+            int64_t page = page_table[(int64_t)i * stride + pos / P];
+            int64_t slot = pos % P;
+            for (int h = 0; h < Hkv; ++h) {
+                int64_t dst = ((page * Hkv + h) * P + slot) * d;
+                int64_t src = (((int64_t)q_offsets[i] + t) * Hkv + h) * d;
+                oracle_rope_rotate(d, 1, k_new + src, &pos32, cos_t, sin_t, rot);
+                for (int c = 0; c < d; ++c) {
+                    k_pool[dst + c] = oracle_double_to_bf16(rot[c]);
+                    v_pool[dst + c] = v_new[src + c];
+                }
+            }
+        }
+    }
+    free(rot);
 }
 
 /* One (request i, new-token t, q-head hq) row of phase 2 (rows A3/A4/A5 all compute this):

@@ -18,6 +18,7 @@ from .workloads import (  # noqa: F401
     f32_to_bf16_bits,
     make_config,
     make_migration_target,
+    make_rope_tables,
     make_step,
     needed_pages,
 )

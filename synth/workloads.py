@@ -261,3 +261,14 @@ def make_migration_target(rng, kv_lens: Sequence[int], page_size: int, *, num_pa
         table[m, :k] = perm[used:used + k]
         used += k
     return table, int(num_pages)
+
+
+# ----------------------------------------------------------------------------- RoPE tables
+def make_rope_tables(table_len: int, head_dim: int, base: float = 10000.0):
+    """The caller-side INPUT of a RoPE-fused append: cos / sin tables fp32 [table_len, head_dim / 2] of the angles
+    pos * base^(-2 c / head_dim), evaluated in float64 and rounded to fp32 once.  Input generation only: the rotation
+    itself is the library's (and, independently, the oracle's)."""
+    pos = np.arange(table_len, dtype=np.float64)[:, None]
+    freq = base ** (-2.0 * np.arange(head_dim // 2, dtype=np.float64) / head_dim)[None, :]
+    ang = pos * freq
+    return np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32)

@@ -357,3 +357,110 @@ def test_O8_needle_selects_exactly_one_key():
     qf = code(c + t + 1)[None, None, :]
     o, _ = oracle.attention_rows(kp, vp, f32_to_bf16_bits(np.concatenate([qv[:t], qf, qv[t + 1:]])), [ql], [c], [0, ql], pt, [(0, t)])
     assert not np.array_equal(o[0, 0], vb[c + t + 1, 0])
+
+
+# ------------------------------------------------------------------ NEXT-4: RoPE fused into the append (oracle pins)
+def _rope_case(seed=50, Hq=4, Hkv=2, d=64, q_lens=(37, 1, 1), ctx_lens=(5, 100, 31)):
+    s = _small_step(seed, Hq, Hkv, d, list(q_lens), list(ctx_lens))
+    cos, sin = synth.make_rope_tables(int((np.asarray(q_lens) + np.asarray(ctx_lens)).max()), d)
+    return s, cos, sin
+
+
+def test_rope_rounding_helper_by_hand_and_against_the_fp32_route():
+    """oracle_double_to_bf16: ties to even and the cases where rounding through fp32 first would go wrong.
+    1 + 2^-8 is a tie -> even (1.0 = 0x3F80); 1 + 2^-8 + 2^-40 is above the tie -> 0x3F81 (fp32 would have dropped the
+    2^-40 and tied down); 1 + 3 * 2^-8 is a tie between odd and even -> even 0x3F82; -2.5 = 0xC020."""
+    got = oracle.double_to_bf16([1.0, 1 + 2.0 ** -8, 1 + 2.0 ** -8 + 2.0 ** -40, 1 + 3 * 2.0 ** -8, -2.5, 0.0])
+    assert got.tolist() == [0x3F80, 0x3F80, 0x3F81, 0x3F82, 0xC020, 0x0000]
+    # values that ARE fp32 numbers: the independent numpy fp32 -> bf16 rounding of synth must agree bit for bit
+    x = np.random.default_rng(0).standard_normal(4000).astype(np.float32)
+    assert np.array_equal(oracle.double_to_bf16(x.astype(np.float64)), f32_to_bf16_bits(x))
+
+
+def test_rope_identity_table_is_the_plain_append():
+    s, cos, sin = _rope_case()
+    kp0, vp0 = s.copy_pools()
+    oracle.kv_append(kp0, vp0, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new)
+    kp, vp = s.copy_pools()
+    oracle.kv_append_rope(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new,
+                          np.ones_like(cos), np.zeros_like(sin))
+    assert np.array_equal(kp, kp0) and np.array_equal(vp, vp0)
+
+
+def test_rope_quarter_turn_swaps_and_negates_and_v_is_copied():
+    """cos = 0, sin = 1: k'[c] = -k[c + d/2], k'[c + d/2] = k[c], exactly (sign flip and swap of bf16 patterns): pins
+    the pairing (c, c + d/2) -- an interleaved (2c, 2c + 1) convention fails -- and both signs."""
+    s, cos, sin = _rope_case()
+    kp, vp = s.copy_pools()
+    oracle.kv_append_rope(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new,
+                          np.zeros_like(cos), np.ones_like(sin))
+    half = s.head_dim // 2
+    for i in range(s.num_reqs):
+        for t in range(int(s.q_lens[i])):
+            pos = int(s.ctx_lens[i]) + t
+            row = kp[s.page_table[i, pos // 16], :, pos % 16, :]
+            src = s.k_new[int(s.q_offsets[i]) + t]
+            assert np.array_equal(row[:, :half], src[:, half:] ^ np.uint16(0x8000))
+            assert np.array_equal(row[:, half:], src[:, :half])
+            assert np.array_equal(vp[s.page_table[i, pos // 16], :, pos % 16, :], s.v_new[int(s.q_offsets[i]) + t])
+
+
+def test_rope_uses_the_table_row_of_the_tokens_position():
+    """Only table row p* is a quarter turn, every other row the identity: exactly the token at position c_i + t == p* of
+    each request is rotated."""
+    s, cos, sin = _rope_case(q_lens=(37, 1, 1), ctx_lens=(5, 20, 31))
+    p_star = 20
+    c2, s2 = np.ones_like(cos), np.zeros_like(sin)
+    c2[p_star], s2[p_star] = 0.0, 1.0
+    kp, vp = s.copy_pools()
+    oracle.kv_append_rope(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new, c2, s2)
+    rotated = 0
+    for i in range(s.num_reqs):
+        for t in range(int(s.q_lens[i])):
+            pos = int(s.ctx_lens[i]) + t
+            row = kp[s.page_table[i, pos // 16], :, pos % 16, :]
+            same = np.array_equal(row, s.k_new[int(s.q_offsets[i]) + t])
+            assert same == (pos != p_star)
+            rotated += not same
+    assert rotated == 2     # request 0 (t = 15) and request 1 (its decode token at position 20)
+
+
+def test_rope_rotation_invariants():
+    """On the unrounded rotation: every (c, c + d/2) pair keeps its norm, and scores depend on the distance only:
+    (R_m q) . (R_n k) = (R_{m-n} q) . (R_0 k) -- the property the embedding exists for."""
+    rng = np.random.default_rng(51)
+    d, n = 128, 64
+    cos, sin = synth.make_rope_tables(512, d)
+    rows = f32_to_bf16_bits(rng.standard_normal((n, d)).astype(np.float32))
+    pos = rng.integers(0, 512, n).astype(np.int32)
+    rot = oracle.rope_rotate(rows, pos, cos, sin)
+    x = bf16_to_f64(rows)
+    half = d // 2
+    # fp32 tables: cos^2 + sin^2 = 1 to ~1e-7
+    assert np.allclose(rot[:, :half] ** 2 + rot[:, half:] ** 2, x[:, :half] ** 2 + x[:, half:] ** 2, rtol=1e-6, atol=1e-9)
+    q = f32_to_bf16_bits(rng.standard_normal((1, d)).astype(np.float32))
+    k = f32_to_bf16_bits(rng.standard_normal((1, d)).astype(np.float32))
+    for m, nn in ((300, 100), (17, 3), (511, 500)):
+        lhs = float((oracle.rope_rotate(q, [m], cos, sin) @ oracle.rope_rotate(k, [nn], cos, sin).T)[0, 0])
+        rhs = float((oracle.rope_rotate(q, [m - nn], cos, sin) @ oracle.rope_rotate(k, [0], cos, sin).T)[0, 0])
+        assert abs(lhs - rhs) <= 2e-5 * (1 + abs(rhs))   # the fp32 tables are the only inexact part
+    assert np.array_equal(oracle.rope_rotate(k, [0], cos, sin), bf16_to_f64(k))   # position 0: angle 0
+
+
+def test_rope_append_equals_rotation_by_explicit_2x2_matrices():
+    """A separate route to the stored bits: numpy fancy indexing for the placement, an explicit 2 x 2 rotation matrix per
+    (position, pair) in float64, torch's own float64 -> bfloat16 conversion for the rounding."""
+    s, cos, sin = _rope_case(seed=52, d=128, q_lens=(70, 1), ctx_lens=(9, 300))
+    kp, vp = s.copy_pools()
+    oracle.kv_append_rope(kp, vp, s.q_lens, s.ctx_lens, s.q_offsets, s.page_table, s.k_new, s.v_new, cos, sin)
+    half = s.head_dim // 2
+    for i in range(s.num_reqs):
+        for t in (0, int(s.q_lens[i]) - 1):
+            pos = int(s.ctx_lens[i]) + t
+            src = bf16_to_f64(s.k_new[int(s.q_offsets[i]) + t])          # [Hkv, d]
+            want = np.empty_like(src)
+            for c in range(half):
+                R = np.array([[cos[pos, c], -sin[pos, c]], [sin[pos, c], cos[pos, c]]], np.float64)
+                want[:, [c, c + half]] = src[:, [c, c + half]] @ R.T
+            bits = torch.from_numpy(want).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+            assert np.array_equal(kp[s.page_table[i, pos // 16], :, pos % 16, :], bits)
