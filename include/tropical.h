@@ -85,6 +85,19 @@ typedef struct {
 int tropical_kv_append(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
                        const void *k_new, const void *v_new, void *cuda_stream);
 
+/* SURVEY.md 8(f) NEXT-4 "fuse RoPE+append": tropical_kv_append with rotary position embedding applied to the K rows on
+ * their way into the pool (V rows are copied).  The paper says nothing about positional encoding; the convention is the
+ * "rotate-half" one of its model family [DESIGN.md, readings]: for pos = c_i + t and channel c < d/2,
+ *   k'[c]       = k[c] * cos[pos][c] - k[c + d/2] * sin[pos][c]
+ *   k'[c + d/2] = k[c + d/2] * cos[pos][c] + k[c] * sin[pos][c]        (fp32 arithmetic, bf16 round-to-nearest-even)
+ *   cos_table, sin_table [device] fp32 [table_len][d/2], 16-byte aligned, caller-owned (angles are the caller's: any
+ *   base / scaling); table_len >= batch->max_kv_len, else INVALID_ARG.  One launch; same stream ordering as
+ * tropical_kv_append.  Queries are rotated by the caller (the attention calls take q as given), and tropical_mixed_step
+ * appends k_new as given: pass it rows that are already rotated, or use this call + tropical_mixed_attention. */
+int tropical_kv_append_rope(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
+                            const void *k_new, const void *v_new, const float *cos_table,
+                            const float *sin_table, int32_t table_len, void *cuda_stream);
+
 /* Row A2 as a standalone check / migration building block: dense copy-out of the first n_keys
  * keys of request req through the page table: k_dense, v_dense [device] bf16 [n_keys][Hkv][d]. */
 int tropical_kv_gather(const tropical_kv_pool_t *pool, const tropical_batch_t *batch, int32_t req,

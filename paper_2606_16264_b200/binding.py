@@ -94,7 +94,7 @@ class SimSummary(ctypes.Structure):
 SIM_COLOCATED, SIM_DISAGGREGATED, SIM_MULTIPLEXED = 0, 1, 2
 
 EXPORTS = (
-    "tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention", "tropical_mixed_step",
+    "tropical_kv_append", "tropical_kv_append_rope", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention", "tropical_mixed_step",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost", "tropical_iter_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
     "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_set_fused", "tropical_debug_wait_profile", "tropical_debug_read_profile", "tropical_debug_timeline",
@@ -122,7 +122,7 @@ def lib():
     L.tropical_status_string.restype = ctypes.c_char_p
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
-    for name in ("tropical_kv_append", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_mixed_step", "tropical_step_host",
+    for name in ("tropical_kv_append", "tropical_kv_append_rope", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_mixed_step", "tropical_step_host",
                  "tropical_step_cost", "tropical_iter_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
                  "tropical_debug_read_profile"):
         getattr(L, name).restype = ctypes.c_int
@@ -269,6 +269,20 @@ def kv_append(pool: KVPool, batch: Batch, k_new: torch.Tensor, v_new: torch.Tens
     p, b = pool.c(), batch.c()
     _check(lib().tropical_kv_append(ctypes.byref(p), ctypes.byref(b), _ptr(k_new), _ptr(v_new), _stream(stream)),
            "tropical_kv_append")
+
+
+def kv_append_rope(pool: KVPool, batch: Batch, k_new: torch.Tensor, v_new: torch.Tensor, cos: torch.Tensor,
+                   sin: torch.Tensor, stream=None) -> None:
+    """tropical_kv_append_rope: the append with rotate-half RoPE on the K rows; cos, sin: float32 CUDA [table_len, d/2]."""
+    _dev2(k_new, "k_new"); _dev2(v_new, "v_new")
+    for t, name in ((cos, "cos"), (sin, "sin")):
+        if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.dim() == 2):
+            raise ValueError(f"{name} must be a contiguous float32 CUDA tensor [table_len, d/2]")
+    if cos.shape != sin.shape or cos.shape[1] * 2 != pool.k_pool.shape[3]:
+        raise ValueError("cos / sin must both be [table_len, head_dim / 2]")
+    p, b = pool.c(), batch.c()
+    _check(lib().tropical_kv_append_rope(ctypes.byref(p), ctypes.byref(b), _ptr(k_new), _ptr(v_new), _ptr(cos), _ptr(sin),
+                                         ctypes.c_int32(cos.shape[0]), _stream(stream)), "tropical_kv_append_rope")
 
 
 def kv_gather(pool: KVPool, batch: Batch, req: int, n_keys: int, stream=None):

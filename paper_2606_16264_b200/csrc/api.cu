@@ -107,6 +107,25 @@ int tropical_kv_append(const tropical_kv_pool_t* pool, const tropical_batch_t* b
     return TROPICAL_OK;
 }
 
+int tropical_kv_append_rope(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* k_new,
+                            const void* v_new, const float* cos_table, const float* sin_table, int32_t table_len,
+                            void* cuda_stream) {
+    g_launches = 0;
+    int rc = check_pool(pool);
+    if (rc != TROPICAL_OK) return rc;
+    rc = check_batch(pool, batch);
+    if (rc != TROPICAL_OK) return rc;
+    if (table_len < 0 || table_len < batch->max_kv_len) return TROPICAL_ERR_INVALID_ARG;  // a row for every position
+    if (batch->total_q == 0) return TROPICAL_OK;
+    if (k_new == nullptr || v_new == nullptr || cos_table == nullptr || sin_table == nullptr) return TROPICAL_ERR_INVALID_ARG;
+    if (((uintptr_t)cos_table & 15) || ((uintptr_t)sin_table & 15)) return TROPICAL_ERR_INVALID_ARG;
+    cudaError_t e = launch_kv_append_rope(to_pool(pool), to_batch(batch), k_new, v_new, cos_table, sin_table,
+                                          (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "kv_append_rope");
+    g_launches = 1;
+    return TROPICAL_OK;
+}
+
 int tropical_kv_gather(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, int32_t req, int32_t n_keys,
                        void* k_dense, void* v_dense, void* cuda_stream) {
     g_launches = 0;

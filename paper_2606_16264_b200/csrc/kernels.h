@@ -10,6 +10,8 @@ namespace tropical {
 
 cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const void* k_new, const void* v_new,
                              cudaStream_t stream);
+cudaError_t launch_kv_append_rope(const PoolDesc& pool, const BatchDesc& b, const void* k_new, const void* v_new,
+                                  const float* cos_t, const float* sin_t, cudaStream_t stream);
 cudaError_t launch_kv_gather(const PoolDesc& pool, const BatchDesc& b, int req, int n_keys, void* k_dense,
                              void* v_dense, cudaStream_t stream);
 // NEXT-3 KV migration (csrc/kv_migrate.cu): source pool through src_pt -> destination pool under dst_pt

@@ -77,6 +77,62 @@ __global__ void __launch_bounds__(256) kv_append_kernel(PoolDesc pool, BatchDesc
     if (threadIdx.x == 0) tl_mark(1, false);
 }
 
+// SURVEY 8(f) NEXT-4 "fuse RoPE+append": the same scatter with rotate-half rotary embedding applied to the K rows on the
+// way (include/tropical.h tropical_kv_append_rope): channel c < d/2 pairs with c + d/2, the token at position pos uses
+// row pos of the caller's fp32 tables cos, sin [table_len][d/2].  One thread per (token, kv head, 16-byte chunk c of the
+// lower half): it reads chunks c and c + d/16 of the K row (the two halves of 8 pairs), 8 cos and 8 sin values, writes
+// both rotated chunks, and copies the two V chunks.  fp32 arithmetic (fmaf), bf16 round-to-nearest-even.
+__device__ __forceinline__ void rope8(const uint4& lo, const uint4& hi, const float4& c0, const float4& c1, const float4& s0,
+                                      const float4& s1, uint4& out_lo, uint4& out_hi) {
+    const uint32_t xl[4] = {lo.x, lo.y, lo.z, lo.w}, xh[4] = {hi.x, hi.y, hi.z, hi.w};
+    const float cs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+    const float sn[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+    uint32_t ol[4], oh[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float x0 = bf16_lo(xl[j]), x1 = bf16_hi(xl[j]), y0 = bf16_lo(xh[j]), y1 = bf16_hi(xh[j]);
+        ol[j] = pack_bf16x2(fmaf(x0, cs[2 * j], -(y0 * sn[2 * j])), fmaf(x1, cs[2 * j + 1], -(y1 * sn[2 * j + 1])));
+        oh[j] = pack_bf16x2(fmaf(y0, cs[2 * j], x0 * sn[2 * j]), fmaf(y1, cs[2 * j + 1], x1 * sn[2 * j + 1]));
+    }
+    out_lo = make_uint4(ol[0], ol[1], ol[2], ol[3]);
+    out_hi = make_uint4(oh[0], oh[1], oh[2], oh[3]);
+}
+
+template <int D>
+__global__ void __launch_bounds__(256) kv_append_rope_kernel(PoolDesc pool, BatchDesc b, const uint4* __restrict__ k_new,
+                                                             const uint4* __restrict__ v_new,
+                                                             const float4* __restrict__ cos_t,
+                                                             const float4* __restrict__ sin_t) {
+    constexpr int CH = D / 8;    // 16-byte chunks per row
+    constexpr int HC = CH / 2;   // chunks of the lower half = threads per row
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // as kv_append_kernel: the tile directory may overlap
+    const long long total = (long long)b.total_q * pool.Hkv * HC;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int chunk = (int)(idx % HC);
+        long long r = idx / HC;
+        const int h = (int)(r % pool.Hkv);
+        const int tok = (int)(r / pool.Hkv);
+        const int req = find_request(b.q_offsets, b.num_reqs, tok);
+        const int pos = __ldg(b.ctx_lens + req) + tok - __ldg(b.q_offsets + req);
+        const int page = __ldg(b.page_table + (size_t)req * b.stride + pos / kPageSize);
+        const size_t src = ((size_t)tok * pool.Hkv + h) * CH + chunk;
+        const size_t dst = (((size_t)page * pool.Hkv + h) * kPageSize + pos % kPageSize) * CH + chunk;
+        const size_t tab = (size_t)pos * (D / 8) + chunk * 2;  // float4 index: row pos of [table_len][D/2] floats
+        const uint4 klo = __ldg(k_new + src), khi = __ldg(k_new + src + HC);
+        const uint4 vlo = __ldg(v_new + src), vhi = __ldg(v_new + src + HC);
+        const float4 c0 = __ldg(cos_t + tab), c1 = __ldg(cos_t + tab + 1), s0 = __ldg(sin_t + tab), s1 = __ldg(sin_t + tab + 1);
+        uint4 olo, ohi;
+        rope8(klo, khi, c0, c1, s0, s1, olo, ohi);
+        uint4* kp = reinterpret_cast<uint4*>(const_cast<uint16_t*>(pool.k_pool));
+        uint4* vp = reinterpret_cast<uint4*>(const_cast<uint16_t*>(pool.v_pool));
+        kp[dst] = olo;
+        kp[dst + HC] = ohi;
+        vp[dst] = vlo;
+        vp[dst + HC] = vhi;
+    }
+}
+
 template <int D>
 __global__ void __launch_bounds__(256) kv_gather_kernel(PoolDesc pool, BatchDesc b, int req, int n_keys,
                                                         uint4* __restrict__ k_dense, uint4* __restrict__ v_dense) {
@@ -165,6 +221,20 @@ cudaError_t launch_kv_append(const PoolDesc& pool, const BatchDesc& b, const voi
         kv_append_kernel<128><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new, (int)hg);
     else
         kv_append_kernel<64><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new, (int)hg);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_kv_append_rope(const PoolDesc& pool, const BatchDesc& b, const void* k_new, const void* v_new,
+                                  const float* cos_t, const float* sin_t, cudaStream_t stream) {
+    if (b.total_q == 0) return cudaSuccess;
+    const long long total = (long long)b.total_q * pool.Hkv * (pool.D / 16);
+    const int grid = grid_for(total, 256, 148LL * 6);
+    if (pool.D == 128)
+        kv_append_rope_kernel<128><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new,
+                                                             (const float4*)cos_t, (const float4*)sin_t);
+    else
+        kv_append_rope_kernel<64><<<grid, 256, 0, stream>>>(pool, b, (const uint4*)k_new, (const uint4*)v_new,
+                                                            (const float4*)cos_t, (const float4*)sin_t);
     return cudaGetLastError();
 }
 
