@@ -91,7 +91,8 @@ typedef struct {
     int64_t kv_capacity_tokens;  /* per worker */
     double migrate_us_per_token; /* KV migration between workers */
     int32_t num_q_heads, num_kv_heads, head_dim, page_size, num_layers;
-    tropical_cost_model_t attn;  /* coefficients of tropical_step_cost for one layer's append + attention */
+    tropical_cost_model_t attn;  /* coefficients of tropical_step_cost for one layer's append + attention; n_sm <= 0:
+                                  * the built-in B200 fits (one set per kernel variant of the step), UNCALIBRATED if none */
     double linear_us_per_token;  /* the rest of an iteration, linear in its new tokens */
     double iter_overhead_us;
     /* NEXT-4: with layer.d_model > 0 an iteration lasts tropical_iter_cost(&attn, &linear, &layer, heads, batch) +

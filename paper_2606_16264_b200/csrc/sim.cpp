@@ -58,16 +58,18 @@ struct Sim {
 
     // duration of an iteration over the batch currently in q_buf / c_buf
     double iter_time() {
+        // attn.n_sm <= 0: the library's built-in fits, one coefficient set per kernel variant of the step
+        const tropical_cost_model_t* attn = cfg.attn.n_sm > 0 ? &cfg.attn : nullptr;
         if (cfg.layer.d_model > 0) {  // NEXT-4: whole-iteration predictor (attention on the head shard + GEMMs + all-reduce)
             double it = 0;
-            const int rc = tropical_iter_cost(&cfg.attn, &cfg.linear, &cfg.layer, cfg.num_q_heads, cfg.num_kv_heads,
+            const int rc = tropical_iter_cost(attn, &cfg.linear, &cfg.layer, cfg.num_q_heads, cfg.num_kv_heads,
                                               cfg.head_dim, cfg.page_size, (int32_t)q_buf.size(), q_buf.data(),
                                               c_buf.data(), &it, nullptr);
             if (rc != TROPICAL_OK) status = rc;
             return it + cfg.iter_overhead_us;
         }
         double us = 0;
-        const int rc = tropical_step_cost(&cfg.attn, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim, cfg.page_size,
+        const int rc = tropical_step_cost(attn, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim, cfg.page_size,
                                           (int32_t)q_buf.size(), q_buf.data(), c_buf.data(), &us, nullptr);
         if (rc != TROPICAL_OK) status = rc;
         long long tokens = 0;

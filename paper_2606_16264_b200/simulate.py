@@ -5,7 +5,8 @@
 
 Drives tropical_sim_run (include/tropical_sim.h) for the 13B-like model of C4 (40/40/128 heads, d_model 5120, FFN 13824,
 40 layers).  Iteration times are tropical_iter_cost (NEXT-4): per layer the step-cost fit of the head shard on this GPU
-(csrc/cost_model_fit.inc; --tp 2 = the paper's TP = 2 inside a worker) plus the linear layers from the fit to
+(csrc/cost_model_fit.inc, one coefficient set per kernel variant of the step: prefill-only iterations of prefill workers
+run the faster fused variant; --tp 2 = the paper's TP = 2 inside a worker) plus the linear layers from the fit to
 library GEMMs measured on the B200 (csrc/linear_model_fit.inc, calibration/b200_gemm.csv).  No norms / RoPE / sampling;
 the all-reduce of TP > 1 is entered from NVLink's nominal 900 GB/s per direction and 5 us latency -- NOT measured (one GPU).
 KV migration costs layers * (K + V bytes per token) at the rate tropical_kv_migrate reached pool to pool on
@@ -24,14 +25,6 @@ import re
 from . import binding as tb
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-
-
-def builtin_model(Hq: int, Hkv: int, d: int) -> tb.CostModel:
-    text = open(os.path.join(HERE, "csrc", "cost_model_fit.inc")).read()
-    for m in re.finditer(r"\{(\d+), (\d+), (\d+), (\d+), \{([^}]*)\}\}", text):   # the plain variant's set (fused = 0)
-        if (int(m.group(1)), int(m.group(2)), int(m.group(3)), int(m.group(4))) == (Hq, Hkv, d, 0):
-            return tb.CostModel(*[float(x) for x in m.group(5).split(",")])
-    raise KeyError(f"no fitted coefficients for {Hq}/{Hkv}/{d}")
 
 
 def builtin_linear() -> tb.LinearModel:
@@ -69,7 +62,8 @@ def config(policy: int, workers: int, prefill_workers: int, ttft_slo_us: float, 
     shape = tb.LayerShape(m["d_model"], m["d_ffn"], 1, m["layers"], tp)
     return tb.SimConfig(policy, workers, prefill_workers, 2048, ttft_slo_us, tpot_slo_us, 0.8, 0.9, 2_000_000,
                         migrate_us_per_token(m["Hkv"] // tp, m["d"], m["layers"], link_gbs), m["Hq"], m["Hkv"], m["d"], 16,
-                        m["layers"], builtin_model(m["Hq"] // tp, m["Hkv"] // tp, m["d"]), 0.0, 0.0, shape, lin,
+                        m["layers"], tb.CostModel(0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0),   # n_sm = 0: the library's built-in fits
+                        0.0, 0.0, shape, lin,
                         1 if role_transitions else 0, 8 if role_transitions else 0)
 
 
