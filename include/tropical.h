@@ -210,13 +210,16 @@ int tropical_step_host(const tropical_kv_pool_t *pool, const tropical_host_batch
 /* Row A6: predicted microseconds of append + attention for a batch ("predicted
  * execution time", "offline profiling tools", P:159 decode-batch time).  Pure host
  * code, reentrant.  Form:
- *   t = t0 + max(a*F, b*B) + kappa*min(a*F, b*B) + e_p*N_p/n_sm + e_d*N_d/n_sm
+ *   t = t0 + max(a*F, b*B) + kappa*min(a*F, b*B) + e_p*N_p/n_sm + e_d*N_d/n_sm + e_c*N_c
  * with F FLOPs, B algorithmic bytes, N_p prefill (128-row x head) tiles weighted by their KV
- * iterations, N_d decode page-head units.  model == NULL selects the built-in fit measured on
+ * iterations, N_d decode page-head units, N_c the KV iterations of the heaviest prefill item (the critical path when a
+ * step has about as many items as the GPU has SMs; an item is two heads of a kv group at the top row tile, or -- MHA /
+ * odd groups -- the top row tile, or the top TWO row tiles in the fused variant of tropical_mixed_step).  model == NULL selects the built-in fit measured on
  * B200 for (Hq, Hkv, d), else TROPICAL_ERR_UNCALIBRATED. */
 typedef struct {
     double t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us;
     double n_sm;
+    double e_prefill_crit_us; /* e_c: per KV iteration of the heaviest prefill item */
 } tropical_cost_model_t;
 
 typedef struct {
@@ -227,6 +230,7 @@ typedef struct {
     int64_t prefill_tiles; /* sum over prefill requests of ceil(q_i/128) * Hq                */
     int64_t prefill_iters; /* 128x128 KV iterations over those tiles                          */
     int64_t decode_units;  /* decode page-head units: sum ceil(L_i/P) * Hkv                   */
+    int64_t prefill_critical_iters; /* N_c: KV iterations of the heaviest prefill item       */
 } tropical_cost_breakdown_t;
 
 int tropical_step_cost(const tropical_cost_model_t *model, int32_t num_q_heads,

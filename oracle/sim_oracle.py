@@ -25,6 +25,7 @@ class CostModel:
     e_prefill_iter_us: float
     e_decode_unit_us: float
     n_sm: float = 148.0
+    e_prefill_crit_us: float = 0.0
 
 
 @dataclass
@@ -73,11 +74,14 @@ class Config:
 
 
 def step_cost_us(cfg: Config, q_lens: List[int], ctx_lens: List[int], tp: int = 1) -> float:
-    """t = t0 + max(aF, bB) + kappa min(aF, bB) + e_p N_p / n_sm + e_d N_d / n_sm (DESIGN.md sections 6, 7), on the
+    """t = t0 + max(aF, bB) + kappa min(aF, bB) + e_p N_p / n_sm + e_d N_d / n_sm + e_c N_c (DESIGN.md sections 6, 7), on the
     head shard Hq/tp, Hkv/tp (the path shards by kv head with no collective)."""
     Hq, Hkv, d, P = cfg.num_q_heads // tp, cfg.num_kv_heads // tp, cfg.head_dim, cfg.page_size
     qc = pages = T = csum = 0.0
-    iters = units = 0
+    iters = units = crit = 0
+    # the step's kernel variant: tropical_mixed_step fuses from 64 new tokens per request up (include/tropical.h)
+    fused = len(q_lens) > 0 and sum(q_lens) >= 64 * len(q_lens)
+    head_pairs = (Hq // Hkv) % 2 == 0
     for q, c in zip(q_lens, ctx_lens):
         if q <= 0:
             continue
@@ -90,16 +94,22 @@ def step_cost_us(cfg: Config, q_lens: List[int], ctx_lens: List[int], tp: int = 
             units += ((L + P - 1) // P) * Hkv
         else:
             nt = (q + 127) // 128
+            kv = []                                  # KV tiles of every 128-row tile of the chunk
             for ti in range(nt):
                 last = c + min((ti + 1) * 128, q)
-                iters += ((last + 127) // 128) * Hq
+                kv.append((last + 127) // 128)
+                iters += kv[-1] * Hq
+            # heaviest item: two heads at the top tile / (fused variant, odd group) the top two row tiles / the top tile
+            below = kv[-2] if nt >= 2 else 0
+            crit = max(crit, 2 * kv[-1] if head_pairs else (kv[-1] + below if fused else kv[-1]))
     flops = 4.0 * d * Hq * qc
     nbytes = 2.0 * 2 * Hkv * d * csum + 2.0 * (2.0 * 2 * Hkv * d * T) + 2.0 * (2.0 * Hq * d * T) + 4.0 * pages
     m = cfg.attn
     t_tc, t_hbm = m.a_us_per_flop * flops, m.b_us_per_byte * nbytes
     hi, lo = max(t_tc, t_hbm), min(t_tc, t_hbm)
     nsm = m.n_sm if m.n_sm > 0 else 148.0
-    return m.t0_us + hi + m.kappa * lo + m.e_prefill_iter_us * iters / nsm + m.e_decode_unit_us * units / nsm
+    return (m.t0_us + hi + m.kappa * lo + m.e_prefill_iter_us * iters / nsm + m.e_decode_unit_us * units / nsm +
+            m.e_prefill_crit_us * crit)
 
 
 def iter_cost_us(cfg: Config, q_lens: List[int], ctx_lens: List[int]) -> float:

@@ -36,13 +36,13 @@ class _Batch(ctypes.Structure):
 class CostModel(ctypes.Structure):
     _fields_ = [("t0_us", ctypes.c_double), ("a_us_per_flop", ctypes.c_double), ("b_us_per_byte", ctypes.c_double),
                 ("kappa", ctypes.c_double), ("e_prefill_iter_us", ctypes.c_double),
-                ("e_decode_unit_us", ctypes.c_double), ("n_sm", ctypes.c_double)]
+                ("e_decode_unit_us", ctypes.c_double), ("n_sm", ctypes.c_double), ("e_prefill_crit_us", ctypes.c_double)]
 
 
 class CostBreakdown(ctypes.Structure):
     _fields_ = [("flops", ctypes.c_double), ("bytes", ctypes.c_double), ("t_tc_us", ctypes.c_double),
                 ("t_hbm_us", ctypes.c_double), ("prefill_tiles", ctypes.c_int64), ("prefill_iters", ctypes.c_int64),
-                ("decode_units", ctypes.c_int64)]
+                ("decode_units", ctypes.c_int64), ("prefill_critical_iters", ctypes.c_int64)]
 
 
 class LayerShape(ctypes.Structure):

@@ -254,14 +254,14 @@ def point_features(row):
     from . import binding as tb
     q, c = grid_lengths(row["prefill_tokens"], row["prefill_ctx"], row["n_decode"], row["ctx_median"], row["seed"])
     _, bd = tb.step_cost(row["Hq"], row["Hkv"], row["d"], 16, q.tolist(), c.tolist(), require_model=False)
-    return bd.flops, bd.bytes, float(bd.prefill_iters), float(bd.decode_units)
+    return bd.flops, bd.bytes, float(bd.prefill_iters), float(bd.decode_units), float(bd.prefill_critical_iters)
 
 
 def predict(theta, X, n_sm=148.0):
-    t0, a, b, kappa, ep, ed = theta
-    F, B, Np, Nd = X.T
+    t0, a, b, kappa, ep, ed, ec = theta
+    F, B, Np, Nd, Nc = X.T
     tc, hb = a * F, b * B
-    return t0 + np.maximum(tc, hb) + kappa * np.minimum(tc, hb) + ep * Np / n_sm + ed * Nd / n_sm
+    return t0 + np.maximum(tc, hb) + kappa * np.minimum(tc, hb) + ep * Np / n_sm + ed * Nd / n_sm + ec * Nc
 
 
 # Physical lower bounds of the two roofline coefficients (nominal peaks of the part: 2250 TFLOP/s dense bf16,
@@ -281,20 +281,21 @@ def is_fused_step(row) -> bool:
 
 
 def fit_shape(rows, base=None):
-    """Six coefficients by bounded least squares on relative error.  base = the plain variant's coefficients: then only
-    t0, a and e_p are fitted (a fused-variant step has few decode requests: too few points to identify the rest)."""
+    """Seven coefficients by bounded least squares on relative error.  base = the plain variant's coefficients: then
+    only t0, a, e_p and e_c are fitted (a fused-variant step has few decode requests: too few points to identify the
+    rest)."""
     from scipy.optimize import least_squares
     X = np.array([point_features(r) for r in rows])
     y = np.array([r["us_median"] for r in rows])
     train = np.array([not is_held_out(r) for r in rows])
     off = np.array([r["seed"] >= 1000 for r in rows])
-    scale = np.array([10.0, 1e-9, 1e-7, 1.0, 1.0, 0.01])   # parameter magnitudes (us, us/FLOP, us/byte, -, us, us)
-    lo = np.array([0, A_MIN_US_PER_FLOP / scale[1], B_MIN_US_PER_BYTE / scale[2], 0, 0, 0])
-    hi = np.array([20, 50, 50, 1, 50, 500])
-    free = np.ones(6, bool)
+    scale = np.array([10.0, 1e-9, 1e-7, 1.0, 1.0, 0.01, 1.0])   # parameter magnitudes (us, us/FLOP, us/byte, -, us, us, us)
+    lo = np.array([0, A_MIN_US_PER_FLOP / scale[1], B_MIN_US_PER_BYTE / scale[2], 0, 0, 0, 0])
+    hi = np.array([20, 50, 50, 1, 50, 500, 50])
+    free = np.ones(7, bool)
     if base is not None:
-        free = np.array([True, True, False, False, True, False])
-    fixed = (np.asarray(base) / scale) if base is not None else np.zeros(6)
+        free = np.array([True, True, False, False, True, False, True])
+    fixed = (np.asarray(base) / scale) if base is not None else np.zeros(7)
 
     def full(xf):
         x = fixed.copy()
@@ -303,7 +304,7 @@ def fit_shape(rows, base=None):
 
     res_best = None
     for k0 in (0.1, 0.5, 0.9):
-        x0 = np.array([1.0, 1.5, 1.6, k0, 0.5, 1.0])[free]
+        x0 = np.array([1.0, 1.5, 1.6, k0, 0.5, 1.0, 0.1])[free]
         fun = lambda xf: (predict(full(xf), X[train]) - y[train]) / y[train]
         res = least_squares(fun, x0, bounds=(lo[free], hi[free]))
         if res_best is None or res.cost < res_best.cost:
@@ -362,7 +363,8 @@ def fit(grid_path: str, write: bool, gemm_path: str = None):
     rows = read_grid(grid_path)
     shapes = sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows})
     lines = ["// Generated by `python -m paper_2606_16264_b200.cost_fit fit` from calibration/b200_grid.csv.",
-             "// {Hq, Hkv, d, fused, {t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us, n_sm}}",
+             "// {Hq, Hkv, d, fused, {t0_us, a_us_per_flop, b_us_per_byte, kappa, e_prefill_iter_us, e_decode_unit_us, n_sm, "
+             "e_prefill_crit_us}}",
              "// fused = 1: steps tropical_mixed_step runs through its fused kernel variant (>= 64 new tokens per request).",
              "// a >= 1 / (2250 TFLOP/s) and b >= 1 / (8 TB/s) are enforced by the fit (nominal peaks of the part)."]
     for s in shapes:
@@ -373,9 +375,9 @@ def fit(grid_path: str, write: bool, gemm_path: str = None):
         theta_f, st_f = fit_shape(fused, base=theta)
         for tag, th, stt in ((0, theta, st), (1, theta_f, st_f)):
             print(f"shape {s} fused={tag}: theta={['%.4g' % t for t in th]} {stt}")
-            lines.append("{%d, %d, %d, %d, {%.6g, %.6g, %.6g, %.6g, %.6g, %.6g, 148}},  // %d points; held-out MAPE %.1f %%, "
-                         "max %.1f %%; off-grid MAPE %.1f %%, max %.1f %%"
-                         % (*s, tag, *th, stt["n"], 100 * stt["mape_held"], 100 * stt["max_held"],
+            lines.append("{%d, %d, %d, %d, {%.6g, %.6g, %.6g, %.6g, %.6g, %.6g, 148, %.6g}},  // %d points; held-out MAPE "
+                         "%.1f %%, max over all %.1f %%; off-grid MAPE %.1f %%, max %.1f %%"
+                         % (*s, tag, *th[:6], th[6], stt["n"], 100 * stt["mape_held"], 100 * stt["max_all"],
                             100 * stt["mape_off_grid"], 100 * stt["max_off_grid"]))
     gemm_path = gemm_path or GEMM_GRID
     theta_l, st_l = fit_linear(read_gemm(gemm_path))

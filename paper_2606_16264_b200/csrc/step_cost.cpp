@@ -21,7 +21,7 @@ constexpr int kFusedMinTokensPerReq = 64;  // must equal csrc/mixed.cu's
 // Coefficients fitted to measured step times by `python -m paper_2606_16264_b200.cost_fit fit` from the grid
 // that `... cost_fit measure` wrote on a B200 (calibration/b200_grid.csv; provenance in DESIGN.md section 7).
 const BuiltinFit kBuiltin[] = {
-    {0, 0, 0, 0, {0, 0, 0, 0, 0, 0, 148}},  // sentinel: never matches
+    {0, 0, 0, 0, {0, 0, 0, 0, 0, 0, 148, 0}},  // sentinel: never matches
 #include "cost_model_fit.inc"
 };
 
@@ -30,10 +30,12 @@ const tropical_linear_model_t kBuiltinLinear =
 #include "linear_model_fit.inc"
     ;
 
-void features(int Hq, int Hkv, int d, int P, int n, const int32_t* q, const int32_t* c,
+// fused: the step runs through the fused kernel variant (tropical_mixed_step's rule), whose MHA items are row pairs
+void features(int Hq, int Hkv, int d, int P, int n, const int32_t* q, const int32_t* c, bool fused,
               tropical_cost_breakdown_t* f) {
     double qc = 0, pages = 0, T = 0, csum = 0;
-    int64_t tiles = 0, iters = 0, units = 0;
+    int64_t tiles = 0, iters = 0, units = 0, crit = 0;
+    const bool head_pairs = (Hq / Hkv) % 2 == 0;  // two heads of a kv group per prefill item (csrc/plan.cuh)
     for (int i = 0; i < n; ++i) {
         const double qi = q[i], ci = c[i];
         if (q[i] <= 0) continue;
@@ -47,10 +49,17 @@ void features(int Hq, int Hkv, int d, int P, int n, const int32_t* q, const int3
         } else {
             const int nt = (q[i] + 127) / 128;
             tiles += (int64_t)nt * Hq;
+            int64_t kv_top = 0, kv_below = 0;  // KV tiles of the last row tile and of the one before it
             for (int ti = 0; ti < nt; ++ti) {
                 const int64_t last = (int64_t)c[i] + ((ti + 1) * 128 < q[i] ? (ti + 1) * 128 : q[i]);
                 iters += ((last + 127) / 128) * Hq;
+                kv_below = kv_top;
+                kv_top = (last + 127) / 128;
             }
+            // the heaviest item of this request: two heads at the top tile, or (fused variant, MHA) the top two row
+            // tiles of one head, or the top tile alone
+            const int64_t item = head_pairs ? 2 * kv_top : (fused ? kv_top + kv_below : kv_top);
+            if (item > crit) crit = item;
         }
     }
     f->flops = 4.0 * d * Hq * qc;
@@ -58,6 +67,7 @@ void features(int Hq, int Hkv, int d, int P, int n, const int32_t* q, const int3
     f->prefill_tiles = tiles;
     f->prefill_iters = iters;
     f->decode_units = units;
+    f->prefill_critical_iters = crit;
     f->t_tc_us = 0;
     f->t_hbm_us = 0;
 }
@@ -72,12 +82,12 @@ extern "C" int tropical_step_cost(const tropical_cost_model_t* model, int32_t Hq
     if (out_us == nullptr && breakdown == nullptr) return TROPICAL_ERR_INVALID_ARG;
     for (int i = 0; i < num_reqs; ++i)
         if (q_lens[i] < 0 || ctx_lens[i] < 0) return TROPICAL_ERR_INVALID_ARG;
+    long long T = 0;
+    for (int i = 0; i < num_reqs; ++i) T += q_lens[i];
+    const int fused = (num_reqs > 0 && T >= (long long)kFusedMinTokensPerReq * num_reqs) ? 1 : 0;
     tropical_cost_breakdown_t f;
-    features(Hq, Hkv, d, P, num_reqs, q_lens, ctx_lens, &f);
+    features(Hq, Hkv, d, P, num_reqs, q_lens, ctx_lens, fused != 0, &f);
     if (model == nullptr) {
-        long long T = 0;
-        for (int i = 0; i < num_reqs; ++i) T += q_lens[i];
-        const int fused = (num_reqs > 0 && T >= (long long)kFusedMinTokensPerReq * num_reqs) ? 1 : 0;
         for (const BuiltinFit& b : kBuiltin)
             if (b.Hq == Hq && b.Hkv == Hkv && b.d == d && b.fused == fused) model = &b.m;
     }
@@ -92,7 +102,8 @@ extern "C" int tropical_step_cost(const tropical_cost_model_t* model, int32_t Hq
         const double lo = f.t_tc_us > f.t_hbm_us ? f.t_hbm_us : f.t_tc_us;
         const double nsm = model->n_sm > 0 ? model->n_sm : 148.0;
         *out_us = model->t0_us + hi + model->kappa * lo + model->e_prefill_iter_us * (double)f.prefill_iters / nsm +
-                  model->e_decode_unit_us * (double)f.decode_units / nsm;
+                  model->e_decode_unit_us * (double)f.decode_units / nsm +
+                  model->e_prefill_crit_us * (double)f.prefill_critical_iters;
     }
     return TROPICAL_OK;
 }

@@ -99,11 +99,14 @@ def test_step_cost_features_match_hand_derivation():
     us, bd = tb.step_cost(4, 2, 64, 16, [130, 1], [0, 17], require_model=False)
     assert bd.flops == golden["A.flops"] and bd.bytes == golden["A.bytes"]
     assert bd.prefill_tiles == golden["A.prefill_tiles"] and bd.prefill_iters == golden["A.prefill_iters"]
-    assert bd.decode_units == golden["A.decode_units"]
+    assert bd.decode_units == golden["A.decode_units"] and bd.prefill_critical_iters == golden["A.prefill_critical_iters"]
     us, bd = tb.step_cost(8, 8, 128, 16, [256], [300], require_model=False)
     assert bd.flops == golden["B.flops"] and bd.bytes == golden["B.bytes"]
     assert bd.prefill_tiles == golden["B.prefill_tiles"] and bd.prefill_iters == golden["B.prefill_iters"]
-    assert bd.decode_units == 0
+    assert bd.decode_units == 0 and bd.prefill_critical_iters == golden["B.prefill_critical_iters"]
+    # the same chunk next to 7 decode requests: 263 tokens in 8 requests < 64 per request -> plain variant: the top tile alone
+    _, bd = tb.step_cost(8, 8, 128, 16, [256] + [1] * 7, [300] + [10] * 7, require_model=False)
+    assert bd.prefill_critical_iters == 5
 
 
 def test_step_cost_properties_with_explicit_model():
@@ -132,18 +135,15 @@ def test_builtin_cost_model_reproduces_measured_grid():
     """A6: the compiled-in coefficients (csrc/cost_model_fit.inc: one set per head shape and kernel variant of the step)
     against the B200 measurements of tropical_mixed_step they were fitted to (calibration/b200_grid.csv).  Held-out rows
     (every fifth grid point, and every off-grid point: recipe values between and beyond the grid lines) were not used by
-    the fit.  The paper gives no accuracy target; SURVEY.md 8(c)'s is held-out MAPE <= 10 %, every point within
-    25 %.  Asserted: MAPE <= 10 % held-out and off-grid per shape; at most 1 % of all points beyond 25 %, none beyond
-    30 % (the outliers are 2048-token chunks on 4096 / 8192 tokens of prior context with no decodes, where one item per
-    SM is the critical path).  Every prediction must also respect the roofline of the part's NOMINAL
-    peaks, which the fit cannot move."""
+    the fit.  The paper gives no accuracy target; the bars are SURVEY.md 8(c)'s: MAPE <= 10 % (held-out and
+    off-grid, per shape) and every one of the 535 points within 25 %.  Every prediction must also respect the roofline of
+    the part's NOMINAL peaks, which the fit cannot move."""
     import numpy as np
     from paper_2606_16264_b200 import cost_fit
     rows = cost_fit.read_grid(cost_fit.DEFAULT_GRID)
     assert len(rows) >= 400
     shapes = sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows})
     assert (20, 20, 128) in shapes and (32, 4, 128) in shapes      # the TP = 2 head shards of C4 / C5 (NEXT-4)
-    beyond = total = 0
     for shape in shapes:
         rel_all, rel_held, rel_off = [], [], []
         for r in rows:
@@ -161,10 +161,7 @@ def test_builtin_cost_model_reproduces_measured_grid():
         assert len(rel_off) >= 20
         assert np.mean(rel_held) <= 0.10, (shape, np.mean(rel_held))
         assert np.mean(rel_off) <= 0.10, (shape, np.mean(rel_off))
-        assert np.max(rel_all) <= 0.30, (shape, np.max(rel_all))
-        beyond += sum(1 for x in rel_all if x > 0.25)
-        total += len(rel_all)
-    assert beyond <= 0.01 * total, (beyond, total)
+        assert np.max(rel_all) <= 0.25, (shape, np.max(rel_all))
 
 
 def test_builtin_linear_model_reproduces_measured_gemms():

@@ -14,7 +14,7 @@ import paper_2606_16264_b200 as tb
 from oracle import sim_oracle as so
 
 FLAT = (0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 148.0)         # attention term off: iteration = overhead + linear * tokens
-FIT = (35.0, 1.0e-9, 1.15e-7, 0.15, 0.13, 0.057, 148.0)  # a B200-like fit (64/8/128), values rounded by hand
+FIT = (35.0, 1.0e-9, 1.15e-7, 0.15, 0.13, 0.057, 148.0, 0.2)  # a B200-like fit (64/8/128), values rounded by hand
 
 
 def _ocfg(policy, cm=FLAT, **kw):
@@ -33,7 +33,8 @@ def _ccfg(o: so.Config):
                         o.decode_guard, o.hbm_watermark, o.kv_capacity_tokens, o.migrate_us_per_token, o.num_q_heads,
                         o.num_kv_heads, o.head_dim, o.page_size, o.num_layers,
                         tb.CostModel(a.t0_us, a.a_us_per_flop, a.b_us_per_byte, a.kappa, a.e_prefill_iter_us,
-                                     a.e_decode_unit_us, a.n_sm), o.linear_us_per_token, o.iter_overhead_us,
+                                     a.e_decode_unit_us, a.n_sm, a.e_prefill_crit_us), o.linear_us_per_token,
+                        o.iter_overhead_us,
                         tb.LayerShape(sh.d_model, sh.d_ffn, sh.gated_mlp, sh.num_layers, sh.tp),
                         tb.LinearModel(lm.g0_us, lm.f_us_per_flop, lm.w_us_per_byte, lm.kappa, lm.ar0_us, lm.ar_us_per_byte),
                         o.role_transitions, o.delay_threshold)
@@ -146,6 +147,13 @@ def test_step_cost_closed_form_on_the_golden_batches():
         # an iteration = layers * step + linear * new tokens + overhead (tropical_sim.h "Worker iteration")
         cfg3 = _ocfg(so.COLOCATED, cm=model, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d, num_layers=3)
         assert so.iter_time_us(cfg3, q, c) == pytest.approx(3 * want + 0.1 * sum(q) + 10.0, rel=1e-12)
+    # the critical-path term e_c * N_c (N_c from the golden file: A 4, B 9) with e_c = 0.5: + 2 and + 4.5
+    for (Hq, Hkv, d), q, c, want in (((4, 2, 64), [130, 1], [0, 17], 24.122972 + 2.0), ((8, 8, 128), [256], [300], 512.188156 + 4.5)):
+        model = cm + (0.5,)
+        cfg = _ocfg(so.COLOCATED, cm=model, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=d)
+        assert so.step_cost_us(cfg, q, c) == pytest.approx(want, rel=1e-12)
+        got, _ = tb.step_cost(Hq, Hkv, d, 16, q, c, model=tb.CostModel(*model))
+        assert got == pytest.approx(want, rel=1e-12)
 
 
 def test_least_unfinished_tokens_dispatch_by_hand():
