@@ -11,8 +11,8 @@ attention launches against the measured HBM peak; `cpu_baseline` = the fp64 orac
 Beyond the contract the line carries: `us_per_step` (median / min / max of per-step event times from a second,
 instrumented pass over the same steps), `sustained` (the same step in a >= 2 s back-to-back loop: C5 runs against
 the board's power limit and the clocks it holds after ~100 ms are lower than in a short burst), fractions against
-the nominal peaks, and -- on the default run -- `extra.C4` (the other "mixed config" of the 70 % bar) and
-`extra.MIG` (KV migration).  `--config MIG` makes the migration the line's own workload.
+the nominal peaks, and -- on the default run -- `extra.C4` (the other "mixed config" of the 70 % bar), `extra.C3`
+(prefill-only: the fused kernel variant), `extra.C5_two_call` and `extra.MIG` (KV migration).  `--config MIG` makes the migration the line's own workload.
 
 N > 1 (torchrun): the path shards by request with no collective; each rank runs its own
 replica of the workload (weak scaling), timing = max over ranks.
@@ -594,6 +594,18 @@ def run_extras(args, tb, torch, peaks, local, st_c5):
                        "clocks": clk}
     except Exception as exc:
         extra["C4"] = {"error": repr(exc)}
+    try:  # the prefill-only config: tropical_mixed_step takes its fused kernel variant there (cold L2, as --config C3)
+        s3, _ = make_workload("C3", 0)
+        st = StepTimer(s3, tb, torch)
+        st.warm(3)
+        n3 = min(steps, 50)
+        us = st.timed(n3) * 1e3 / n3
+        _, _, t_roof, t_nom = roofline_times(st.cnt, peaks)
+        extra["C3"] = {"workload": f"C3 ({describe('C3')})", "value": round(us, 2), "unit": UNIT, "steps": n3,
+                       "frac": round(t_roof / us, 4), "t_roof_us": round(t_roof, 2), "launches_per_step": st.launches_per_step,
+                       "l2": "flushed between timed steps"}
+    except Exception as exc:
+        extra["C3"] = {"error": repr(exc)}
     return extra
 
 
