@@ -22,6 +22,8 @@
  *     pointer after a call returns.  Process-global state: per-device cached attributes
  *     (SM count, one-time cudaFuncSetAttribute), the resolved cuTensorMapEncodeTiled entry
  *     point.  Any number of devices per process; calls act on the current device.
+ *     One exception to "owns nothing": the module carries a fixed scratch array of
+ *     TROPICAL_STATIC_WORKSPACE_BYTES for tropical_mixed_attention_static (see there).
  *   - Test and measurement hooks live in tropical_debug.h, not here.
  *   - Device work is enqueued on the caller's stream (void* = cudaStream_t, NULL = legacy
  *     default stream).  No host synchronisation, no H2D/D2H inside the device-pointer calls;
@@ -50,7 +52,8 @@ typedef enum {
     TROPICAL_ERR_UNSUPPORTED = 2,  /* head_dim not in {64,128}, page_size != 16, Hq/Hkv > 64 */
     TROPICAL_ERR_WORKSPACE = 3,    /* workspace NULL / misaligned (256 B) / smaller than tropical_workspace_bytes */
     TROPICAL_ERR_CUDA = 4,         /* launch or runtime failure; see tropical_last_cuda_error */
-    TROPICAL_ERR_UNCALIBRATED = 5  /* tropical_step_cost: no coefficients for this head shape */
+    TROPICAL_ERR_UNCALIBRATED = 5, /* tropical_step_cost: no coefficients for this head shape */
+    TROPICAL_ERR_STATIC_CAPACITY = 6 /* tropical_mixed_attention_static: the step needs more scratch than the built-in array holds */
 } tropical_status_t;
 
 /* Paged KV pool, caller-owned.  Layout "HND": one (page, kv_head) is a contiguous
@@ -157,6 +160,43 @@ size_t tropical_workspace_bytes(const tropical_kv_pool_t *pool, int32_t num_reqs
 int tropical_mixed_attention(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
                              const void *q, void *out, float *lse, float sm_scale,
                              void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* tropical_mixed_attention for callers that cannot provide a workspace because they cannot allocate device memory.
+ *
+ * Who that is: tropical_mixed_attention wants 20-60 MB of scratch from its caller (work lists, tickets, split-K
+ * partials).  A serving worker that handed every free byte of HBM to its KV pool at start-up (the cache is
+ * sized to the memory watermark) has nothing left to cudaMalloc when a step arrives, and would not want to: cudaMalloc
+ * and cudaFree synchronise the whole device, which stalls every stream of a loop that runs once per decode iteration.
+ * The same holds for a host program that embeds this library under a "no allocation after initialisation" rule, or
+ * that reaches it from a context where it may only enqueue work (its own allocator is not reachable from there).
+ *
+ * What it does: exactly what tropical_mixed_attention does -- same kernels, same arguments except that workspace and
+ * workspace_bytes are gone, same results -- with the scratch taken from an array that is part of the library image
+ * (a file-scope __device__ array, 256-byte aligned, TROPICAL_STATIC_WORKSPACE_BYTES long).  The call allocates
+ * nothing and frees nothing: no cudaMalloc / cudaFree / cudaMallocAsync, no allocating library routine.  The caller
+ * still owns and passes every input and output (pool, batch metadata, q, out, lse).
+ *
+ * Cost and limit: every GPU on which the library's module is loaded keeps the TROPICAL_STATIC_WORKSPACE_BYTES (64 MiB)
+ * from module load until the process exits, whether this entry point is ever called or not.  A step whose
+ * tropical_workspace_bytes(pool, num_reqs, total_q, max_kv_len) exceeds that is refused with
+ * TROPICAL_ERR_STATIC_CAPACITY before anything is launched (tropical_last_cuda_error() then says how many bytes were
+ * needed); nothing is truncated.  64 MiB covers all five BASELINE.json configs (C4, the largest, needs 58.4 MB); at
+ * d = 128 it is roughly num_reqs * Hkv * ceil(Hq / Hkv / 8) <= 6000 with total_q of a few thousand.
+ *
+ * First call on a device: the array's device address is looked up then (cudaGetSymbolAddress, once per device, with
+ * that device current, remembered afterwards), and the kernels' one-time attributes are set as in every entry point.
+ * Make that first call during start-up, outside any stream capture; later calls only enqueue the two launches.
+ *
+ * One array per GPU, shared by every call and every stream: two calls of this entry point that can overlap on the
+ * same GPU (different streams, or different host threads without stream ordering between them) race on it and give
+ * wrong results.  Order them on one stream, or give the second caller tropical_mixed_attention with its own
+ * workspace.  The array keeps whatever the last call left in it; nothing in it needs to start at zero, because the
+ * tile-directory kernel rewrites the header, the ticket counters and the split-group counters of each step before
+ * the step kernel reads them, so no clearing pass is enqueued. */
+#define TROPICAL_STATIC_WORKSPACE_BYTES (64u << 20)
+int tropical_mixed_attention_static(const tropical_kv_pool_t *pool, const tropical_batch_t *batch,
+                                    const void *q, void *out, float *lse, float sm_scale,
+                                    void *cuda_stream);
 
 /* One multiplexed iteration in ONE call -- rows A0-A5 with the KV append (A1) included: the same results as
  * tropical_kv_append followed by tropical_mixed_attention (pool bit-identical afterwards, out / lse bit-identical to that

@@ -16,7 +16,7 @@ _lib = None
 class TropicalError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = status
-        detail = lib().tropical_last_cuda_error().decode() if status == 4 else ""
+        detail = lib().tropical_last_cuda_error().decode() if status in (4, 6) else ""
         super().__init__(f"{where}: {status_string(status)} (status {status}) {detail}".strip())
 
 
@@ -94,7 +94,7 @@ class SimSummary(ctypes.Structure):
 SIM_COLOCATED, SIM_DISAGGREGATED, SIM_MULTIPLEXED = 0, 1, 2
 
 EXPORTS = (
-    "tropical_kv_append", "tropical_kv_append_rope", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention", "tropical_mixed_step",
+    "tropical_kv_append", "tropical_kv_append_rope", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_workspace_bytes", "tropical_mixed_attention", "tropical_mixed_attention_static", "tropical_mixed_step",
     "tropical_step_host_staging_bytes", "tropical_step_host", "tropical_step_cost", "tropical_iter_cost",
     "tropical_last_launch_count", "tropical_status_string", "tropical_last_cuda_error", "tropical_version",
     "tropical_debug_attention_simt", "tropical_debug_set_grid", "tropical_debug_set_split_pages", "tropical_debug_set_fused", "tropical_debug_wait_profile", "tropical_debug_read_profile", "tropical_debug_timeline",
@@ -122,7 +122,7 @@ def lib():
     L.tropical_status_string.restype = ctypes.c_char_p
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
-    for name in ("tropical_kv_append", "tropical_kv_append_rope", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_mixed_step", "tropical_step_host",
+    for name in ("tropical_kv_append", "tropical_kv_append_rope", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_mixed_attention_static", "tropical_mixed_step", "tropical_step_host",
                  "tropical_step_cost", "tropical_iter_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
                  "tropical_debug_read_profile"):
         getattr(L, name).restype = ctypes.c_int
@@ -372,6 +372,28 @@ def mixed_attention(pool: KVPool, batch: Batch, q: torch.Tensor, out: Optional[t
     _check(lib().tropical_mixed_attention(ctypes.byref(p), ctypes.byref(b), _ptr(q), _ptr(out), _ptr(lse),
                                           ctypes.c_float(sm_scale), _ptr(ws), ctypes.c_size_t(ws.numel()),
                                           _stream(stream)), "tropical_mixed_attention")
+    return out
+
+
+STATIC_WORKSPACE_BYTES = 64 << 20  # TROPICAL_STATIC_WORKSPACE_BYTES in include/tropical.h
+
+
+def mixed_attention_static(pool: KVPool, batch: Batch, q: torch.Tensor, out: torch.Tensor,
+                           lse: Optional[torch.Tensor] = None, sm_scale: float = 0.0, stream=None) -> torch.Tensor:
+    """tropical_mixed_attention_static: mixed_attention for a caller that cannot allocate a workspace.
+
+    The scratch comes from a 64 MiB array built into the library (one per GPU, shared by all calls: do not let two
+    of these calls overlap on one GPU), so nothing is allocated here either: `out` is required, not created.  A
+    step that needs more than STATIC_WORKSPACE_BYTES raises TropicalError (status 6).  Make the first call on each
+    device during start-up.  Details and the list of callers this is for: include/tropical.h."""
+    _dev2(q, "q")
+    _dev2(out, "out")
+    p, b = pool.c(), batch.c()
+    if lse is not None and not (lse.is_cuda and lse.dtype == torch.float32 and lse.is_contiguous()):
+        raise ValueError("lse must be a contiguous float32 CUDA tensor")
+    _check(lib().tropical_mixed_attention_static(ctypes.byref(p), ctypes.byref(b), _ptr(q), _ptr(out), _ptr(lse),
+                                                 ctypes.c_float(sm_scale), _stream(stream)),
+           "tropical_mixed_attention_static")
     return out
 
 

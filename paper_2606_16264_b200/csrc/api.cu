@@ -5,6 +5,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <atomic>
+
 #include "../../include/tropical.h"
 #include "../../include/tropical_debug.h"
 #include "kernels.h"
@@ -85,6 +87,38 @@ int mixed_attention_impl(const tropical_kv_pool_t* pool, const tropical_batch_t*
     cudaError_t e = launch_mixed_attention(to_pool(pool), to_batch(batch), q, k_new, v_new, out, lse, scale_log2,
                                            workspace, stream, launches);
     if (e != cudaSuccess) return cuda_fail(e, "mixed_attention");
+    return TROPICAL_OK;
+}
+
+
+// ---- built-in scratch for tropical_mixed_attention_static (include/tropical.h) ----------------------------------
+// The step's work lists and split-K partials normally live in a workspace the caller allocates.  A caller that may
+// not allocate device memory gets this array instead: it is part of the loaded module, so every GPU that loads
+// libtropical.so holds TROPICAL_STATIC_WORKSPACE_BYTES of it from module load until the process exits, used or not.
+// In host code `g_static_ws` is only a handle for the runtime's symbol calls, never a device address: the address
+// this device gave the array comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_static_ws[TROPICAL_STATIC_WORKSPACE_BYTES];
+
+constexpr int kStaticWsDevices = 64;
+std::atomic<void*> g_static_ws_addr[kStaticWsDevices];  // per device: the array's address there, nullptr = not asked yet
+
+// Address of g_static_ws on the current device (looked up on the first call per device, remembered afterwards).
+int static_workspace(void** ws) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "mixed_attention_static: cudaGetDevice");
+    const bool cached = dev >= 0 && dev < kStaticWsDevices;
+    void* p = cached ? g_static_ws_addr[dev].load(std::memory_order_acquire) : nullptr;
+    if (p == nullptr) {
+        e = cudaGetSymbolAddress(&p, g_static_ws);
+        if (e != cudaSuccess) return cuda_fail(e, "mixed_attention_static: cudaGetSymbolAddress");
+        if (p == nullptr || ((uintptr_t)p & 255)) {
+            snprintf(g_cuda_err, sizeof g_cuda_err, "mixed_attention_static: static workspace address %p unusable", p);
+            return TROPICAL_ERR_CUDA;
+        }
+        if (cached) g_static_ws_addr[dev].store(p, std::memory_order_release);
+    }
+    *ws = p;
     return TROPICAL_OK;
 }
 
@@ -247,6 +281,34 @@ int tropical_mixed_attention(const tropical_kv_pool_t* pool, const tropical_batc
                                 (cudaStream_t)cuda_stream, &g_launches);
 }
 
+int tropical_mixed_attention_static(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* q,
+                                    void* out, float* lse, float sm_scale, void* cuda_stream) {
+    g_launches = 0;
+    int rc = check_pool(pool);
+    if (rc != TROPICAL_OK) return rc;
+    rc = check_batch(pool, batch);
+    if (rc != TROPICAL_OK) return rc;
+    if (batch->total_q == 0) return TROPICAL_OK;
+    if (q == nullptr || out == nullptr) return TROPICAL_ERR_INVALID_ARG;
+    // the size check comes before any CUDA call: a step that does not fit is refused, never run on a short array
+    const size_t need = tropical_workspace_bytes(pool, batch->num_reqs, batch->total_q, batch->max_kv_len);
+    if (need == 0 || need > (size_t)TROPICAL_STATIC_WORKSPACE_BYTES) {
+        snprintf(g_cuda_err, sizeof g_cuda_err,
+                 "mixed_attention_static: this step needs %zu bytes of scratch, the built-in array holds %zu "
+                 "(TROPICAL_STATIC_WORKSPACE_BYTES); use tropical_mixed_attention with a caller workspace",
+                 need, (size_t)TROPICAL_STATIC_WORKSPACE_BYTES);
+        return TROPICAL_ERR_STATIC_CAPACITY;
+    }
+    void* ws = nullptr;
+    rc = static_workspace(&ws);
+    if (rc != TROPICAL_OK) return rc;
+    // Nothing in the array has to be zero when the kernels start: the tile-directory kernel rewrites the header, both
+    // ticket counters and every split group's arrival counter it will use, and the split-K partials are written by
+    // the decode units before the combine reads them.  What the previous call left behind is never read.
+    return mixed_attention_impl(pool, batch, q, nullptr, nullptr, out, lse, sm_scale, ws,
+                                (size_t)TROPICAL_STATIC_WORKSPACE_BYTES, (cudaStream_t)cuda_stream, &g_launches);
+}
+
 int tropical_mixed_step(const tropical_kv_pool_t* pool, const tropical_batch_t* batch, const void* q, const void* k_new,
                         const void* v_new, void* out, float* lse, float sm_scale, void* workspace,
                         size_t workspace_bytes, void* cuda_stream) {
@@ -364,6 +426,8 @@ const char* tropical_status_string(int s) {
         case TROPICAL_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
         case TROPICAL_ERR_CUDA: return "CUDA failure";
         case TROPICAL_ERR_UNCALIBRATED: return "no cost-model coefficients for this shape";
+        case TROPICAL_ERR_STATIC_CAPACITY:
+            return "step needs more scratch than the built-in static workspace holds (TROPICAL_STATIC_WORKSPACE_BYTES)";
         default: return "unknown status";
     }
 }
