@@ -117,6 +117,9 @@ int tropical_kv_gather(const tropical_kv_pool_t *pool, const tropical_batch_t *b
  *     The call runs on the CURRENT device, which must own src_pool; dst_pool may live on a peer device whose memory
  *     is mapped here (tropical_enable_peer_access, cudaDeviceEnablePeerAccess or a VMM mapping): the source GPU then
  *     pushes over NVLink.  The two pools must not overlap in the pages the tables name.
+ *     STATUS OF THE PEER CASE: UNVERIFIED ON HARDWARE.  Every box this library has run on had one GPU, so bulk
+ *     stores into peer-mapped memory have never been compared with the oracle; the comparison is armed
+ *     (tests/test_gpu_migrate.py, the tests that need two GPUs) and runs on the first box that has them.
  *   Two requests of the list naming the same destination (page, slot) are undefined behaviour; page ids are not
  *   validated (device data).  Up to 1024 requests per launch; longer lists are split into several launches.
  * Returns INVALID_ARG for null pointers / negative sizes / strides smaller than ceil(max_kv_len / P) / mismatched pool

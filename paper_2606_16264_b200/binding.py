@@ -122,6 +122,10 @@ def lib():
     L.tropical_status_string.restype = ctypes.c_char_p
     L.tropical_last_cuda_error.restype = ctypes.c_char_p
     L.tropical_version.restype = ctypes.c_char_p
+    if b"WHATIF" in L.tropical_version() and "WHATIF" not in os.environ.get("TROPICAL_NVCC_EXTRA", ""):
+        # a measurement build whose attention results are wrong by design must be asked for, never picked up
+        raise ImportError(f"{path} is a what-if measurement build ({L.tropical_version().decode()}); "
+                          "rebuild without TROPICAL_NVCC_EXTRA, or set it to load this library on purpose")
     for name in ("tropical_kv_append", "tropical_kv_append_rope", "tropical_kv_gather", "tropical_kv_migrate", "tropical_enable_peer_access", "tropical_validate_batch", "tropical_mixed_attention", "tropical_mixed_attention_static", "tropical_mixed_step", "tropical_step_host",
                  "tropical_step_cost", "tropical_iter_cost", "tropical_last_launch_count", "tropical_debug_attention_simt",
                  "tropical_debug_read_profile"):

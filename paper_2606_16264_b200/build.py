@@ -9,6 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtropical.so")
+STAMP = LIB + ".flags"  # the extra nvcc flags the library on disk was built with (git-ignored, travels with the .so)
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 NVCC_FLAGS = [
@@ -24,8 +25,25 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
 
 
+def _extra_flags() -> list:
+    # e.g. -DTROPICAL_DEBUG_WAIT (names a timed-out mbarrier wait), -DTROPICAL_WHATIF_* / -DTROPICAL_TIMELINE (measurement builds)
+    return os.environ.get("TROPICAL_NVCC_EXTRA", "").split()
+
+
+def _built_flags():
+    try:
+        with open(STAMP) as f:
+            return f.read().split()
+    except OSError:
+        return None  # a library without a stamp: built by something else, taken as a plain build
+
+
 def _stale() -> bool:
     if not os.path.exists(LIB):
+        return True
+    # A measurement build (attention results wrong by design under -DTROPICAL_WHATIF_*) overwrites the same file:
+    # a change of the flag set forces a rebuild, so a later plain run never loads it by accident.
+    if (_built_flags() or []) != _extra_flags():
         return True
     t = os.path.getmtime(LIB)
     deps = sources() + glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.inc")) + \
@@ -38,7 +56,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + f".tmp{os.getpid()}"
-    extra = os.environ.get("TROPICAL_NVCC_EXTRA", "").split()  # e.g. -DTROPICAL_DEBUG_WAIT (names a timed-out mbarrier wait)
+    extra = _extra_flags()
     cmd = [nvcc] + NVCC_FLAGS + extra + ["-I", INCLUDE, "-o", tmp] + sources()
     res = subprocess.run(cmd, capture_output=True, text=True)
     log = res.stdout + res.stderr
@@ -50,6 +68,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if verbose:
         print(log)
     os.replace(tmp, LIB)
+    with open(STAMP, "w") as f:
+        f.write(" ".join(extra) + "\n")
     return LIB
 
 

@@ -95,9 +95,11 @@ __device__ __noinline__ void append_worker(const DecodeArgs& A) {
     for (;;) {
         // look before taking a ticket: at the end of a step every decode worker passes here, and ~1800 atomics on one
         // address would serialise the kernel's tail
-        if (*reinterpret_cast<volatile int*>(ticket) >= n_tickets) break;
-        int tk = 0;
-        if (lane == 0) tk = atomicAdd(ticket, 1);
+        // Lane 0 alone looks and takes; the warp leaves on the broadcast value.  (Every lane reading the counter for
+        // itself could see different values while other CTAs bump it, and lanes that left early would then be
+        // missing from the full-mask shuffles below.)
+        int tk = n_tickets;
+        if (lane == 0 && *reinterpret_cast<volatile int*>(ticket) < n_tickets) tk = atomicAdd(ticket, 1);
         tk = __shfl_sync(0xffffffffu, tk, 0);
         if (tk >= n_tickets) break;
         const int t0 = tk * kAppendTokens, nt = min(kAppendTokens, T - t0);

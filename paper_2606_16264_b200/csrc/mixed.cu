@@ -9,6 +9,7 @@
 #include "kernels.h"
 #include "plan.cuh"
 #include "prefill.cuh"
+#include "step_variant.h"
 #include "tma_host.h"
 
 namespace tropical {
@@ -105,6 +106,7 @@ mixed_kernel(PrefillArgs PA, DecodeArgs DA, const __grid_constant__ StepMaps TM)
         tmem_alloc(&PB->tmem_base, C::TM_COLS);
         tmem_relinquish();
     }
+    // (Invariant 2 of csrc/plan.cuh: keep it that way -- no global load or store above this line.)
     // Programmatic dependent launch: everything above (barriers, TMEM, descriptor prefetch) touches no global memory
     // and overlaps the tile-directory kernel and the tail of the append.  From here on the workspace and the pool are
     // read: wait until the directory kernel has completed -- which, by its own final griddepcontrol.wait, implies
@@ -252,11 +254,11 @@ void set_debug_fused(int mode) { g_fused_mode.store(mode < 0 ? -1 : (mode ? 1 : 
 // step to begin with.  The host sees only the scalars of the batch, not its contexts: a step is taken as
 // prefill-dominated when its requests carry at least kFusedMinTokensPerReq new tokens on average, i.e. when it has at
 // most one decode request per ~64 prefill tokens.
-constexpr int kFusedMinTokensPerReq = 64;
+// The rule itself lives in step_variant.h, shared with the step-cost model whose fits are keyed on it.
 static bool choose_fused(const BatchDesc& b) {
     const int mode = g_fused_mode.load(std::memory_order_relaxed);
     if (mode >= 0) return mode == 1;
-    return (long long)b.total_q >= (long long)kFusedMinTokensPerReq * b.num_reqs;
+    return step_is_prefill_dominated(b.total_q, b.num_reqs);
 }
 
 template <int D, bool FUSED>

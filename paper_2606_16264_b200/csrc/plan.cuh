@@ -108,6 +108,14 @@ __device__ __forceinline__ int plan_block_max(int v, int* s_warp) {
     return m;
 }
 
+// INVARIANTS of the three-kernel chain append -> plan_kernel -> step kernel (checked only by
+// tests/test_gpu_parity.py::test_append_then_attention_ordering_stress, so keep that test in the default suite):
+//   1. EVERY exit path of plan_kernel executes griddepcontrol.wait (the early return of the extra blocks below and
+//      the end of the kernel).  The step kernel's own griddepcontrol.wait covers only ITS prerequisite grid -- this
+//      one -- so the append's writes reach the step kernel only because this grid does not complete before the
+//      append has completed and flushed.  A return that skips the wait breaks that silently.
+//   2. The step kernel's prologue (everything before its griddepcontrol.wait, csrc/mixed.cu) must not load from or
+//      store to global memory: it may run while the append and this kernel are still writing.
 __global__ void __launch_bounds__(kPlanThreads) plan_kernel(BatchDesc b, int Hq, int Hkv, PlanPtrs P, int forced_split,
                                                             int row_pairs) {
     // the step kernel (a programmatic dependent of this one) may start its prologue now; it waits for this kernel's

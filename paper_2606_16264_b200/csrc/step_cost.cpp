@@ -6,17 +6,17 @@
 #include <stdint.h>
 
 #include "../../include/tropical.h"
+#include "step_variant.h"
 
 namespace {
 
 // One coefficient set per head shape and kernel variant of the step: tropical_mixed_step runs prefill-dominated steps
-// (at least kFusedMinTokensPerReq new tokens per request on average, csrc/mixed.cu) through its fused variant -- append
+// (at least kFusedMinTokensPerReq new tokens per request on average, csrc/step_variant.h) through its fused variant -- append
 // inside, two softmax warpgroups -- whose prefill role is up to 35 % faster; one closed form cannot follow that switch.
 struct BuiltinFit {
     int Hq, Hkv, d, fused;
     tropical_cost_model_t m;
 };
-constexpr int kFusedMinTokensPerReq = 64;  // must equal csrc/mixed.cu's
 
 // Coefficients fitted to measured step times by `python -m paper_2606_16264_b200.cost_fit fit` from the grid
 // that `... cost_fit measure` wrote on a B200 (calibration/b200_grid.csv; provenance in DESIGN.md section 7).
@@ -84,7 +84,7 @@ extern "C" int tropical_step_cost(const tropical_cost_model_t* model, int32_t Hq
         if (q_lens[i] < 0 || ctx_lens[i] < 0) return TROPICAL_ERR_INVALID_ARG;
     long long T = 0;
     for (int i = 0; i < num_reqs; ++i) T += q_lens[i];
-    const int fused = (num_reqs > 0 && T >= (long long)kFusedMinTokensPerReq * num_reqs) ? 1 : 0;
+    const int fused = tropical::step_is_prefill_dominated(T, num_reqs) ? 1 : 0;
     tropical_cost_breakdown_t f;
     features(Hq, Hkv, d, P, num_reqs, q_lens, ctx_lens, fused != 0, &f);
     if (model == nullptr) {

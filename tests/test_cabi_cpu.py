@@ -189,3 +189,17 @@ def test_builtin_linear_model_reproduces_measured_gemms():
     us2, bd2 = tb.iter_cost(tb.LayerShape(5120, 13824, 1, 40, 2), Hq, Hkv, d, P, q.tolist(), c.tolist())
     assert bd2.attn_us < bd1.attn_us and bd2.linear_us < bd1.linear_us and us2 < us1
     assert us1 == pytest.approx(40 * (bd1.attn_us + bd1.linear_us))
+
+
+def test_change_of_build_flags_forces_a_rebuild(monkeypatch):
+    """A measurement build (TROPICAL_NVCC_EXTRA=-DTROPICAL_WHATIF_..., results wrong by design) overwrites
+    libtropical.so; the flag set it was built with is stamped beside it, so a later run with other flags rebuilds."""
+    from paper_2606_16264_b200 import build
+    monkeypatch.delenv("TROPICAL_NVCC_EXTRA", raising=False)
+    tb.lib()
+    assert not build._stale()
+    monkeypatch.setenv("TROPICAL_NVCC_EXTRA", "-DTROPICAL_TIMELINE")
+    assert build._stale()
+    monkeypatch.delenv("TROPICAL_NVCC_EXTRA")
+    assert not build._stale()
+    assert b"WHATIF" not in tb.lib().tropical_version()

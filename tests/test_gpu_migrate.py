@@ -116,3 +116,104 @@ def test_migrate_rejects_mismatched_pools():
         tb.kv_migrate(tb.KVPool(a, a.clone(), 2), tb.KVPool(b, b.clone(), 4), lens, pt, pt, 1)
     with pytest.raises(tb.TropicalError):
         tb.kv_migrate(tb.KVPool(a, a.clone(), 2), tb.KVPool(a.clone(), a.clone(), 2), lens, pt, pt, 40)  # stride < pages
+
+
+# ------------------------------------------------------------------ the GPU-to-GPU hop (needs a second GPU)
+def _two_gpus():
+    return torch.cuda.is_available() and torch.cuda.device_count() >= 2
+
+
+needs_two_gpus = pytest.mark.skipif(not _two_gpus(), reason="KV migration to a peer GPU needs 2 visible GPUs (P:155 Path 1, P:171)")
+
+
+def _peer_migration(d0, d1):
+    """Body of the peer test; (d0, d1) = (0, 0) runs the same code on one GPU (how it was exercised before any 2-GPU box)."""
+    with torch.cuda.device(d0):
+        if not tb.enable_peer_access(d1):
+            pytest.skip(f"no peer path between cuda:{d0} and cuda:{d1}")
+        s = synth.make_step(np.random.default_rng(90), 16, 4, 128, 16, [1, 1, 1, 1, 40], [700, 16, 2500, 63, 130])
+        ref, _, kp, vp = oracle.step(s)
+        dev = DeviceStep(s)
+        out_src, _ = dev.step()
+        L = (s.q_lens + s.ctx_lens).tolist()
+        Hkv, P, d = s.num_kv_heads, s.page_size, s.head_dim
+        dst_pt, n_dst = synth.make_migration_target(np.random.default_rng(91), L, P)
+        kd_ref = np.full((n_dst, Hkv, P, d), synth.POISON_BF16, np.uint16)
+        vd_ref = kd_ref.copy()
+        oracle.kv_migrate(kp, vp, kd_ref, vd_ref, L, s.page_table, dst_pt)
+        k_dst = torch.full((n_dst, Hkv, P, d), synth.POISON_BF16, dtype=torch.int16, device=f"cuda:{d1}")
+        v_dst = k_dst.clone()
+        torch.cuda.synchronize(d1)
+        dst = tb.KVPool(k_dst, v_dst, s.num_q_heads)
+        tb.kv_migrate(dev.pool, dst, torch.tensor(np.asarray(L, np.int32), device=f"cuda:{d0}"), to_dev(s.page_table),
+                      to_dev(dst_pt), int(max(L)))
+        torch.cuda.synchronize(d0)
+        assert np.array_equal(bits(k_dst), kd_ref), "peer destination K pool differs from the oracle's"
+        assert np.array_equal(bits(v_dst), vd_ref), "peer destination V pool differs from the oracle's"
+        assert np.array_equal(bits(dev.k_pool), kp) and np.array_equal(bits(dev.v_pool), vp), "source was written"
+        out0 = bits(dev.out).copy()
+    with torch.cuda.device(d1):  # the request now decodes on the destination worker
+        to1 = lambda t: t.to(f"cuda:{d1}")
+        batch = tb.Batch(to1(dev.batch.q_lens), to1(dev.batch.ctx_lens), to1(dev.batch.q_offsets),
+                         torch.from_numpy(dst_pt).to(f"cuda:{d1}"), s.total_q, s.max_kv_len)
+        q1 = to1(dev.q)
+        out1 = torch.zeros_like(q1)
+        tb.mixed_attention(dst, batch, q1, out=out1)
+        torch.cuda.synchronize(d1)
+        assert np.array_equal(bits(out1), out0)
+    assert np.abs(out_src - ref).max() <= 2e-2
+
+
+def _head_shards(d0, d1):
+    s = synth.make_step(np.random.default_rng(92), 16, 4, 128, 16, [300, 1, 1, 1, 17], [200, 4097, 513, 15, 0])
+    tb.debug_set_split_pages(32)  # the automatic split size depends on the head count: pin the split boundaries equal
+    try:
+        with torch.cuda.device(d0):
+            full = DeviceStep(s)
+            full.step(impl="product")
+            want = bits(full.out).copy()
+        Hq, Hkv = s.num_q_heads, s.num_kv_heads
+        shards = []
+        for r, dv in enumerate((d0, d1)):
+            hq = slice(r * Hq // 2, (r + 1) * Hq // 2)
+            hk = slice(r * Hkv // 2, (r + 1) * Hkv // 2)
+            sh = synth.StepInputs(s.name, s.seed, Hq // 2, Hkv // 2, s.head_dim, 16, s.num_pages, s.q_lens, s.ctx_lens,
+                                  s.q_offsets, s.page_table, np.ascontiguousarray(s.k_pool[:, hk]),
+                                  np.ascontiguousarray(s.v_pool[:, hk]), np.ascontiguousarray(s.q[:, hq]),
+                                  np.ascontiguousarray(s.k_new[:, hk]), np.ascontiguousarray(s.v_new[:, hk]))
+            with torch.cuda.device(dv):
+                shards.append(DeviceStep(sh))
+        for dv, dev in zip((d0, d1), shards):  # both GPUs busy at once: enqueue on each, then wait for both
+            with torch.cuda.device(dv):
+                dev.append()
+                dev.attention()
+        for dv in (d0, d1):
+            torch.cuda.synchronize(dv)
+        got = np.concatenate([bits(dev.out) for dev in shards], axis=1)
+        assert np.array_equal(got, want)
+    finally:
+        tb.debug_set_split_pages(0)
+
+
+@needs_two_gpus
+def test_peer_migration_whole_destination_pool_bit_exact_and_attention_on_the_peer():
+    """Source pool on cuda:0, destination pool on cuda:1, mapped into cuda:0 by tropical_enable_peer_access; the kernel
+    runs on cuda:0 and its bulk stores land in peer memory over NVLink.  Destination bit-identical to oracle.kv_migrate
+    over the whole pool, source untouched, and the same decode step on cuda:1 over the migrated cache gives the bits
+    cuda:0 gives over the original.  NEVER RUN on two GPUs so far (every box this suite has seen had one); the body was
+    run with both roles on one GPU."""
+    _peer_migration(0, 1)
+
+
+@needs_two_gpus
+def test_head_shards_on_two_gpus_concatenate_to_the_unsharded_step():
+    """TP = 2 inside a worker: kv heads [0, Hkv/2) with their q heads on cuda:0, the rest on cuda:1, both steps
+    enqueued before either is waited for; the concatenated outputs equal the one-GPU step bit for bit."""
+    _head_shards(0, 1)
+
+
+def test_two_gpu_test_bodies_on_one_gpu():
+    """The bodies of the two tests above with both roles on cuda:0, so that the code a 2-GPU box will run for the first
+    time has at least run (same kernels, no NVLink hop)."""
+    _peer_migration(0, 0)
+    _head_shards(0, 0)

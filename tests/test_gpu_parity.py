@@ -510,3 +510,19 @@ def test_validate_batch_finds_the_first_bad_request():
     dev.batch.q_offsets[2] -= 1
     dev.batch.ctx_lens[4] = -1
     assert tb.validate_batch(dev.pool, dev.batch) == 4
+
+
+def test_predictor_and_launcher_agree_on_the_step_variant():
+    """The built-in cost fits are keyed on the kernel variant tropical_mixed_step picks (csrc/step_variant.h, one rule for
+    both).  Either side of the rule's boundary: the launcher's choice shows in its launch count (2 = fused variant,
+    3 = append kernel + plain variant), the predictor's in the critical-path feature of an MHA prefill item (the fused
+    variant pairs the top two row tiles of a head: 3 + 2 KV iterations; the plain one takes the top tile alone: 3)."""
+    for q0, fused in ((316, True), (315, False)):  # 4 decode requests: T = q0 + 4 against 64 * 5
+        q_lens, ctx_lens = [q0, 1, 1, 1, 1], [0, 40, 300, 17, 5]
+        s = _step(50, 8, 8, 128, q_lens, ctx_lens)
+        dev = DeviceStep(s)
+        dev.fused_step()
+        torch.cuda.synchronize()
+        assert tb.last_launch_count() == (2 if fused else 3)
+        _, bd = tb.step_cost(8, 8, 128, 16, q_lens, ctx_lens, require_model=False)  # features only: no fit for 8/8
+        assert bd.prefill_critical_iters == (5 if fused else 3)
