@@ -174,6 +174,18 @@ def max_over_ranks(value: float, world: int, device) -> float:
     return float(t.item())
 
 
+def gather_over_ranks(value: float, world: int, device) -> list:
+    """Every rank's figure, in rank order (reported beside the maximum)."""
+    if world <= 1:
+        return [float(value)]
+    import torch
+    import torch.distributed as dist
+    mine = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    parts = [torch.zeros_like(mine) for _ in range(world)]
+    dist.all_gather(parts, mine)
+    return [float(p.item()) for p in parts]
+
+
 def whole_job_tokens_per_s(new_tokens_per_replica: float, world: int, us_per_step: float) -> float:
     """Aggregate over all replicas (weak scaling: every rank runs its own copy of the workload)."""
     return new_tokens_per_replica * world / (us_per_step * 1e-6)
@@ -473,6 +485,7 @@ def run_ours(args, rank, world):
             st.one_step()
         torch.cuda.synchronize()
     clocks = sampler.finish()
+    per_rank_us = [round(ms / args.steps * 1e3, 2) for ms in gather_over_ranks(total_ms, world, "cuda")]
     total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms / args.steps
     us = ms_per_step * 1e3
@@ -511,6 +524,7 @@ def run_ours(args, rank, world):
                        if st.launches_per_step == 2 else
                        "decode-heavy step: its append kernel in front of the plain step kernel (3 launches)")),
         "tokens_per_s": round(whole_job_tokens_per_s(cnt["new_tokens"], world, us), 1),
+        "per_rank_us": per_rank_us,  # value = their maximum
         "us_per_step": {"mean_timed_region": round(us, 2), "median": round(float(np.median(step_us)), 2),
                         "min": round(float(step_us.min()), 2), "max": round(float(step_us.max()), 2),
                         "of": f"{n_k} per-step event pairs, second pass (rank 0)"},
@@ -686,6 +700,45 @@ def run_reference(args, rank, world):
     }))
 
 
+def launch_ranks(args) -> int:
+    """`python bench.py --gpus N` without torchrun around it: start N ranks of this same command line, one GPU each
+    (torch.distributed.run sets RANK / LOCAL_RANK / WORLD_SIZE / MASTER_*; NCCL carries only the timing reductions).
+    Refuses instead of quietly measuring fewer replicas than asked for.  P:184: 8 GPUs per node, P:186 request dispatch
+    over independent workers -- the replicas share nothing."""
+    import socket
+    import subprocess
+    if args.impl == "ours" and not args.rank_check:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            print(f"bench.py: --gpus {args.gpus} asked for, {have} CUDA device(s) visible: refusing to run fewer "
+                  "replicas under the same label", file=sys.stderr)
+            return 2
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def rank_check(rank: int, world: int) -> None:
+    """The rank plumbing of the timed legs with no GPU in it: every rank reports a made-up step time (slower with
+    rank), the job's time is the maximum, its throughput the sum over replicas; rank 0 prints one JSON line."""
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+    mine = 100.0 + 25.0 * rank
+    per_rank = gather_over_ranks(mine, world, "cpu")
+    us = max_over_ranks(mine, world, "cpu")
+    print(f"rank {rank} of {world}: {mine} us", file=sys.stderr, flush=True)
+    if rank == 0:
+        print(json.dumps({"rank_check": True, "n_gpus": world, "per_rank_us": per_rank, "value": us, "unit": UNIT,
+                          "tokens_per_s": whole_job_tokens_per_s(60, world, us), "scaling": "weak"}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -700,9 +753,18 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-extra", action="store_true", help="skip extra.C4 / extra.MIG on the default run")
     ap.add_argument("--sustain-seconds", type=float, default=2.0, help="length of the sustained loop (0 = skip)")
+    ap.add_argument("--rank-check", action="store_true",
+                    help="launcher check without GPU work: the ranks rendezvous over gloo, reduce a made-up time and "
+                         "rank 0 prints the line's rank bookkeeping (what the CPU test of --gpus N drives)")
     args = ap.parse_args()
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        sys.exit(launch_ranks(args))
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
+    if world != max(args.gpus, 1) and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; running {world} ranks", file=sys.stderr)
+    if args.rank_check:
+        return rank_check(rank, world)
     if args.impl == "reference":
         run_reference(args, rank, world)
     else:

@@ -66,3 +66,30 @@ def test_single_rank_reduction_is_identity():
     import bench
     assert bench.max_over_ranks(3.5, 1, "cpu") == 3.5
     assert bench.whole_job_tokens_per_s(60, 1, 100.0) == pytest.approx(6e5)
+
+
+def test_bench_gpus_flag_starts_that_many_ranks():
+    """`python bench.py --gpus 2` with no torchrun around it starts two ranks itself (the launcher the GPU legs use;
+    --rank-check swaps the GPU work for a made-up time and NCCL for gloo, everything else is the same path)."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--rank-check"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                     # rank 0 alone prints the JSON line
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["per_rank_us"] == [100.0, 125.0] and line["value"] == 125.0
+    assert line["tokens_per_s"] == pytest.approx(2 * 60 / 125e-6)
+    assert "rank 0 of 2" in res.stderr and "rank 1 of 2" in res.stderr
+
+
+def test_bench_refuses_more_gpus_than_visible():
+    import subprocess
+    n = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", str(n + 2), "--steps", "1"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert res.returncode == 2 and "refusing" in res.stderr
+    assert not [l for l in res.stdout.splitlines() if l.startswith("{")]
