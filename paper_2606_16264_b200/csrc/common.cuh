@@ -135,6 +135,34 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+// try_wait with a suspend-time hint: the hardware may park the thread for up to `ns` nanoseconds before it reports
+// "not yet" (PTX ISA, mbarrier.try_wait, suspendTimeHint); a parked warp issues nothing.
+__device__ __forceinline__ bool mbar_try_wait_hint(uint64_t* bar, uint32_t parity, uint32_t ns) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(ns)
+        : "memory");
+    return ok != 0;
+}
+// Spin policy of mbar_wait's slow path (A/B record: profiles/r3_wait_spin.md):
+//   0 = round 2: try_wait + clock64() + 64-bit compare on every iteration (9 SASS instructions per spin)
+//   1 = no clock read in the loop: iterations are counted and the deadline is looked at every 2^14 of them
+//   2 = 1 + suspend-time hint on the try_wait
+//   3 = 2 + nanosleep back-off on the long waits (decode ring, producer slot, MMA waiting for P)
+//   4 = 1 + one clock read per iteration, its value unused (policy 0's pacing without its compare); 5 = two reads
+// Policy 0 stays the product's: every alternative measured 1-5 % SLOWER on C5, burst and sustained, although each
+// raised the SM clock the board holds at its power limit (fewer instructions per spin, but more cycles per step).
+#ifndef TROPICAL_WAIT_V
+#define TROPICAL_WAIT_V 0
+#endif
+#ifndef TROPICAL_WAIT_HINT_NS
+#define TROPICAL_WAIT_HINT_NS 2000
+#endif
+
 #ifdef TROPICAL_WAIT_PROF
 // Measurement build only (-DTROPICAL_WAIT_PROF): cycles and calls of every mbar_wait, by tag (lane 0 of each warp).
 static __device__ unsigned long long g_wait_cycles[512];
@@ -155,6 +183,47 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int ta
 #ifdef TROPICAL_WAIT_PROF
     const long long tp = clock64();
 #endif
+#if TROPICAL_WAIT_V >= 1 && !defined(TROPICAL_DEBUG_WAIT)
+    if (!mbar_try_wait(bar, parity)) {
+        // Most of a step's waits end here within a few tries, and the step is bound by board power: the loop holds
+        // nothing but the try, a counter and the branch.  The deadline (a protocol bug traps instead of hanging the
+        // GPU) costs a clock read once per 2^14 tries.
+        long long t0 = 0;
+        bool ok = false;
+        do {
+#pragma unroll 1
+            for (uint32_t spins = 0; spins < 0x4000u; ++spins) {
+#if TROPICAL_WAIT_V == 2 || TROPICAL_WAIT_V == 3
+                ok = mbar_try_wait_hint(bar, parity, TROPICAL_WAIT_HINT_NS);
+#else
+                ok = mbar_try_wait(bar, parity);
+#endif
+                if (ok) break;
+#if TROPICAL_WAIT_V == 3
+                if ((tag == 201 || tag == 202 || tag == 103 || tag == 109) && spins >= 4) __nanosleep(64);
+#endif
+#if TROPICAL_WAIT_V == 4 || TROPICAL_WAIT_V == 5
+                {   // policy 1 paced like policy 0: the clock read(s) without the compare
+                    long long dummy;
+                    asm volatile("mov.u64 %0, %%clock64;" : "=l"(dummy));
+#if TROPICAL_WAIT_V == 5
+                    asm volatile("mov.u64 %0, %%clock64;" : "=l"(dummy));
+#endif
+                }
+#endif
+            }
+#ifndef TROPICAL_NO_WAIT_TRAP
+            if (!ok) {
+                // ~20 s at 1.9 GHz: far beyond any legitimate wait even under time-slicing or MPS (a step takes < 1 ms);
+                // build with -DTROPICAL_NO_WAIT_TRAP to wait forever (debugger sessions)
+                const long long now = clock64();
+                if (t0 == 0) t0 = now;
+                else if (now - t0 > 40000000000LL) __trap();
+            }
+#endif
+        } while (!ok);
+    }
+#else
     if (!mbar_try_wait(bar, parity)) {
         long long t0 = clock64();
         while (!mbar_try_wait(bar, parity)) {
@@ -195,6 +264,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int ta
 #endif
         }
     }
+#endif  // TROPICAL_WAIT_V
 #ifdef TROPICAL_WAIT_PROF
     if ((threadIdx.x & 31) == 0) {
         atomicAdd(&g_wait_cycles[tag & 511], (unsigned long long)(clock64() - tp));
