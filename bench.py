@@ -66,15 +66,32 @@ def load_peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
 
 
+KERNEL_SOURCES = ("common.cuh", "decode.cuh", "mixed.cu", "plan.cuh", "prefill.cuh", "kv_append.cu", "step_variant.h")
+
+
+def kernel_source_sha() -> str:
+    """Fingerprint of the step's kernel sources as they are on disk (`python bench.py --kernel-sha` prints it): an ncu
+    capture is only quoted for the kernels it was taken from."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2606_16264_b200", "csrc", name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()[:12]
+
+
 def ncu_traffic(config: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one launch, from the committed ncu capture
-    of this config (profiles/ncu_traffic.csv; the .md beside it names the command); None when there is none."""
+    of this config (profiles/ncu_traffic.csv: config, bytes, capture file, kernel_source_sha at capture time; the .md
+    beside it names the command).  None when there is no capture of THESE kernel sources: a capture of an older kernel
+    is not quoted."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(path):
         return None
+    sha = kernel_source_sha()
     for line in open(path):
         f = line.strip().split(",")
-        if f and f[0] == config:
+        if len(f) >= 4 and f[0] == config and f[3] == sha:
             return float(f[1])
     return None
 
@@ -289,6 +306,20 @@ class StepTimer:
         e1.record(self.stream)
         torch.cuda.synchronize()
         return sum(a.elapsed_time(b) for a, b in st) if self.flush else e0.elapsed_time(e1)
+
+    def timed_warm(self, steps):
+        """Small configs only: the same per-step event pairs as `timed`, WITHOUT the L2 flush in between -- the step's
+        working set (pages, q, workspace) is still in the 126 MB L2 from the step before.  Returns ms for `steps` steps."""
+        torch = self.torch
+        ev = lambda: torch.cuda.Event(enable_timing=True)
+        st = [(ev(), ev()) for _ in range(steps)]
+        torch.cuda.synchronize()
+        for k in range(steps):
+            st[k][0].record(self.stream)
+            self.one_step()
+            st[k][1].record(self.stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in st)
 
     def instrumented(self, steps):
         """Second pass over the same steps with events around every step and between its two calls: per-step times
@@ -553,9 +584,17 @@ def run_ours(args, rank, world):
         "gpu_launches": int(st.launches_per_step) * args.steps,
         "clocks": clocks,
         "gen_seconds": round(gen_s, 1),
-        "role_finish_us": dict({k: round(v / 1e3, 1) for k, v in roles.items()},
-                               launch="last step kernel of the second (instrumented) pass"),
+        "role_finish_us": (dict({k: round(v / 1e3, 1) for k, v in roles.items()},
+                                launch="last step kernel of the second (instrumented) pass") if roles is not None else
+                           "not stamped: product build (measurement builds: TROPICAL_NVCC_EXTRA=-DTROPICAL_ROLE_PROF)"),
     }
+    if st.launches_per_step == 3:  # row A1 on its own: the append kernel between its two events of the second pass
+        app_us = float(np.median(step_us - attn_us))
+        app_bytes = cnt["step_bytes"] - cnt["attn_bytes"]
+        line["append_kernel"] = {"us": round(app_us, 2), "bytes": app_bytes, "gbs": round(app_bytes / (app_us * 1e3), 1),
+                                 "frac_of_hbm_peak": round(app_bytes / (app_us * 1e3) / peaks["hbm_gbs"], 4),
+                                 "of": f"median over {n_k} event pairs of the second pass (includes the event and launch gaps around an "
+                                       "11 us kernel: profiles/r3b_final.md has its ncu time); bytes = rows read + rows written"}
     if sus is not None:
         line["sustained"] = {"value": round(sus["us"], 2), "unit": UNIT, "frac": round(t_roof / sus["us"], 4),
                              "steps": sus["steps"], "clocks": sus["clocks"],
@@ -615,11 +654,42 @@ def run_extras(args, tb, torch, peaks, local, st_c5):
         n3 = min(steps, 50)
         us = st.timed(n3) * 1e3 / n3
         _, _, t_roof, t_nom = roofline_times(st.cnt, peaks)
+        warm_us = st.timed_warm(n3) * 1e3 / n3
         extra["C3"] = {"workload": f"C3 ({describe('C3')})", "value": round(us, 2), "unit": UNIT, "steps": n3,
                        "frac": round(t_roof / us, 4), "t_roof_us": round(t_roof, 2), "launches_per_step": st.launches_per_step,
-                       "l2": "flushed between timed steps"}
+                       "l2": "flushed between timed steps", "warm_l2": {"value": round(warm_us, 2), "frac": round(t_roof / warm_us, 4)}}
     except Exception as exc:
         extra["C3"] = {"error": repr(exc)}
+    try:  # the decode-only config (bandwidth bound; 1.33 GB per step, no flush needed)
+        s2, _ = make_workload("C2", 0)
+        st = StepTimer(s2, tb, torch)
+        st.warm(3)
+        sampler = ClockSampler(local)
+        sampler.start()
+        us = st.timed(steps) * 1e3 / steps
+        step_us, attn_us = st.instrumented(min(steps, 50))
+        clk = sampler.finish()
+        _, _, t_roof, t_nom = roofline_times(st.cnt, peaks)
+        extra["C2"] = {"workload": f"C2 ({describe('C2')})", "value": round(us, 2), "unit": UNIT, "steps": steps,
+                       "frac": round(t_roof / us, 4), "frac_of_nominal_peaks": round(t_nom / us, 4),
+                       "t_roof_us": round(t_roof, 2), "median": round(float(np.median(step_us)), 2),
+                       "min": round(float(step_us.min()), 2), "kernel_us": round(float(np.median(attn_us)), 2),
+                       "launches_per_step": st.launches_per_step, "clocks": clk}
+    except Exception as exc:
+        extra["C2"] = {"error": repr(exc)}
+    try:  # the tiny config: launch-latency bound; cold and warm L2 separately
+        s1, _ = make_workload("C1", 0)
+        st = StepTimer(s1, tb, torch)
+        st.warm(3)
+        n1 = min(steps, 50)
+        us = st.timed(n1) * 1e3 / n1
+        warm_us = st.timed_warm(n1) * 1e3 / n1
+        _, _, t_roof, _ = roofline_times(st.cnt, peaks)
+        extra["C1"] = {"workload": f"C1 ({describe('C1')})", "value": round(us, 2), "unit": UNIT, "steps": n1,
+                       "frac": round(t_roof / us, 4), "t_roof_us": round(t_roof, 3), "launches_per_step": st.launches_per_step,
+                       "l2": "flushed between timed steps", "warm_l2": {"value": round(warm_us, 2), "frac": round(t_roof / warm_us, 4)}}
+    except Exception as exc:
+        extra["C1"] = {"error": repr(exc)}
     return extra
 
 
@@ -683,11 +753,12 @@ def run_reference(args, rank, world):
     _, _, cores, dt0 = oracle_sample_us(s, budget_rows_flops=2e8, seed=12345)  # calibrate rows/s
     per_step_s = min(10.0, max(0.05, 90.0 / max(1, args.steps + args.warmup)))
     budget = max(2e7, 2e8 * per_step_s / max(dt0, 1e-3))
-    vals, desc = [], ""
+    vals, secs, desc = [], [], ""
     for k in range(args.warmup + args.steps):
-        us, desc, cores, _ = oracle_sample_us(s, budget_rows_flops=budget, seed=k)
+        us, desc, cores, dt = oracle_sample_us(s, budget_rows_flops=budget, seed=k)
         if k >= args.warmup:
             vals.append(us)
+            secs.append(dt)
     us = float(np.mean(vals)) if vals else float("nan")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": round(us, 1), "unit": UNIT, "n_gpus": world,
@@ -697,6 +768,9 @@ def run_reference(args, rank, world):
                                                           s.ctx_lens)), world),
         "cpu_baseline": {"value": round(us, 1), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": round(us, 1), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        # value / ms_per_step are whole-step figures EXTRAPOLATED by FLOP ratio from a bounded sample of rows per "step":
+        # steps x ms_per_step is therefore not the wall time of this run, sample_seconds x steps (+ the appends) is
+        "sampled": True, "sample_seconds": round(float(np.mean(secs)), 3) if secs else None,
     }))
 
 
@@ -756,7 +830,11 @@ def main():
     ap.add_argument("--rank-check", action="store_true",
                     help="launcher check without GPU work: the ranks rendezvous over gloo, reduce a made-up time and "
                          "rank 0 prints the line's rank bookkeeping (what the CPU test of --gpus N drives)")
+    ap.add_argument("--kernel-sha", action="store_true", help="print the fingerprint of the kernel sources and exit")
     args = ap.parse_args()
+    if args.kernel_sha:
+        print(kernel_source_sha())
+        return
     if "WORLD_SIZE" not in os.environ and args.gpus > 1:
         sys.exit(launch_ranks(args))
     rank = int(os.environ.get("RANK", 0))

@@ -170,10 +170,13 @@ def debug_wait_profile(reset: bool = True):
 
 def debug_read_profile(workspace: torch.Tensor, stream=None):
     """Role timestamps (ns, relative to kernel start) of the last fused step kernel run with `workspace`:
-    dict(prefill_done, decode_done, late_decode_done); 0 = that role never ran."""
+    dict(prefill_done, decode_done, late_decode_done); 0 = that role never ran.  None unless the library was built
+    with -DTROPICAL_ROLE_PROF (the product kernel carries no stamps)."""
     out = (ctypes.c_uint64 * 4)()
     _check(lib().tropical_debug_read_profile(_ptr(_aligned(workspace)), out, _stream(stream)), "debug_read_profile")
     t0 = int(out[0])
+    if t0 == 2 ** 64 - 1:  # the tile directory's initial value: nobody stamped the kernel start
+        return None
     rel = lambda v: int(v) - t0 if int(v) else 0
     return {"prefill_done": rel(out[1]), "decode_done": rel(out[2]), "late_decode_done": rel(out[3])}
 

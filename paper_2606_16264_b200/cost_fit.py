@@ -267,7 +267,7 @@ def predict(theta, X, n_sm=148.0):
 # Physical lower bounds of the two roofline coefficients (nominal peaks of the part: 2250 TFLOP/s dense bf16,
 # 8 TB/s HBM3e): a fit below them would predict steps faster than the hardware can run.  The measured copy figure of
 # MEASURED_PEAKS.json is not used here: it is a read + write mix, and the step kernel has been measured above it on
-# pure reads (6.8 TB/s of DRAM reads on C4, profiles/r1f_final.md).
+# pure reads (6.8 TB/s of DRAM reads on C4, profiles/r3b_final.md).
 A_MIN_US_PER_FLOP = 1e6 / 2250e12
 B_MIN_US_PER_BYTE = 1e6 / 8000e9
 
