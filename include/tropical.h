@@ -294,7 +294,8 @@ int tropical_step_cost(const tropical_cost_model_t *model, int32_t num_q_heads,
  *   all-reduce (tp > 1)   : two per layer over T d_model bf16 values: 2 (ar0 + ar_b * 2 T d_model).
  *   total = num_layers * (attention + linear + all-reduce).
  * linear == NULL selects the built-in fit of `python -m paper_2606_16264_b200.cost_fit measure-gemm | fit` (library
- * GEMMs on a B200; its all-reduce coefficients are 0: one GPU is all that could be measured).
+ * GEMMs on a B200; its all-reduce coefficients are 0: one GPU is all that could be measured, DESIGN.md section 7;
+ * `python -m paper_2606_16264_b200.cost_fit measure-allreduce` on a box with two GPUs, then `... cost_fit fit`, fills them in).
  * attn == NULL selects the built-in step model of the SHARD shape, else TROPICAL_ERR_UNCALIBRATED.  No norms, RoPE,
  * sampling or embedding: the form is this build's (parity unpinned, like row A6).
  * INVALID_ARG: null shape, non-positive sizes, tp not dividing num_kv_heads / d_ffn, and whatever tropical_step_cost

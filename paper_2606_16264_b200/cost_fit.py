@@ -3,6 +3,7 @@
     python -m paper_2606_16264_b200.cost_fit measure [--out calibration/b200_grid.csv]   # needs a B200
     python -m paper_2606_16264_b200.cost_fit measure-gemm [--out calibration/b200_gemm.csv]   # needs a B200
     python -m paper_2606_16264_b200.cost_fit sweep-split  [--out split_sweep.csv]             # needs a B200
+    python -m paper_2606_16264_b200.cost_fit measure-allreduce [--world 2]                    # needs >= 2 B200s (NCCL)
     python -m paper_2606_16264_b200.cost_fit fit     [--grid calibration/b200_grid.csv]  # CPU only
 
 `measure` times the step -- tropical_mixed_step: KV append + attention in one call -- (CUDA events, inputs resident) over a grid of synthetic batches --
@@ -27,6 +28,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 DEFAULT_GRID = os.path.join(HERE, "calibration", "b200_grid.csv")
 FIT_INC = os.path.join(HERE, "csrc", "cost_model_fit.inc")
 LINEAR_INC = os.path.join(HERE, "csrc", "linear_model_fit.inc")
+ALLREDUCE_GRID = os.path.join(HERE, "calibration", "b200_allreduce.csv")
 
 SHAPES = [(32, 32, 128), (40, 40, 128), (64, 8, 128),      # BASELINE.json configs[1..4]
           (20, 20, 128), (32, 4, 128)]                      # their TP = 2 head shards (NEXT-4)
@@ -359,6 +361,107 @@ def fit_linear(rows):
                        max_held=float(rel[~train].max()), max_all=float(rel.max()))
 
 
+# ------------------------------------------------------------------------------------------ all-reduce (NEXT-4, TP = 2)
+ALLREDUCE_COLUMNS = ["world", "backend", "bytes", "us_median", "us_min"]
+ALLREDUCE_D_MODEL = (4096, 5120, 8192)   # hidden sizes of the paper's model family; the payload is T x d_model bf16
+
+
+def allreduce_sizes(max_tokens: int):
+    """Payload bytes of the per-layer activations all-reduce of a tensor-parallel worker: T x d_model x 2."""
+    sizes, t = set(), 1
+    while t <= max_tokens:
+        for dm in ALLREDUCE_D_MODEL:
+            sizes.add(t * dm * 2)
+        t *= 2
+    return sorted(sizes)
+
+
+def measure_allreduce(out_path: str, iters: int, world: int, backend: str, max_tokens: int) -> int:
+    """Times sum-all-reduces of bf16 payloads across `world` ranks and writes one CSV row per size (rank 0).  Started
+    without a launcher it starts its own ranks (torch.distributed.run, one GPU per rank).  backend "nccl" is the
+    measurement (needs `world` GPUs; refused otherwise); "gloo" runs the same plumbing on CPU tensors so that the command
+    can be tested without GPUs -- `fit` ignores its rows."""
+    import torch
+    if "WORLD_SIZE" not in os.environ:
+        import socket
+        import subprocess
+        if backend == "nccl":
+            have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+            if have < world:
+                print(f"measure-allreduce: {world} GPUs needed for the NCCL measurement, {have} visible", file=sys.stderr)
+                return 2
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0))
+            port = so.getsockname()[1]
+        return subprocess.call([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={world}",
+                                "--master-addr", "127.0.0.1", "--master-port", str(port), "-m",
+                                "paper_2606_16264_b200.cost_fit", "measure-allreduce", "--out", out_path, "--iters",
+                                str(iters), "--world", str(world), "--backend", backend, "--max-tokens", str(max_tokens)])
+    import time
+    import torch.distributed as dist
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    cuda = backend == "nccl"
+    if cuda:
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
+    dist.init_process_group(backend)
+    dev = "cuda" if cuda else "cpu"
+    rows = []
+    for nbytes in allreduce_sizes(max_tokens):
+        x = torch.ones(nbytes // 2, dtype=torch.bfloat16, device=dev)
+        for _ in range(3):
+            dist.all_reduce(x)
+        per = []
+        for _ in range(iters):
+            x.fill_(1.0)
+            dist.barrier()
+            if cuda:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                dist.all_reduce(x)
+                e1.record()
+                torch.cuda.synchronize()
+                us = e0.elapsed_time(e1) * 1e3
+            else:
+                t0 = time.perf_counter()
+                dist.all_reduce(x)
+                us = (time.perf_counter() - t0) * 1e6
+            t = torch.tensor([us], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)   # the collective is done when its slowest rank is
+            per.append(float(t.item()))
+        assert float(x[0].item()) == float(world), "all-reduce result"
+        rows.append((world, backend, nbytes, float(np.median(per)), float(np.min(per))))
+    if rank == 0:
+        with open(out_path, "w", newline="") as f:
+            w = csv.writer(f)
+            w.writerow(ALLREDUCE_COLUMNS)
+            for r in rows:
+                w.writerow([r[0], r[1], r[2], "%.3f" % r[3], "%.3f" % r[4]])
+        print(f"wrote {out_path}: {len(rows)} sizes, world {world}, backend {backend}")
+    dist.destroy_process_group()
+    return 0
+
+
+def read_allreduce(path: str):
+    """Rows of a measure-allreduce CSV taken with NCCL (the CPU plumbing check's gloo rows never enter a fit)."""
+    if not os.path.exists(path):
+        return []
+    with open(path, newline="") as f:
+        return [dict(world=int(r["world"]), bytes=float(r["bytes"]), us=float(r["us_median"]))
+                for r in csv.DictReader(f) if r["backend"] == "nccl"]
+
+
+def fit_allreduce(rows):
+    """ar0_us + ar_us_per_byte x bytes, least squares on relative errors, both coefficients >= 0."""
+    from scipy.optimize import nnls
+    b = np.array([r["bytes"] for r in rows])
+    t = np.array([r["us"] for r in rows])
+    A = np.stack([np.ones_like(b), b], axis=1) / t[:, None]
+    theta, _ = nnls(A, np.ones_like(t))
+    rel = np.abs(A @ theta - 1.0)
+    return theta, dict(n=len(rows), mape=float(rel.mean()), max=float(rel.max()))
+
+
 def fit(grid_path: str, write: bool, gemm_path: str = None):
     rows = read_grid(grid_path)
     shapes = sorted({(r["Hq"], r["Hkv"], r["d"]) for r in rows})
@@ -385,8 +488,18 @@ def fit(grid_path: str, write: bool, gemm_path: str = None):
     lin = ["// Generated by `python -m paper_2606_16264_b200.cost_fit fit` from calibration/b200_gemm.csv.",
            "// {g0_us, f_us_per_flop, w_us_per_byte, kappa, ar0_us, ar_us_per_byte}; held-out MAPE %.1f %%, max %.1f %%;"
            % (100 * st_l["mape_held"], 100 * st_l["max_held"]),
-           "// all-reduce coefficients 0: not measurable on one GPU (DESIGN.md section 7).",
-           "{%.6g, %.6g, %.6g, %.6g, 0, 0}" % tuple(theta_l)]
+           ]
+    ar_rows = read_allreduce(ALLREDUCE_GRID)
+    if ar_rows:
+        theta_a, st_a = fit_allreduce(ar_rows)
+        print(f"all-reduce: theta={['%.4g' % t for t in theta_a]} {st_a}")
+        lin.append("// all-reduce coefficients from calibration/b200_allreduce.csv (world %d, NCCL): MAPE %.1f %%, max %.1f %%."
+                   % (ar_rows[0]["world"], 100 * st_a["mape"], 100 * st_a["max"]))
+        lin.append("{%.6g, %.6g, %.6g, %.6g, %.6g, %.6g}" % (*theta_l, *theta_a))
+    else:
+        lin.append("// all-reduce coefficients 0: not measurable on one GPU (DESIGN.md section 7); `cost_fit measure-allreduce`")
+        lin.append("// on a box with two GPUs writes calibration/b200_allreduce.csv, and the next `fit` fills them in.")
+        lin.append("{%.6g, %.6g, %.6g, %.6g, 0, 0}" % tuple(theta_l))
     if write:
         with open(FIT_INC, "w") as f:
             f.write("\n".join(lines) + "\n")
@@ -409,6 +522,12 @@ def main(argv=None):
     mg = sub.add_parser("measure-gemm")
     mg.add_argument("--out", default=GEMM_GRID)
     mg.add_argument("--iters", type=int, default=20)
+    ma = sub.add_parser("measure-allreduce")
+    ma.add_argument("--out", default=ALLREDUCE_GRID)
+    ma.add_argument("--iters", type=int, default=20)
+    ma.add_argument("--world", type=int, default=2, help="ranks = GPUs (the paper's workers run TP = 2, P:184)")
+    ma.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="gloo: CPU plumbing check, ignored by fit")
+    ma.add_argument("--max-tokens", type=int, default=8192)
     f = sub.add_parser("fit")
     f.add_argument("--grid", default=DEFAULT_GRID)
     f.add_argument("--no-write", action="store_true")
@@ -421,6 +540,8 @@ def main(argv=None):
         sweep_split(a.out, a.iters, shapes)
     elif a.cmd == "measure-gemm":
         measure_gemm(a.out, a.iters)
+    elif a.cmd == "measure-allreduce":
+        return measure_allreduce(a.out, a.iters, a.world, a.backend, a.max_tokens)
     else:
         fit(a.grid, not a.no_write)
 

@@ -93,3 +93,30 @@ def test_bench_refuses_more_gpus_than_visible():
                          capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
     assert res.returncode == 2 and "refusing" in res.stderr
     assert not [l for l in res.stdout.splitlines() if l.startswith("{")]
+
+
+def test_measure_allreduce_command_runs_two_ranks_and_its_fit_recovers_a_line(tmp_path):
+    """NEXT-4 (TP = 2 inside a worker): the command that will measure the all-reduce term on the first box with
+    two GPUs, driven here over gloo on CPU tensors (same launcher, same loop, same CSV); its rows are marked gloo and the
+    fit ignores them.  The fit itself is checked on made-up NCCL rows that lie on a known line."""
+    import csv
+    import subprocess
+    from paper_2606_16264_b200 import cost_fit
+    out = tmp_path / "ar.csv"
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, "-m", "paper_2606_16264_b200.cost_fit", "measure-allreduce", "--backend", "gloo",
+                          "--out", str(out), "--iters", "2", "--max-tokens", "4"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert res.returncode == 0, res.stderr[-2000:]
+    rows = list(csv.DictReader(open(out)))
+    assert [int(r["bytes"]) for r in rows] == cost_fit.allreduce_sizes(4) and len(rows) == 7   # 3 hidden sizes x T = 1, 2, 4, merged
+    assert all(r["world"] == "2" and r["backend"] == "gloo" and float(r["us_median"]) > 0 for r in rows)
+    assert cost_fit.read_allreduce(str(out)) == []                     # never enters a fit
+    # asking for the NCCL measurement without two GPUs is refused, not degraded
+    if not (torch.cuda.is_available() and torch.cuda.device_count() >= 2):
+        res = subprocess.run([sys.executable, "-m", "paper_2606_16264_b200.cost_fit", "measure-allreduce", "--out", str(out)],
+                             capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+        assert res.returncode == 2 and "GPUs needed" in res.stderr
+    made_up = [dict(world=2, bytes=float(b), us=9.0 + 2.5e-6 * b) for b in cost_fit.allreduce_sizes(8192)]
+    theta, st = cost_fit.fit_allreduce(made_up)
+    assert theta[0] == pytest.approx(9.0, rel=1e-6) and theta[1] == pytest.approx(2.5e-6, rel=1e-6) and st["max"] < 1e-9
