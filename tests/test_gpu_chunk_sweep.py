@@ -56,4 +56,4 @@ def test_chunk_cost_grows_with_chunk_index_and_matches_oracle():
     assert all(b > a for a, b in zip(times, times[1:])), times      # measured: later chunks cost more
     assert all(b > a for a, b in zip(preds, preds[1:])), preds      # and the predictor says so too
     for t, p in zip(times, preds):
-        assert abs(p - t) / t <= 0.35, (times, preds)
+        assert abs(p - t) / t <= 0.25, (times, preds)   # the survey's per-point bar; first measured margins: +5 .. +14 %
