@@ -4,7 +4,8 @@ acts on predicted step times).  The built-in step-cost fits were made from a gri
 no grid line -- three native head shapes, both kernel variants of tropical_mixed_step -- are timed through the product
 call and compared with tropical_step_cost.  Boxes of this pool differ by ~6 % (clocks, HBM stacks): the comparison is
 made on ratios to a decode-only anchor step measured in the same test on the same shape.
-Bars: SURVEY.md 8(c) step-cost model: mean absolute percentage error <= 10 %, every point within 25 %."""
+Bars: SURVEY.md 8(c) step-cost model: mean absolute percentage error <= 10 %, every point within 25 %.
+The file name sorts after the parity tests on purpose: this is a timing test, and pytest -x must not let a slow box hide them."""
 import numpy as np
 import pytest
 
